@@ -1,0 +1,241 @@
+/* oracle/mm_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, fp64 CPU statement of the bound-motor microscale substep of Cook & Shinar
+ * (arxiv 1908.04279), in the re-parametrised form BASELINE.json `north_star` names:
+ * density m over configuration c=(x,y,theta) x arc length s x stalk offset (xi,eta).
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may build, load or call this file.  It shares no code with paper_1908_04279_b200/.
+ *
+ * The method is an explicit iteration, so the oracle IS the algorithm, step by step, as
+ * literal loops in flux-difference form, in the order of SURVEY.md section 8(c) S1..S9:
+ *   - motor equation  d_t M_b + d_s M_b = -k_off M_b + k_on M_f 1_{D_rc}   PAPER.md:60 (Eq. 4)
+ *   - capture-radius restriction |x + s p - r0| <= r_c
+ *   - per-unit explicit update, units independent                          PAPER.md:91, Alg. 2
+ *   - motor force / reduction per unit                                     PAPER.md:80-81 (Eq. 10), Alg. 2 l.14 PAPER.md:206-208
+ *   - force-dependent walking speed, head-relative-to-tail advection in (xi,eta), Bell
+ *     detachment, end detachment, spring-force moments: BASELINE.json north_star (1)-(3).
+ * The paper prints no discretisation; every reading (Q1..Q23) is listed in DESIGN.md.
+ *
+ * Parity pins (tests/test_oracle_pins.py): C1 mass conservation, C1b discrete mass budget,
+ * C2 pure detachment closed form, C3 exact shift at CFL=1, C4 steady-state recursion,
+ * C5 brute-force/analytic moments on 2x2x2x4x3x3, C6 single-cell delta column, C7 point
+ * symmetry, C8 independence/additivity, C9 positivity/affinity.  No function is unpinned.
+ *
+ * Parallelism: `#pragma omp parallel for` over configurations only (they never interact).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct { int32_t nx, ny, ntheta, ns, nxi, neta; } mmo_grid;
+
+typedef struct {
+    double v0, f_stall, k_spring, k_on, k_off0, f_detach, end_detach_mult, m_free, R;
+    double s_lo, s_hi;
+    int32_t n_end_cells;
+    uint32_t flags;
+} mmo_params;
+
+#define MMO_S_PERIODIC 1u
+#define MMO_OFFSET_PERIODIC_NOMASK 2u
+
+static const double MMO_PI = 3.14159265358979323846264338327950288;
+
+/* S1: exact integer disc test  xi_a^2 + eta_b^2 <= R^2  at cell centres */
+static int inside(const mmo_grid *g, const mmo_params *p, int a, int b)
+{
+    if (p->flags & MMO_OFFSET_PERIODIC_NOMASK) return 1;
+    int64_t u = 2 * (int64_t)a + 1 - g->nxi, v = 2 * (int64_t)b + 1 - g->neta;
+    int64_t nx2 = (int64_t)g->nxi * g->nxi, ne2 = (int64_t)g->neta * g->neta;
+    return u * u * ne2 + v * v * nx2 <= nx2 * ne2;
+}
+
+/* S3: walking speed, linear force-velocity law clamped below at 0 (Q5, Q6) */
+static double walk_speed(const mmo_params *p, double ct, double st, double xi, double eta)
+{
+    double load = p->k_spring * (xi * ct + eta * st) / p->f_stall;
+    double f = 1.0 - load;
+    return p->v0 * (f > 0.0 ? f : 0.0);
+}
+
+static double dmax(double a, double b) { return a > b ? a : b; }
+static double dmin(double a, double b) { return a < b ? a : b; }
+
+/* One explicit substep (S2..S7) of ONE configuration.
+ * m, mnew: [ns][nxi][neta], b fastest.  scratch: 3 flux arrays (sizes below). */
+static void substep_config(const mmo_grid *g, const mmo_params *p, int itheta,
+                           double U, double V, double Om, double dt,
+                           const double *m, double *mnew,
+                           double *Fs, double *Fxi, double *Feta)
+{
+    const int ns = g->ns, nxi = g->nxi, neta = g->neta;
+    const int per_s = (p->flags & MMO_S_PERIODIC) != 0;
+    const int per_o = (p->flags & MMO_OFFSET_PERIODIC_NOMASK) != 0;
+    const double R = p->R;
+    const double ds = (p->s_hi - p->s_lo) / ns, dxi = 2.0 * R / nxi, deta = 2.0 * R / neta;
+    /* S1/S2 */
+    const double theta = 2.0 * MMO_PI * (double)itheta / (double)g->ntheta;
+    const double ct = cos(theta), st = sin(theta);
+#define M(j, a, b) m[((size_t)(j) * nxi + (a)) * neta + (b)]
+    /* S5, s-faces.  Fs index jf = 0..ns  is the face s_{jf - 1/2}; upwind cell is jf-1 (W >= 0). */
+#define FS(jf, a, b) Fs[((size_t)(jf) * nxi + (a)) * neta + (b)]
+    for (int a = 0; a < nxi; ++a)
+        for (int b = 0; b < neta; ++b) {
+            double xi = -R + (a + 0.5) * dxi, eta = -R + (b + 0.5) * deta;
+            double W = walk_speed(p, ct, st, xi, eta);            /* S4: W[c,a,b] */
+            for (int jf = 1; jf <= ns; ++jf) FS(jf, a, b) = W * M(jf - 1, a, b);
+            FS(0, a, b) = per_s ? FS(ns, a, b) : 0.0;             /* zero inflow at s = s_lo (Q9) */
+        }
+    /* S5, xi-faces.  index af = 0..nxi is the face xi_{af - 1/2} = -R + af*dxi. */
+#define FXI(j, af, b) Fxi[((size_t)(j) * (nxi + 1) + (af)) * neta + (b)]
+    for (int j = 0; j < ns; ++j) {
+        double sj = p->s_lo + (j + 0.5) * ds;
+        for (int af = 0; af <= nxi; ++af)
+            for (int b = 0; b < neta; ++b) {
+                if (per_o && af == nxi) { FXI(j, af, b) = FXI(j, 0, b); continue; }  /* ONE wrapped face */
+                double xif = -R + af * dxi, eta = -R + (b + 0.5) * deta;
+                double A = U + walk_speed(p, ct, st, xif, eta) * ct - sj * Om * st;   /* S4: A_xi */
+                double mL, mR;
+                if (per_o) {
+                    mL = M(j, (af - 1 + nxi) % nxi, b);
+                    mR = M(j, af % nxi, b);
+                } else {
+                    mL = af >= 1 ? M(j, af - 1, b) : 0.0;        /* ghost = 0 (Q10) */
+                    mR = af < nxi ? M(j, af, b) : 0.0;
+                }
+                FXI(j, af, b) = dmax(A, 0.0) * mL + dmin(A, 0.0) * mR;
+            }
+    }
+    /* S5, eta-faces.  index bf = 0..neta is the face eta_{bf - 1/2} = -R + bf*deta. */
+#define FETA(j, a, bf) Feta[((size_t)(j) * nxi + (a)) * (neta + 1) + (bf)]
+    for (int j = 0; j < ns; ++j) {
+        double sj = p->s_lo + (j + 0.5) * ds;
+        for (int a = 0; a < nxi; ++a)
+            for (int bf = 0; bf <= neta; ++bf) {
+                if (per_o && bf == neta) { FETA(j, a, bf) = FETA(j, a, 0); continue; }
+                double xi = -R + (a + 0.5) * dxi, etaf = -R + bf * deta;
+                double A = V + walk_speed(p, ct, st, xi, etaf) * st + sj * Om * ct;   /* S4: A_eta */
+                double mL, mR;
+                if (per_o) {
+                    mL = M(j, a, (bf - 1 + neta) % neta);
+                    mR = M(j, a, bf % neta);
+                } else {
+                    mL = bf >= 1 ? M(j, a, bf - 1) : 0.0;
+                    mR = bf < neta ? M(j, a, bf) : 0.0;
+                }
+                FETA(j, a, bf) = dmax(A, 0.0) * mL + dmin(A, 0.0) * mR;
+            }
+    }
+    /* S6 + S7 */
+    for (int j = 0; j < ns; ++j) {
+        double E = (j < p->n_end_cells || j >= ns - p->n_end_cells) ? p->end_detach_mult : 1.0;  /* Q8 */
+        for (int a = 0; a < nxi; ++a)
+            for (int b = 0; b < neta; ++b) {
+                double xi = -R + (a + 0.5) * dxi, eta = -R + (b + 0.5) * deta;
+                double r = sqrt(xi * xi + eta * eta);
+                double kappa = p->k_off0 * exp(p->k_spring * r / p->f_detach) * E;     /* Bell law (Q7) */
+                int in = inside(g, p, a, b);
+                double src = in ? p->k_on * p->m_free : 0.0;                           /* Q11 */
+                double mc = M(j, a, b);
+                double div = (FS(j + 1, a, b) - FS(j, a, b)) / ds
+                           + (FXI(j, a + 1, b) - FXI(j, a, b)) / dxi
+                           + (FETA(j, a, b + 1) - FETA(j, a, b)) / deta;
+                double mp = mc - dt * div + dt * (src - kappa * mc);
+                mnew[((size_t)j * nxi + a) * neta + b] = in ? mp : 0.0;
+            }
+    }
+#undef M
+#undef FS
+#undef FXI
+#undef FETA
+}
+
+static size_t scratch_doubles(const mmo_grid *g)
+{
+    size_t ns = g->ns, nxi = g->nxi, neta = g->neta;
+    return (ns + 1) * nxi * neta + ns * (nxi + 1) * neta + ns * nxi * (neta + 1) + ns * nxi * neta;
+}
+
+/* Advance configurations [0, n_configs) by n_sub substeps of size dt, in place.
+ * m: [n_configs][ns][nxi][neta]; U,V,Om: [n_configs]; itheta0: theta index of the first
+ * configuration is (c_first % ntheta) where c_first is the global index of m's first config. */
+int mmo_run(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
+            const double *U, const double *V, const double *Om,
+            double *m, int32_t n_sub, double dt)
+{
+    const size_t inner = (size_t)g->ns * g->nxi * g->neta;
+    int fail = 0;
+#pragma omp parallel for schedule(static)
+    for (int64_t c = 0; c < n_configs; ++c) {
+        double *scr = (double *)malloc(sizeof(double) * scratch_doubles(g));
+        if (!scr) { fail = 1; continue; }
+        double *Fs = scr;
+        double *Fxi = Fs + (size_t)(g->ns + 1) * g->nxi * g->neta;
+        double *Feta = Fxi + (size_t)g->ns * (g->nxi + 1) * g->neta;
+        double *tmp = Feta + (size_t)g->ns * g->nxi * (g->neta + 1);
+        double *cur = m + (size_t)c * inner;
+        int itheta = (int)((c_first + c) % g->ntheta);
+        for (int n = 0; n < n_sub; ++n) {
+            substep_config(g, p, itheta, U[c], V[c], Om[c], dt, cur, tmp, Fs, Fxi, Feta);
+            memcpy(cur, tmp, sizeof(double) * inner);   /* "swap buffers" */
+        }
+        free(scr);
+    }
+    return fail ? -1 : 0;
+}
+
+/* S9: per-configuration moments; force [n][2], torque [n]; optional (may be NULL) test-only
+ * cancellation-free scales N0 = dV sum m, SF = k dV sum r m, Stau = k dV sum |s| r m. */
+int mmo_moments(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
+                const double *m, double *force, double *torque,
+                double *N0, double *SF, double *Stau)
+{
+    const int ns = g->ns, nxi = g->nxi, neta = g->neta;
+    const double R = p->R, k = p->k_spring;
+    const double ds = (p->s_hi - p->s_lo) / ns, dxi = 2.0 * R / nxi, deta = 2.0 * R / neta;
+    const double dV = ds * dxi * deta;
+    const size_t inner = (size_t)ns * nxi * neta;
+#pragma omp parallel for schedule(static)
+    for (int64_t c = 0; c < n_configs; ++c) {
+        int itheta = (int)((c_first + c) % g->ntheta);
+        double theta = 2.0 * MMO_PI * (double)itheta / (double)g->ntheta;
+        double ct = cos(theta), st = sin(theta);
+        double sx = 0.0, sy = 0.0, stq = 0.0, s0 = 0.0, sf = 0.0, sta = 0.0;
+        const double *mc = m + (size_t)c * inner;
+        for (int j = 0; j < ns; ++j) {
+            double sj = p->s_lo + (j + 0.5) * ds;
+            for (int a = 0; a < nxi; ++a)
+                for (int b = 0; b < neta; ++b) {
+                    double xi = -R + (a + 0.5) * dxi, eta = -R + (b + 0.5) * deta;
+                    double v = mc[((size_t)j * nxi + a) * neta + b];
+                    double r = sqrt(xi * xi + eta * eta);
+                    sx += xi * v;
+                    sy += eta * v;
+                    stq += sj * (eta * ct - xi * st) * v;
+                    s0 += v;
+                    sf += r * v;
+                    sta += fabs(sj) * r * v;
+                }
+        }
+        force[2 * c + 0] = -k * dV * sx;
+        force[2 * c + 1] = -k * dV * sy;
+        torque[c] = -k * dV * stq;
+        if (N0) N0[c] = dV * s0;
+        if (SF) SF[c] = k * dV * sf;
+        if (Stau) Stau[c] = k * dV * sta;
+    }
+    return 0;
+}
+
+int mmo_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,109 @@
+"""ctypes wrapper of oracle/mm_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It imports nothing from paper_1908_04279_b200/ or mm_inputs/.
+See mm_oracle.c's header for the passages followed (Eq. 4, PAPER.md:43,
+PAPER.md:80-81 Eq. 10, Alg. 2; BASELINE.json north_star (1)-(3)).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "mm_oracle.c")
+_SO = os.path.join(_HERE, "libmm_oracle.so")
+_lib = None
+
+S_PERIODIC = 1
+OFFSET_PERIODIC_NOMASK = 2
+
+
+class OGrid(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("nx", "ny", "ntheta", "ns", "nxi", "neta")]
+
+
+class OParams(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_double) for n in
+                ("v0", "f_stall", "k_spring", "k_on", "k_off0", "f_detach", "end_detach_mult", "m_free", "R",
+                 "s_lo", "s_hi")] + [("n_end_cells", ctypes.c_int32), ("flags", ctypes.c_uint32)]
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -fopenmp, no -ffast-math."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-ffp-contract=off",
+                               "-o", _SO, _SRC, "-lm"])
+    return _SO
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_SO)
+        vp, i64, i32, dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double
+        lib.mmo_run.restype = ctypes.c_int
+        lib.mmo_run.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, dbl]
+        lib.mmo_moments.restype = ctypes.c_int
+        lib.mmo_moments.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp, vp]
+        lib.mmo_threads.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def _grid(grid) -> OGrid:
+    return OGrid(*(int(getattr(grid, n)) for n in ("nx", "ny", "ntheta", "ns", "nxi", "neta")))
+
+
+def _params(p) -> OParams:
+    return OParams(*(float(getattr(p, n)) for n in
+                     ("v0", "f_stall", "k_spring", "k_on", "k_off0", "f_detach", "end_detach_mult", "m_free", "R",
+                      "s_lo", "s_hi")), int(p.n_end_cells), int(p.flags))
+
+
+def _f64(x, n=None):
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    if n is not None:
+        assert x.size == n, (x.size, n)
+    return x
+
+
+def threads() -> int:
+    return _load().mmo_threads()
+
+
+def run(grid, params, U, V, Om, m, n_sub: int, dt: float, c_first: int = 0) -> np.ndarray:
+    """n_sub explicit substeps (S2-S7) of the configurations held in ``m``.
+
+    m: [n][ns][nxi][neta] (any float dtype; promoted to fp64, Q18); U,V,Om: [n], the velocities of
+    exactly these configurations; c_first = global index of the first one (fixes theta).  Returns a
+    new fp64 array."""
+    lib = _load()
+    g, p = _grid(grid), _params(params)
+    inner = grid.ns * grid.nxi * grid.neta
+    out = np.array(m, dtype=np.float64, order="C", copy=True)
+    n = out.size // inner
+    assert out.size == n * inner
+    U, V, Om = _f64(U, n), _f64(V, n), _f64(Om, n)
+    rc = lib.mmo_run(ctypes.byref(g), ctypes.byref(p), c_first, n, U.ctypes.data, V.ctypes.data, Om.ctypes.data,
+                     out.ctypes.data, n_sub, dt)
+    if rc != 0:
+        raise MemoryError("oracle scratch allocation failed")
+    return out.reshape(n, grid.ns, grid.nxi, grid.neta)
+
+
+def moments(grid, params, m, c_first: int = 0):
+    """S9.  Returns dict(force[n,2], torque[n], N0[n], SF[n], Stau[n])."""
+    lib = _load()
+    g, p = _grid(grid), _params(params)
+    inner = grid.ns * grid.nxi * grid.neta
+    m = _f64(m)
+    n = m.size // inner
+    force = np.empty((n, 2)); torque = np.empty(n); N0 = np.empty(n); SF = np.empty(n); St = np.empty(n)
+    lib.mmo_moments(ctypes.byref(g), ctypes.byref(p), c_first, n, m.ctypes.data, force.ctypes.data,
+                    torque.ctypes.data, N0.ctypes.data, SF.ctypes.data, St.ctypes.data)
+    return dict(force=force, torque=torque, N0=N0, SF=SF, Stau=St)
