@@ -1,0 +1,141 @@
+/* mm.h -- C ABI of libmm: the GPU-resident bound-motor microscale step (sm_100a).
+ *
+ * What it computes.  The microscale half of the micro-macro gliding-assay model of Cook & Shinar
+ * (arxiv 1908.04279): the bound-motor density M_b of Eq. 4,
+ *      d_t M_b + d_s M_b = -k_off M_b + k_on M_f 1_{D_rc},
+ * restricted to the capture disc |x + s p - r0| <= r_c, advanced by many explicit
+ * substeps that stay resident on the GPU between macro steps (section 3.1 PAPER.md:131-145,
+ * Algorithm 2), followed by the per-unit reduction the macroscale consumes
+ * (Eq. 10; Alg. 2 l.14 PAPER.md:206-208).  The density is parametrised as
+ * BASELINE.json `north_star` states: configuration c = (x, y, theta) x arc length s x stalk offset
+ * (xi, eta) = head - tail; one substep = (1) conservative first-order upwind advection in s at the
+ * force-dependent walking speed and in (xi, eta) at the head's velocity relative to the anchored
+ * tail, (2) Bell-law detachment with enhanced end detachment + uniform attachment inside the disc,
+ * and on request (3) the spring-force moments per configuration.  The exact discrete formulas
+ * (S1-S9) and every reading of the paper are listed in DESIGN.md.
+ *
+ * Conventions.
+ *  - Plain C, no C++ types, nothing throws across the boundary.  Every call returns an mm_status
+ *    (0 = success, negative = error); mm_last_error(ctx) gives a message for the last failure.
+ *  - "device pointer" = CUDA device memory of the CURRENT device; "host pointer" = ordinary or
+ *    pinned host memory.  Arguments named *_on_device say which one a void* is.
+ *  - Canonical density layout: [ix][iy][itheta][j][a][b], b (eta index) fastest; element type is the
+ *    context's dtype.  Configuration index c = (ix*ny + iy)*ntheta + itheta, Nc = nx*ny*ntheta.
+ *    Flat indices are 64-bit: more than 2^32 elements are supported.
+ *  - All work is enqueued on the cudaStream_t given to mm_create.  Calls with device destinations
+ *    are stream-ordered and do not synchronise; calls with host sources/destinations synchronise
+ *    that stream before returning.
+ *  - A handle is not thread-safe; distinct handles are independent.
+ *  - There is no CPU fallback: without a CUDA device every compute call fails with MM_ERR_CUDA.
+ */
+#ifndef MM_H_
+#define MM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mm_ctx mm_ctx; /* opaque */
+
+typedef enum { MM_F32 = 0, MM_F64 = 1 } mm_dtype;
+
+typedef enum {
+    MM_OK = 0,
+    MM_ERR_INVALID_ARG = -1, /* NULL pointer, bad dimension, non-finite or out-of-range parameter */
+    MM_ERR_CUDA = -2,        /* a CUDA runtime call or kernel launch failed (message in mm_last_error) */
+    MM_ERR_NOMEM = -3,       /* host or device allocation failed */
+    MM_ERR_STATE = -4,       /* substep/moments before density and velocities were set */
+    MM_ERR_UNSTABLE = -5     /* MM_FLAG_CHECK_DT set and dt violates the positivity bound (S8) */
+} mm_status;
+
+/* Grid sizes.  (x, y) periodic labels; theta_k = 2 pi k / ntheta; s, xi, eta cell
+ * centred: s_j = s_lo + (j+1/2) ds, xi_a = -R + (a+1/2) 2R/nxi, eta_b likewise. */
+typedef struct {
+    int32_t nx, ny, ntheta, ns, nxi, neta;
+} mm_grid;
+
+#define MM_FLAG_S_PERIODIC 1u              /* test-only: s wraps (default: zero inflow at s_lo, walk-off at s_hi) */
+#define MM_FLAG_OFFSET_PERIODIC_NOMASK 2u  /* test-only: (xi, eta) wrap and the disc mask is off */
+#define MM_FLAG_CHECK_DT 4u                /* mm_substep returns MM_ERR_UNSTABLE when dt breaks the S8 bound */
+
+/* Model parameters (BASELINE.json configs[0] gives the benchmark values in brackets). */
+typedef struct {
+    double v0;              /* unloaded walking speed                                   [1]   */
+    double f_stall;         /* stall force of the linear force-velocity law, > 0        [6]   */
+    double k_spring;        /* stalk spring constant k, >= 0                            [50]  */
+    double k_on;            /* attachment rate, >= 0                                    [5]   */
+    double k_off0;          /* unloaded detachment rate, >= 0                           [1]   */
+    double f_detach;        /* Bell force scale f_d, > 0                                [2]   */
+    double end_detach_mult; /* detachment multiplier in the n_end_cells outermost s cells [10] */
+    double m_free;          /* unbound source density M_f (constant on this path)       [1]   */
+    double R;               /* capture radius r_c; offsets live on [-R, R]^2, > 0       [0.1] */
+    double s_lo, s_hi;      /* arc-length interval, s_hi > s_lo                         [-0.5, 0.5] */
+    int32_t n_end_cells;    /* >= 0, 2*n_end_cells <= ns                                [1]   */
+    uint32_t flags;         /* MM_FLAG_*                                                [0]   */
+} mm_params;
+
+/* Tuning / test options for mm_set_option.  Defaults are what bench.py times. */
+typedef enum {
+    MM_OPT_KERNEL = 0,       /* 0 auto (default); 1 force the generic global-memory kernels;
+                                2 force the warp-streamed TMA kernels (error if the grid is unsupported) */
+    MM_OPT_FUSE_T = 1,       /* max substeps fused per HBM pass by the streamed kernel, 1..MM_MAX_FUSE_T */
+    MM_OPT_FUSE_MOMENTS = 2  /* 1 (default): the last pass of mm_substep also reduces the moments, so a
+                                following mm_moments is a copy; 0: mm_moments always runs its own pass */
+} mm_option;
+#define MM_MAX_FUSE_T 4
+
+/* Create a context.
+ *  grid, params : copied.  Invalid (MM_ERR_INVALID_ARG): any dim < 1, R <= 0, f_stall <= 0,
+ *                 f_detach <= 0, s_hi <= s_lo, negative rates/speeds, 2*n_end_cells > ns, non-finite.
+ *  dens_buf0/1  : device pointers to two density buffers of >= cells*sizeof(real) bytes each,
+ *                 16-byte aligned, BORROWED (must outlive the context; e.g. torch tensors).  Pass
+ *                 NULL, NULL and the library allocates and owns them (MM_ERR_NOMEM on failure).
+ *                 Passing exactly one NULL is invalid.
+ *  cuda_stream  : a cudaStream_t (NULL = the legacy default stream).
+ *  out          : receives the handle.  On error *out is NULL. */
+mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_dtype dtype,
+                    void *dens_buf0, void *dens_buf1, void *cuda_stream, mm_ctx **out);
+
+/* Upload / download the whole density in canonical layout and the context's dtype.
+ * src/dst hold cells elements.  mm_get_density returns the state after the last completed substep. */
+mm_status mm_set_density(mm_ctx *ctx, const void *src, int src_on_device);
+mm_status mm_get_density(mm_ctx *ctx, void *dst, int dst_on_device);
+
+/* Same for a contiguous range of configurations [c_begin, c_begin + n_configs): lets a caller stream
+ * a density that is larger than host memory (checkpoint/restart primitive).  After every
+ * configuration has been covered by set calls the density counts as set. */
+mm_status mm_set_density_range(mm_ctx *ctx, int64_t c_begin, int64_t n_configs, const void *src, int src_on_device);
+mm_status mm_get_density_range(mm_ctx *ctx, int64_t c_begin, int64_t n_configs, void *dst, int dst_on_device);
+
+/* Per-configuration filament velocities (U, V, Omega), Nc elements each, index c, context dtype
+ * (the macro-timescale input; "Psi ... is transferred as before"). */
+mm_status mm_set_filament_velocity(mm_ctx *ctx, const void *U, const void *V, const void *Omega, int on_device);
+
+/* n_sub explicit substeps of size dt (S2-S7), asynchronous on the stream.  n_sub >= 0; dt > 0 and finite
+ * when n_sub > 0.  MM_ERR_STATE unless density and velocities have been set. */
+mm_status mm_substep(mm_ctx *ctx, int32_t n_sub, double dt);
+
+/* Moments (S9) of the current density: force [Nc][2] = (Fx, Fy), torque [Nc]; always fp64
+ * (macroscale data stays double precision).  Either pointer may be NULL to skip it. */
+mm_status mm_moments(mm_ctx *ctx, double *force, double *torque, int dst_on_device);
+
+mm_status mm_set_option(mm_ctx *ctx, mm_option opt, int64_t value);
+
+/* Number of kernels this context has launched so far (bench.py's gpu_launches). */
+int64_t mm_launch_count(const mm_ctx *ctx);
+/* Name of the substep kernel variant the last mm_substep used ("stream<f64,16x16,T=2>", "generic<f64>", ...). */
+const char *mm_kernel_name(const mm_ctx *ctx);
+
+/* Destroy; frees library-owned buffers.  NULL is a no-op.  Does not synchronise borrowed buffers' users
+ * beyond the context's own stream. */
+mm_status mm_destroy(mm_ctx *ctx);
+
+const char *mm_status_string(mm_status s);
+const char *mm_last_error(const mm_ctx *ctx); /* "" if none; ctx may be NULL (returns the create-time error) */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MM_H_ */

@@ -1,0 +1,176 @@
+"""Thin ctypes binding of libmm (include/mm.h).  Argument marshalling only: every step of the hot path
+runs in the library's CUDA kernels.  PyTorch supplies device memory and the stream, nothing else.
+
+There is no CPU fallback: if libmm.so cannot be loaded, or no CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+MM_F32, MM_F64 = 0, 1
+MM_OK, MM_ERR_INVALID_ARG, MM_ERR_CUDA, MM_ERR_NOMEM, MM_ERR_STATE, MM_ERR_UNSTABLE = 0, -1, -2, -3, -4, -5
+MM_FLAG_S_PERIODIC, MM_FLAG_OFFSET_PERIODIC_NOMASK, MM_FLAG_CHECK_DT = 1, 2, 4
+MM_OPT_KERNEL, MM_OPT_FUSE_T, MM_OPT_FUSE_MOMENTS = 0, 1, 2
+MM_MAX_FUSE_T = 4
+
+EXPORTS = ["mm_create", "mm_set_density", "mm_get_density", "mm_set_density_range", "mm_get_density_range",
+           "mm_set_filament_velocity", "mm_substep", "mm_moments", "mm_set_option", "mm_launch_count",
+           "mm_kernel_name", "mm_destroy", "mm_status_string", "mm_last_error"]
+
+
+class mm_grid(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("nx", "ny", "ntheta", "ns", "nxi", "neta")]
+
+
+class mm_params(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_double) for n in
+                ("v0", "f_stall", "k_spring", "k_on", "k_off0", "f_detach", "end_detach_mult", "m_free", "R",
+                 "s_lo", "s_hi")] + [("n_end_cells", ctypes.c_int32), ("flags", ctypes.c_uint32)]
+
+
+class MMError(RuntimeError):
+    def __init__(self, status: int, name: str, msg: str):
+        super().__init__(f"{name} ({status}): {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib():
+    """Load libmm.so (building it in-tree first if the sources are newer).  Raises if impossible."""
+    global _lib
+    if _lib is None:
+        so = _build.SO
+        if not _build.up_to_date():
+            so = _build.build()
+        L = ctypes.CDLL(so)
+        vp, i32, i64, dbl = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+        L.mm_create.argtypes = [ctypes.POINTER(mm_grid), ctypes.POINTER(mm_params), ctypes.c_int, vp, vp, vp,
+                                ctypes.POINTER(vp)]
+        L.mm_set_density.argtypes = [vp, vp, ctypes.c_int]
+        L.mm_get_density.argtypes = [vp, vp, ctypes.c_int]
+        L.mm_set_density_range.argtypes = [vp, i64, i64, vp, ctypes.c_int]
+        L.mm_get_density_range.argtypes = [vp, i64, i64, vp, ctypes.c_int]
+        L.mm_set_filament_velocity.argtypes = [vp, vp, vp, vp, ctypes.c_int]
+        L.mm_substep.argtypes = [vp, i32, dbl]
+        L.mm_moments.argtypes = [vp, vp, vp, ctypes.c_int]
+        L.mm_set_option.argtypes = [vp, ctypes.c_int, i64]
+        L.mm_launch_count.argtypes = [vp]
+        L.mm_launch_count.restype = i64
+        L.mm_kernel_name.argtypes = [vp]
+        L.mm_kernel_name.restype = ctypes.c_char_p
+        L.mm_destroy.argtypes = [vp]
+        L.mm_status_string.argtypes = [ctypes.c_int]
+        L.mm_status_string.restype = ctypes.c_char_p
+        L.mm_last_error.argtypes = [vp]
+        L.mm_last_error.restype = ctypes.c_char_p
+        for n in EXPORTS:
+            if getattr(L, n).restype is ctypes.c_int:
+                pass
+        _lib = L
+    return _lib
+
+
+def _grid_struct(grid) -> mm_grid:
+    return mm_grid(*(int(getattr(grid, n)) for n in ("nx", "ny", "ntheta", "ns", "nxi", "neta")))
+
+
+def _params_struct(p) -> mm_params:
+    return mm_params(*(float(getattr(p, n)) for n in
+                       ("v0", "f_stall", "k_spring", "k_on", "k_off0", "f_detach", "end_detach_mult", "m_free", "R",
+                        "s_lo", "s_hi")), int(p.n_end_cells), int(p.flags))
+
+
+def _ptr(x):
+    """(address, on_device) of a torch tensor / numpy array / None."""
+    if x is None:
+        return None, 0
+    if hasattr(x, "data_ptr"):  # torch tensor
+        assert x.is_contiguous()
+        return ctypes.c_void_p(x.data_ptr()), int(x.is_cuda)
+    assert x.flags.c_contiguous  # numpy
+    return ctypes.c_void_p(x.ctypes.data), 0
+
+
+class MM:
+    """One libmm context.  Method names follow include/mm.h (mm_create -> MM(...), mm_substep -> .substep)."""
+
+    def __init__(self, grid, params, dtype: str, buf0=None, buf1=None, stream: int | None = None):
+        self._L = lib()
+        self._h = ctypes.c_void_p()
+        self.grid, self.params, self.dtype = grid, params, dtype
+        self.nc = grid.nx * grid.ny * grid.ntheta
+        self.inner = grid.ns * grid.nxi * grid.neta
+        self._keep = (buf0, buf1)  # borrowed buffers must outlive the context
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        p0, _ = _ptr(buf0)
+        p1, _ = _ptr(buf1)
+        g, p = _grid_struct(grid), _params_struct(params)
+        st = self._L.mm_create(ctypes.byref(g), ctypes.byref(p), MM_F64 if dtype == "f64" else MM_F32, p0, p1,
+                               ctypes.c_void_p(stream), ctypes.byref(self._h))
+        if st != MM_OK:
+            raise MMError(st, self._L.mm_status_string(st).decode(), self._L.mm_last_error(None).decode())
+
+    def _check(self, st: int):
+        if st != MM_OK:
+            raise MMError(st, self._L.mm_status_string(st).decode(), self._L.mm_last_error(self._h).decode())
+
+    def set_density(self, src):
+        p, dev = _ptr(src)
+        self._check(self._L.mm_set_density(self._h, p, dev))
+
+    def get_density(self, dst):
+        p, dev = _ptr(dst)
+        self._check(self._L.mm_get_density(self._h, p, dev))
+        return dst
+
+    def set_density_range(self, c_begin: int, n_configs: int, src):
+        p, dev = _ptr(src)
+        self._check(self._L.mm_set_density_range(self._h, c_begin, n_configs, p, dev))
+
+    def get_density_range(self, c_begin: int, n_configs: int, dst):
+        p, dev = _ptr(dst)
+        self._check(self._L.mm_get_density_range(self._h, c_begin, n_configs, p, dev))
+        return dst
+
+    def set_filament_velocity(self, U, V, Om):
+        (pu, d0), (pv, d1), (po, d2) = _ptr(U), _ptr(V), _ptr(Om)
+        assert d0 == d1 == d2
+        self._check(self._L.mm_set_filament_velocity(self._h, pu, pv, po, d0))
+
+    def substep(self, n_sub: int, dt: float):
+        self._check(self._L.mm_substep(self._h, int(n_sub), float(dt)))
+
+    def moments(self, force, torque):
+        (pf, d0), (pt, d1) = _ptr(force), _ptr(torque)
+        dev = d0 if force is not None else d1
+        self._check(self._L.mm_moments(self._h, pf, pt, dev))
+        return force, torque
+
+    def set_option(self, opt: int, value: int):
+        self._check(self._L.mm_set_option(self._h, opt, value))
+
+    @property
+    def launch_count(self) -> int:
+        return int(self._L.mm_launch_count(self._h))
+
+    @property
+    def kernel_name(self) -> str:
+        return self._L.mm_kernel_name(self._h).decode()
+
+    def destroy(self):
+        if self._h:
+            self._L.mm_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -1,0 +1,448 @@
+// mm_api.cu -- the C ABI of libmm (include/mm.h): context, validation, buffer ownership, kernel dispatch.
+// All arithmetic of the hot path lives in the kernels (mm_stream.cuh, mm_generic.cuh); this file only
+// marshals arguments and launches.  There is no CPU fallback.
+#include "../../include/mm.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "mm_generic.cuh"
+#include "mm_stream.cuh"
+
+using namespace mm;
+
+struct mm_ctx {
+    mm_grid g;
+    mm_params p;
+    mm_dtype dtype;
+    size_t esize;
+    int64_t nc, inner, cells;
+    cudaStream_t stream;
+    void *buf[2];
+    bool owns;
+    int cur;
+    void *U, *V, *Om;               // [nc] real
+    void *kappa, *cos_t, *sin_t;    // tables (real)
+    uint8_t *inside;
+    double *mom_force, *mom_torque; // [nc][2], [nc]
+    unsigned int *flag_dev;         // stability-check flag
+    bool mom_valid, vel_set;
+    std::vector<uint8_t> dens_cov;  // per configuration: density uploaded
+    int64_t dens_cov_count;
+    int opt_kernel, opt_fuse_t, opt_fuse_mom;
+    double checked_dt;              // dt the S8 check last passed with (NaN = none)
+    int64_t launches;
+    int sm_count;
+    std::string err;
+    char kname[64];
+};
+
+static thread_local std::string g_create_err;
+
+static mm_status fail(mm_ctx *ctx, mm_status s, const std::string &msg)
+{
+    if (ctx) ctx->err = msg; else g_create_err = msg;
+    return s;
+}
+#define CUDA_TRY(ctx, expr)                                                                          \
+    do {                                                                                             \
+        cudaError_t e_ = (expr);                                                                     \
+        if (e_ != cudaSuccess)                                                                       \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? MM_ERR_NOMEM : MM_ERR_CUDA,           \
+                        std::string(#expr) + ": " + cudaGetErrorString(e_));                         \
+    } while (0)
+
+template <typename real>
+static KParams<real> make_kparams(const mm_ctx *c, double dt)
+{
+    KParams<real> k;
+    const mm_grid &g = c->g;
+    const mm_params &p = c->p;
+    k.nc = c->nc; k.ns = g.ns; k.nxi = g.nxi; k.neta = g.neta; k.ntheta = g.ntheta;
+    k.n_end = p.n_end_cells; k.flags = p.flags;
+    const double ds = (p.s_hi - p.s_lo) / g.ns, dxi = 2.0 * p.R / g.nxi, deta = 2.0 * p.R / g.neta;
+    k.v0 = (real)p.v0; k.kload = (real)(p.k_spring / p.f_stall);
+    k.R = (real)p.R; k.dxi = (real)dxi; k.deta = (real)deta; k.ds = (real)ds; k.s_lo = (real)p.s_lo;
+    k.dt = (real)dt; k.dt_ds = (real)(dt / ds); k.dt_dxi = (real)(dt / dxi); k.dt_deta = (real)(dt / deta);
+    k.dt_src = (real)(dt * p.k_on * p.m_free);
+    k.dt_endx = (real)(dt * (p.end_detach_mult - 1.0));
+    k.mom_scale = -p.k_spring * ds * dxi * deta;
+    k.U = (const real *)c->U; k.V = (const real *)c->V; k.Om = (const real *)c->Om;
+    k.cos_t = (const real *)c->cos_t; k.sin_t = (const real *)c->sin_t;
+    k.kappa = (const real *)c->kappa; k.inside = c->inside;
+    return k;
+}
+
+// ---- S8 positivity bound (only with MM_FLAG_CHECK_DT) -----------------------------------------
+template <typename real>
+__global__ void check_dt_kernel(const __grid_constant__ KParams<real> kp, unsigned int *flag)
+{
+    const int plane = kp.nxi * kp.neta;
+    const int64_t total = kp.nc * (int64_t)kp.ns * plane;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t c = idx / ((int64_t)kp.ns * plane);
+        int rem = (int)(idx - c * (int64_t)kp.ns * plane);
+        const int j = rem / plane; rem -= j * plane;
+        const int a = rem / kp.neta, b = rem - a * kp.neta;
+        const int kth = (int)(c % kp.ntheta);
+        const double ct = kp.cos_t[kth], st = kp.sin_t[kth], U = kp.U[c], V = kp.V[c], Om = kp.Om[c];
+        const double R = kp.R, dxi = kp.dxi, deta = kp.deta;
+        const double sj = (double)kp.s_lo + (j + 0.5) * (double)kp.ds;
+        const double xi = -R + (a + 0.5) * dxi, eta = -R + (b + 0.5) * deta;
+        auto w = [&](double x, double e) { return walk_speed<double>(kp.v0, kp.kload, ct, st, x, e); };
+        const double Axh = U + w(xi + 0.5 * dxi, eta) * ct - sj * Om * st, Axl = U + w(xi - 0.5 * dxi, eta) * ct - sj * Om * st;
+        const double Aeh = V + w(xi, eta + 0.5 * deta) * st + sj * Om * ct, Ael = V + w(xi, eta - 0.5 * deta) * st + sj * Om * ct;
+        const bool endc = (j < kp.n_end) || (j >= kp.ns - kp.n_end);
+        const double kap = (double)kp.kappa[rem] * (endc ? 1.0 + (double)kp.dt_endx / (double)kp.dt : 1.0);
+        const double rate = w(xi, eta) / (double)kp.ds + (fmax(Axh, 0.0) - fmin(Axl, 0.0)) / dxi +
+                            (fmax(Aeh, 0.0) - fmin(Ael, 0.0)) / deta + kap;
+        if (!(1.0 - (double)kp.dt * rate >= 0.0)) *flag = 1u;
+    }
+}
+
+// ---- streamed-kernel dispatch -----------------------------------------------------------------
+template <typename real, int NXI, int NETA, int CB, int T, bool MOM>
+static mm_status launch_stream_inst(mm_ctx *c, double dt, const void *in, void *out)
+{
+    constexpr int P = 2, D = 3, WARPS = 4;
+    using Cfg = StreamCfg<real, NXI, NETA, CB, P, D, WARPS>;
+    auto kern = substep_stream_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS>;
+    static int blocks_per_sm = 0;
+    if (blocks_per_sm == 0) {
+        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
+        int n = 0;
+        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, Cfg::SMEM_BYTES));
+        if (n < 1) return fail(c, MM_ERR_CUDA, "streamed kernel does not fit on an SM");
+        blocks_per_sm = n;
+    }
+    int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
+    const int64_t need = (c->nc + WARPS - 1) / WARPS;
+    if (grid > need) grid = need;
+    KParams<real> kp = make_kparams<real>(c, dt);
+    kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(kp, (const real *)in, (real *)out, c->mom_force,
+                                                                      c->mom_torque);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches++;
+    snprintf(c->kname, sizeof c->kname, "stream<%s,%dx%d,CB=%d,T=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
+             CB, T, MOM ? ",mom" : "");
+    return MM_OK;
+}
+
+template <typename real, int NXI, int NETA, int CB>
+static mm_status launch_stream_shape(mm_ctx *c, int T, bool mom, double dt, const void *in, void *out)
+{
+#define MM_CASE(TT)                                                                                     \
+    case TT:                                                                                            \
+        return mom ? launch_stream_inst<real, NXI, NETA, CB, TT, true>(c, dt, in, out)                  \
+                   : launch_stream_inst<real, NXI, NETA, CB, TT, false>(c, dt, in, out);
+    switch (T) {
+        MM_CASE(1)
+        MM_CASE(2)
+        MM_CASE(3)
+        MM_CASE(4)
+    }
+#undef MM_CASE
+    return fail(c, MM_ERR_INVALID_ARG, "unsupported fuse depth");
+}
+
+static bool stream_supported(const mm_ctx *c)
+{
+    if (c->p.flags & (MM_FLAG_S_PERIODIC | MM_FLAG_OFFSET_PERIODIC_NOMASK)) return false;
+    return (c->g.nxi == 16 && c->g.neta == 16) || (c->g.nxi == 8 && c->g.neta == 8);
+}
+
+static mm_status launch_stream(mm_ctx *c, int T, bool mom, double dt, const void *in, void *out)
+{
+    const bool big = c->g.nxi == 16;
+    if (c->dtype == MM_F64)
+        return big ? launch_stream_shape<double, 16, 16, 2>(c, T, mom, dt, in, out)
+                   : launch_stream_shape<double, 8, 8, 2>(c, T, mom, dt, in, out);
+    return big ? launch_stream_shape<float, 16, 16, 4>(c, T, mom, dt, in, out)
+               : launch_stream_shape<float, 8, 8, 2>(c, T, mom, dt, in, out);
+}
+
+template <typename real>
+static mm_status launch_generic(mm_ctx *c, double dt, const void *in, void *out)
+{
+    KParams<real> kp = make_kparams<real>(c, dt);
+    int64_t blocks = (c->cells + 255) / 256;
+    const int64_t cap = (int64_t)c->sm_count * 64;
+    if (blocks > cap) blocks = cap;
+    substep_generic_kernel<real><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, (const real *)in, (real *)out);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches++;
+    snprintf(c->kname, sizeof c->kname, "generic<%s>", sizeof(real) == 8 ? "f64" : "f32");
+    return MM_OK;
+}
+
+template <typename real>
+static mm_status launch_moments(mm_ctx *c)
+{
+    KParams<real> kp = make_kparams<real>(c, 1.0);
+    int64_t blocks = c->nc;
+    const int64_t cap = (int64_t)c->sm_count * 16;
+    if (blocks > cap) blocks = cap;
+    moments_generic_kernel<real><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, (const real *)c->buf[c->cur], c->mom_force,
+                                                                          c->mom_torque);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches++;
+    return MM_OK;
+}
+
+// ---- C ABI -----------------------------------------------------------------------------------
+static bool finite_nonneg(double x) { return std::isfinite(x) && x >= 0.0; }
+
+extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_dtype dtype, void *b0, void *b1,
+                               void *cuda_stream, mm_ctx **out)
+{
+    if (out) *out = nullptr;
+    if (!grid || !params || !out) return fail(nullptr, MM_ERR_INVALID_ARG, "NULL argument");
+    const mm_grid &g = *grid;
+    const mm_params &p = *params;
+    if (g.nx < 1 || g.ny < 1 || g.ntheta < 1 || g.ns < 1 || g.nxi < 1 || g.neta < 1)
+        return fail(nullptr, MM_ERR_INVALID_ARG, "grid dimensions must be >= 1");
+    if (dtype != MM_F32 && dtype != MM_F64) return fail(nullptr, MM_ERR_INVALID_ARG, "bad dtype");
+    if (!(std::isfinite(p.R) && p.R > 0) || !(std::isfinite(p.f_stall) && p.f_stall > 0) ||
+        !(std::isfinite(p.f_detach) && p.f_detach > 0) || !finite_nonneg(p.v0) || !finite_nonneg(p.k_spring) ||
+        !finite_nonneg(p.k_on) || !finite_nonneg(p.k_off0) || !finite_nonneg(p.end_detach_mult) ||
+        !finite_nonneg(p.m_free) || !std::isfinite(p.s_lo) || !std::isfinite(p.s_hi) || !(p.s_hi > p.s_lo))
+        return fail(nullptr, MM_ERR_INVALID_ARG, "parameter out of range or not finite");
+    if (p.n_end_cells < 0 || 2 * (int64_t)p.n_end_cells > g.ns)
+        return fail(nullptr, MM_ERR_INVALID_ARG, "need 0 <= 2*n_end_cells <= ns");
+    if (p.flags & ~(MM_FLAG_S_PERIODIC | MM_FLAG_OFFSET_PERIODIC_NOMASK | MM_FLAG_CHECK_DT))
+        return fail(nullptr, MM_ERR_INVALID_ARG, "unknown flag");
+    if ((b0 == nullptr) != (b1 == nullptr)) return fail(nullptr, MM_ERR_INVALID_ARG, "pass both density buffers or neither");
+    if (b0 && (b0 == b1 || ((uintptr_t)b0 & 15) || ((uintptr_t)b1 & 15)))
+        return fail(nullptr, MM_ERR_INVALID_ARG, "density buffers must be distinct and 16-byte aligned");
+    const int64_t nc = (int64_t)g.nx * g.ny * g.ntheta;
+    const int64_t inner = (int64_t)g.ns * g.nxi * g.neta;
+    if (nc > (int64_t)1 << 40 || inner > (int64_t)1 << 30) return fail(nullptr, MM_ERR_INVALID_ARG, "grid too large");
+
+    int dev = 0;
+    CUDA_TRY(nullptr, cudaGetDevice(&dev));
+    mm_ctx *c = new (std::nothrow) mm_ctx();
+    if (!c) return fail(nullptr, MM_ERR_NOMEM, "host allocation failed");
+    c->g = g; c->p = p; c->dtype = dtype; c->esize = dtype == MM_F64 ? 8 : 4;
+    c->nc = nc; c->inner = inner; c->cells = nc * inner;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->buf[0] = b0; c->buf[1] = b1; c->owns = (b0 == nullptr); c->cur = 0;
+    c->U = c->V = c->Om = c->kappa = c->cos_t = c->sin_t = nullptr;
+    c->inside = nullptr; c->mom_force = c->mom_torque = nullptr; c->flag_dev = nullptr;
+    c->mom_valid = c->vel_set = false;
+    c->dens_cov_count = 0;
+    c->opt_kernel = 0; c->opt_fuse_t = 1; c->opt_fuse_mom = 1;
+    c->checked_dt = NAN; c->launches = 0; c->kname[0] = 0;
+    try { c->dens_cov.assign((size_t)nc, 0); } catch (...) { delete c; return fail(nullptr, MM_ERR_NOMEM, "host allocation failed"); }
+
+    auto bail = [&](mm_status s, const std::string &m) { std::string mm_ = m; mm_destroy(c); return fail(nullptr, s, mm_); };
+#define CR(expr)                                                                                              \
+    do {                                                                                                      \
+        cudaError_t e_ = (expr);                                                                              \
+        if (e_ != cudaSuccess)                                                                                \
+            return bail(e_ == cudaErrorMemoryAllocation ? MM_ERR_NOMEM : MM_ERR_CUDA,                         \
+                        std::string(#expr) + ": " + cudaGetErrorString(e_));                                  \
+    } while (0)
+    CR(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    if (c->owns) {
+        CR(cudaMalloc(&c->buf[0], (size_t)c->cells * c->esize));
+        CR(cudaMalloc(&c->buf[1], (size_t)c->cells * c->esize));
+    }
+    const size_t plane = (size_t)g.nxi * g.neta;
+    CR(cudaMalloc(&c->U, (size_t)nc * c->esize));
+    CR(cudaMalloc(&c->V, (size_t)nc * c->esize));
+    CR(cudaMalloc(&c->Om, (size_t)nc * c->esize));
+    CR(cudaMalloc(&c->kappa, plane * c->esize));
+    CR(cudaMalloc(&c->cos_t, (size_t)g.ntheta * c->esize));
+    CR(cudaMalloc(&c->sin_t, (size_t)g.ntheta * c->esize));
+    CR(cudaMalloc(&c->inside, plane));
+    CR(cudaMalloc(&c->mom_force, (size_t)nc * 2 * sizeof(double)));
+    CR(cudaMalloc(&c->mom_torque, (size_t)nc * sizeof(double)));
+    CR(cudaMalloc(&c->flag_dev, sizeof(unsigned int)));
+    const int nomask = (p.flags & MM_FLAG_OFFSET_PERIODIC_NOMASK) ? 1 : 0;
+    if (dtype == MM_F64)
+        setup_tables_kernel<double><<<8, 128, 0, c->stream>>>(g.nxi, g.neta, g.ntheta, p.R, p.k_spring, p.k_off0,
+                                                              p.f_detach, nomask, (double *)c->kappa, c->inside,
+                                                              (double *)c->cos_t, (double *)c->sin_t);
+    else
+        setup_tables_kernel<float><<<8, 128, 0, c->stream>>>(g.nxi, g.neta, g.ntheta, p.R, p.k_spring, p.k_off0,
+                                                             p.f_detach, nomask, (float *)c->kappa, c->inside,
+                                                             (float *)c->cos_t, (float *)c->sin_t);
+    CR(cudaGetLastError());
+    c->launches++;
+#undef CR
+    *out = c;
+    return MM_OK;
+}
+
+extern "C" mm_status mm_destroy(mm_ctx *c)
+{
+    if (!c) return MM_OK;
+    cudaStreamSynchronize(c->stream);
+    if (c->owns) { cudaFree(c->buf[0]); cudaFree(c->buf[1]); }
+    cudaFree(c->U); cudaFree(c->V); cudaFree(c->Om);
+    cudaFree(c->kappa); cudaFree(c->cos_t); cudaFree(c->sin_t); cudaFree(c->inside);
+    cudaFree(c->mom_force); cudaFree(c->mom_torque); cudaFree(c->flag_dev);
+    delete c;
+    return MM_OK;
+}
+
+static mm_status copy_in(mm_ctx *c, void *dst, const void *src, size_t bytes, int src_on_device)
+{
+    CUDA_TRY(c, cudaMemcpyAsync(dst, src, bytes, src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
+                                c->stream));
+    if (!src_on_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MM_OK;
+}
+static mm_status copy_out(mm_ctx *c, void *dst, const void *src, size_t bytes, int dst_on_device)
+{
+    CUDA_TRY(c, cudaMemcpyAsync(dst, src, bytes, dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+                                c->stream));
+    if (!dst_on_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MM_OK;
+}
+
+extern "C" mm_status mm_set_density_range(mm_ctx *c, int64_t c_begin, int64_t n, const void *src, int on_device)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    if (!src || c_begin < 0 || n < 0 || c_begin + n > c->nc) return fail(c, MM_ERR_INVALID_ARG, "bad range or NULL source");
+    if (n == 0) return MM_OK;
+    char *dst = (char *)c->buf[c->cur] + (size_t)c_begin * c->inner * c->esize;
+    mm_status s = copy_in(c, dst, src, (size_t)n * c->inner * c->esize, on_device);
+    if (s != MM_OK) return s;
+    for (int64_t i = c_begin; i < c_begin + n; ++i)
+        if (!c->dens_cov[(size_t)i]) { c->dens_cov[(size_t)i] = 1; c->dens_cov_count++; }
+    c->mom_valid = false;
+    return MM_OK;
+}
+extern "C" mm_status mm_set_density(mm_ctx *c, const void *src, int on_device)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    return mm_set_density_range(c, 0, c->nc, src, on_device);
+}
+extern "C" mm_status mm_get_density_range(mm_ctx *c, int64_t c_begin, int64_t n, void *dst, int on_device)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    if (!dst || c_begin < 0 || n < 0 || c_begin + n > c->nc) return fail(c, MM_ERR_INVALID_ARG, "bad range or NULL destination");
+    if (c->dens_cov_count != c->nc) return fail(c, MM_ERR_STATE, "density not set");
+    if (n == 0) return MM_OK;
+    const char *src = (const char *)c->buf[c->cur] + (size_t)c_begin * c->inner * c->esize;
+    return copy_out(c, dst, src, (size_t)n * c->inner * c->esize, on_device);
+}
+extern "C" mm_status mm_get_density(mm_ctx *c, void *dst, int on_device)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    return mm_get_density_range(c, 0, c->nc, dst, on_device);
+}
+
+extern "C" mm_status mm_set_filament_velocity(mm_ctx *c, const void *U, const void *V, const void *Om, int on_device)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    if (!U || !V || !Om) return fail(c, MM_ERR_INVALID_ARG, "NULL velocity array");
+    const size_t bytes = (size_t)c->nc * c->esize;
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    CUDA_TRY(c, cudaMemcpyAsync(c->U, U, bytes, kind, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->V, V, bytes, kind, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->Om, Om, bytes, kind, c->stream));
+    if (!on_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->vel_set = true;
+    c->checked_dt = NAN;
+    return MM_OK;
+}
+
+extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    if (n_sub < 0) return fail(c, MM_ERR_INVALID_ARG, "n_sub < 0");
+    if (n_sub == 0) return MM_OK;
+    if (!(std::isfinite(dt) && dt > 0)) return fail(c, MM_ERR_INVALID_ARG, "dt must be finite and > 0");
+    if (c->dens_cov_count != c->nc || !c->vel_set) return fail(c, MM_ERR_STATE, "set density and filament velocity first");
+    if ((c->p.flags & MM_FLAG_CHECK_DT) && !(c->checked_dt == dt)) {
+        CUDA_TRY(c, cudaMemsetAsync(c->flag_dev, 0, sizeof(unsigned int), c->stream));
+        const int blocks = c->sm_count * 16;
+        if (c->dtype == MM_F64) check_dt_kernel<double><<<blocks, 256, 0, c->stream>>>(make_kparams<double>(c, dt), c->flag_dev);
+        else check_dt_kernel<float><<<blocks, 256, 0, c->stream>>>(make_kparams<float>(c, dt), c->flag_dev);
+        CUDA_TRY(c, cudaGetLastError());
+        c->launches++;
+        unsigned int flag = 0;
+        CUDA_TRY(c, cudaMemcpyAsync(&flag, c->flag_dev, sizeof flag, cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (flag) return fail(c, MM_ERR_UNSTABLE, "dt violates the positivity bound S8");
+        c->checked_dt = dt;
+    }
+    const bool want_stream = c->opt_kernel == 2 || (c->opt_kernel == 0 && stream_supported(c));
+    if (c->opt_kernel == 2 && !stream_supported(c))
+        return fail(c, MM_ERR_INVALID_ARG, "streamed kernel does not support this grid/flags");
+    c->mom_valid = false;
+    int remaining = n_sub;
+    while (remaining > 0) {
+        mm_status s;
+        int t = 1;
+        if (want_stream) {
+            t = remaining < c->opt_fuse_t ? remaining : c->opt_fuse_t;
+            const bool mom = c->opt_fuse_mom && remaining == t;
+            s = launch_stream(c, t, mom, dt, c->buf[c->cur], c->buf[c->cur ^ 1]);
+            if (s == MM_OK && mom) c->mom_valid = true;
+        } else {
+            s = c->dtype == MM_F64 ? launch_generic<double>(c, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
+                                   : launch_generic<float>(c, dt, c->buf[c->cur], c->buf[c->cur ^ 1]);
+        }
+        if (s != MM_OK) return s;
+        c->cur ^= 1;
+        remaining -= t;
+    }
+    return MM_OK;
+}
+
+extern "C" mm_status mm_moments(mm_ctx *c, double *force, double *torque, int on_device)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    if (c->dens_cov_count != c->nc) return fail(c, MM_ERR_STATE, "density not set");
+    if (!c->mom_valid) {
+        mm_status s = c->dtype == MM_F64 ? launch_moments<double>(c) : launch_moments<float>(c);
+        if (s != MM_OK) return s;
+        c->mom_valid = true;
+    }
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (force) CUDA_TRY(c, cudaMemcpyAsync(force, c->mom_force, (size_t)c->nc * 2 * sizeof(double), kind, c->stream));
+    if (torque) CUDA_TRY(c, cudaMemcpyAsync(torque, c->mom_torque, (size_t)c->nc * sizeof(double), kind, c->stream));
+    if (!on_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MM_OK;
+}
+
+extern "C" mm_status mm_set_option(mm_ctx *c, mm_option opt, int64_t v)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    switch (opt) {
+    case MM_OPT_KERNEL:
+        if (v < 0 || v > 2) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_KERNEL in 0..2");
+        c->opt_kernel = (int)v; return MM_OK;
+    case MM_OPT_FUSE_T:
+        if (v < 1 || v > MM_MAX_FUSE_T) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_FUSE_T in 1..MM_MAX_FUSE_T");
+        c->opt_fuse_t = (int)v; return MM_OK;
+    case MM_OPT_FUSE_MOMENTS:
+        c->opt_fuse_mom = v ? 1 : 0; return MM_OK;
+    }
+    return fail(c, MM_ERR_INVALID_ARG, "unknown option");
+}
+
+extern "C" int64_t mm_launch_count(const mm_ctx *c) { return c ? c->launches : 0; }
+extern "C" const char *mm_kernel_name(const mm_ctx *c) { return c ? c->kname : ""; }
+
+extern "C" const char *mm_status_string(mm_status s)
+{
+    switch (s) {
+    case MM_OK: return "MM_OK";
+    case MM_ERR_INVALID_ARG: return "MM_ERR_INVALID_ARG";
+    case MM_ERR_CUDA: return "MM_ERR_CUDA";
+    case MM_ERR_NOMEM: return "MM_ERR_NOMEM";
+    case MM_ERR_STATE: return "MM_ERR_STATE";
+    case MM_ERR_UNSTABLE: return "MM_ERR_UNSTABLE";
+    }
+    return "MM_ERR_?";
+}
+extern "C" const char *mm_last_error(const mm_ctx *c) { return c ? c->err.c_str() : g_create_err.c_str(); }

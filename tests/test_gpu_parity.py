@@ -1,0 +1,129 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Sizes here are small enough for the oracle to finish in seconds while still spanning several warps,
+several TMA ring wraps, ragged chunk tails (Ns odd) and more configurations than resident warps.
+Full BASELINE.json sizes live in test_gpu_baseline_configs.py.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import mm_inputs as mi
+from mm_inputs import Grid, Params
+from util import check_parity, gpu_run, oracle_run, random_inputs, p1_density, TOL
+
+pytestmark = pytest.mark.gpu
+
+
+def _dt(g, p, om=1.0, cfl=0.4):
+    return mi.benchmark_dt(g, p, om, cfl=cfl)
+
+
+# ------------------------------------------------------------------ generic kernels: any size, all flags
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", [(2, 2, 2, 4, 3, 3), (1, 3, 5, 5, 3, 7), (2, 1, 4, 9, 16, 16), (1, 1, 3, 2, 1, 1)])
+def test_generic_small_grids(dtype, shape):
+    g = Grid(*shape)
+    p = Params()
+    check_parity(g, p, dtype, [3, 4], _dt(g, p), kernel=1)
+
+
+@pytest.mark.parametrize("flags", [mi.FLAG_S_PERIODIC, mi.FLAG_OFFSET_PERIODIC_NOMASK,
+                                   mi.FLAG_S_PERIODIC | mi.FLAG_OFFSET_PERIODIC_NOMASK])
+def test_generic_periodic_flags(flags):
+    g = Grid(2, 2, 4, 6, 5, 4)
+    p = Params(flags=flags)
+    check_parity(g, p, "f64", [5, 5], _dt(g, p), kernel=1)
+
+
+def test_generic_stall_clamp_and_wide_ends():
+    g = Grid(1, 2, 8, 12, 8, 8)
+    p = Params(k_spring=200.0, n_end_cells=3, end_detach_mult=4.0)
+    check_parity(g, p, "f64", [6], 0.3 * _dt(g, p), kernel=1)
+
+
+# ------------------------------------------------------------------ streamed kernels
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("T", [1, 2, 3, 4])
+@pytest.mark.parametrize("nxi", [16, 8])
+def test_stream_kernel_parity(dtype, T, nxi):
+    # 700 configurations > resident warps on 148 SMs? no (that needs ~2000); still several per warp when
+    # the grid is capped to ceil(Nc/4) blocks; Ns=7 gives a ragged last chunk (P=2).
+    g = Grid(5, 7, 20, 7, nxi, nxi)
+    p = Params()
+    e, info = check_parity(g, p, dtype, [5, 3], _dt(g, p), kernel=2, fuse_t=T)
+    assert info["kernel"].startswith("stream<"), info
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_stream_many_configs_per_warp(dtype):
+    """More configurations than the launch has warps: exercises the ring running across configuration
+    boundaries and per-configuration re-initialisation."""
+    g = Grid(16, 16, 16, 6, 8, 8)   # 4096 configs of 384 cells
+    p = Params()
+    check_parity(g, p, dtype, [4], _dt(g, p), kernel=2, fuse_t=2)
+
+
+def test_stream_equals_generic_and_fusion_invariance():
+    """C8 on the GPU: T-fused passes == T=1 passes == generic kernel, and substep(a);substep(b) == substep(a+b)."""
+    g = Grid(3, 3, 8, 10, 16, 16)
+    p = Params()
+    dt = _dt(g, p)
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    ref, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [7], dt, kernel=1)
+    for T in (1, 2, 3, 4):
+        out, _, info = gpu_run(g, p, "f64", U, V, Om, m0, [7], dt, kernel=2, fuse_t=T)
+        assert p1_density(out, ref) < 1e-13, (T, info)
+    a, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [3, 4], dt, kernel=2, fuse_t=2)
+    b, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [7], dt, kernel=2, fuse_t=2)
+    assert p1_density(a, b) < 1e-13
+
+
+def test_stream_moments_fused_equals_standalone():
+    g = Grid(2, 3, 8, 12, 16, 16)
+    p = Params()
+    dt = _dt(g, p)
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    _, mf, _ = gpu_run(g, p, "f64", U, V, Om, m0, [4, 4], dt, kernel=2, fuse_t=2, fuse_mom=1)
+    _, ms, _ = gpu_run(g, p, "f64", U, V, Om, m0, [4, 4], dt, kernel=2, fuse_t=2, fuse_mom=0)
+    for (f1, t1), (f2, t2) in zip(mf, ms):
+        assert np.allclose(f1, f2, rtol=0, atol=1e-15) and np.allclose(t1, t2, rtol=0, atol=1e-15)
+
+
+def test_stream_stall_clamp_wide_ends_and_omega2():
+    g = Grid(2, 2, 8, 9, 16, 16)
+    p = Params(k_spring=200.0, n_end_cells=2, end_detach_mult=3.0)
+    check_parity(g, p, "f64", [6], 0.25 * _dt(g, p, 2.0), omega_max=2.0, kernel=2, fuse_t=3)
+
+
+def test_library_owned_buffers_and_permutation_invariance():
+    """NULL,NULL buffers (library allocates) and C8: same-theta configurations swapped -> outputs swapped bitwise."""
+    g = Grid(2, 2, 4, 8, 8, 8)
+    p = Params()
+    dt = _dt(g, p)
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    out, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [5], dt, own_buffers=True)
+    perm = np.arange(g.nc); perm[[1, 1 + g.ntheta]] = perm[[1 + g.ntheta, 1]]
+    out2, _, _ = gpu_run(g, p, "f64", U[perm], V[perm], Om[perm], m0[perm], [5], dt, own_buffers=True)
+    assert np.array_equal(out2, out[perm])
+
+
+def test_positivity_and_mask_on_gpu():
+    g = Grid(2, 2, 8, 16, 16, 16)
+    p = Params()
+    U, V, Om, m0 = random_inputs(g, p, "f32")
+    out, _, _ = gpu_run(g, p, "f32", U, V, Om, m0, [50], _dt(g, p))
+    mask = mi.inside_mask(16, 16)
+    assert (out >= 0).all() and (out[:, :, ~mask] == 0).all() and (out[:, :, mask] > 0).all()
+
+
+def test_dirty_masked_input_is_dropped():
+    g = Grid(1, 2, 4, 6, 16, 16)
+    p = Params()
+    dt = _dt(g, p)
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    m0 = m0.copy(); m0[:, :, ~mi.inside_mask(16, 16)] = 3.0
+    out, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [2], dt, kernel=2, fuse_t=2)
+    ref, _ = oracle_run(g, p, U, V, Om, m0, [2], dt)
+    assert p1_density(out, ref) < TOL["f64"]
