@@ -1,0 +1,421 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the bound-motor microscale hot path (libmm, sm_100a) on BASELINE.json's configs.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cuda|reference] [--config i] [--fuse-t T]
+
+One "step" = one macro step of the whole hot path on one workload of
+BASELINE.json `configs`: mm_set_filament_velocity, then n_sub explicit substeps with the moment reduction at
+the config's cadence (configs[3-4]: 50 substeps, moments every 10).  The density stays resident on the GPU
+between steps, as the paper prescribes; step k+1 continues from step k's state.
+
+Prints ONE JSON line (rank 0).  `value` = motor-cell updates/s (G/s), whole job, inputs resident in HBM;
+`e2e` = same metric through the same C-ABI calls with pinned HOST buffers for (U,V,Omega) and the moments,
+i.e. the host<->device copies of every macro step inside the timed region.  `roofline` is for the dominant
+kernel (the fused advect+react(+moments) substep kernel), timed live with CUDA events on the library's stream.
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+import mm_inputs as mi
+
+METRIC = "motor_cell_updates_per_s"
+UNIT = "G cell-updates/s"
+ES = {"f64": 8, "f32": 4}
+
+
+# --------------------------------------------------------------------------------------------- helpers
+def measured_peaks():
+    """HBM peak (GB/s) from the driver-written MEASURED_PEAKS.json, else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, device copy)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons during the timed region (NVML; nvidia-smi as a fallback)."""
+
+    BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
+    NOTE = {"sw_power_cap": 0x4, "hw_power_brake": 0x80, "sync_boost": 0x10, "app_clocks": 0x2, "idle": 0x1}
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _once(self):
+        if self._nv is not None:
+            nv = self._nv
+            self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+            try:
+                bits = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+            except Exception:
+                bits = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+            for name, bit in {**self.BAD, **self.NOTE}.items():
+                if bits & bit and name != "idle":
+                    self.reasons.add(name)
+        else:
+            import subprocess
+            out = subprocess.run(["nvidia-smi", f"--id={self.index}", "--query-gpu=clocks.sm,clocks.max.sm,"
+                                  "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+                                  "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap",
+                                  "--format=csv,noheader,nounits"], capture_output=True, text=True).stdout.strip()
+            f = [x.strip() for x in out.split(",")]
+            if len(f) >= 6:
+                self.samples.append(float(f[0]))
+                self.max_mhz = float(f[1])
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[2:6]):
+                    if v == "Active":
+                        self.reasons.add(name)
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self._once()
+            except Exception:
+                pass
+            self._stop.wait(0.05 if self._nv is not None else 0.2)
+
+    def start(self):
+        self._thr = threading.Thread(target=self._run, daemon=True)
+        self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def pick_workload(idx, free_bytes=None):
+    """BASELINE.json north_star quotes the target 'at the largest config, on one GPU': configs[4] when its two
+    density buffers fit, else the largest that does."""
+    if idx is not None:
+        return idx
+    order = [4, 3, 1, 0]
+    for i in order:
+        w = mi.CONFIGS[i]
+        need = 2 * w.grid.cells * ES[w.dtype] + (2 << 30)
+        if free_bytes is None or need <= free_bytes:
+            return i
+    return 0
+
+
+def rank_workload(w: mi.Workload, rank: int):
+    """Weak scaling: configurations never interact, so rank r runs its own copy of the workload
+    grid -- the r-th x-slab of a world-times-larger periodic domain -- drawn from seed + r.  No data-path collective."""
+    return mi.Workload(w.name, w.grid, w.dtype, w.n_sub, w.moments_every, w.omega_max, w.seed + rank, w.params)
+
+
+def upload_inputs(mm, w, chunk_configs=2048, log=None):
+    """S11 inputs for the whole workload, generated on the host in chunks of configurations and uploaded."""
+    npdt = np.float64 if w.dtype == "f64" else np.float32
+    g = w.grid
+    st = mi.Stream(g, w.params.R, w.seed, w.omega_max)
+    U, V, Om = st.velocities(npdt)
+    buf = np.empty((min(chunk_configs, g.nc), g.ns, g.nxi, g.neta), npdt)
+    t0 = time.time()
+    for c0 in range(0, g.nc, chunk_configs):
+        n = min(chunk_configs, g.nc - c0)
+        st.density(n, npdt, out=buf[:n])
+        mm.set_density_range(c0, n, buf[:n])
+    st.close()
+    if log:
+        log(f"inputs: {g.cells/1e9:.2f} G cells generated+uploaded in {time.time()-t0:.1f} s")
+    return U, V, Om
+
+
+# --------------------------------------------------------------------------------------------- CUDA arm
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1908_04279_b200 import MM, binding as b
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libmm has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def log(msg):
+        if rank == 0:
+            print(f"[bench] {msg}", file=sys.stderr, flush=True)
+
+    free_b, _ = torch.cuda.mem_get_info()
+    idx = pick_workload(args.config, free_b)
+    w = rank_workload(mi.CONFIGS[idx], rank)
+    g, es = w.grid, ES[w.dtype]
+    tdt = torch.float64 if w.dtype == "f64" else torch.float32
+    log(f"workload configs[{idx}] {w.name}: Nc={g.nc} cells={g.cells} dtype={w.dtype} n_sub={w.n_sub} "
+        f"moments every {w.moments_every}; dt={w.dt:.6e}")
+
+    stream = torch.cuda.current_stream()
+    b0 = torch.empty(g.cells, dtype=tdt, device=dev)
+    b1 = torch.empty(g.cells, dtype=tdt, device=dev)
+    mm = MM(g, w.params, w.dtype, b0, b1, stream=stream.cuda_stream)
+    if args.fuse_t:
+        mm.set_option(b.MM_OPT_FUSE_T, args.fuse_t)
+    if args.kernel is not None:
+        mm.set_option(b.MM_OPT_KERNEL, args.kernel)
+    Uh, Vh, Oh = upload_inputs(mm, w, log=log)
+
+    n_mom = w.n_sub // w.moments_every
+    # device-resident inputs/outputs for `value`
+    Ud, Vd, Od = (torch.from_numpy(x).to(dev) for x in (Uh, Vh, Oh))
+    Fd = torch.empty((n_mom, g.nc, 2), dtype=torch.float64, device=dev)
+    Td = torch.empty((n_mom, g.nc), dtype=torch.float64, device=dev)
+    # pinned host buffers for `e2e`
+    Up, Vp, Op = (torch.from_numpy(x).pin_memory() for x in (Uh, Vh, Oh))
+    Fp = torch.empty((n_mom, g.nc, 2), dtype=torch.float64).pin_memory()
+    Tp = torch.empty((n_mom, g.nc), dtype=torch.float64).pin_memory()
+
+    sub_events = []   # (start, stop, n_sub) around every mm_substep call of the timed region
+
+    def step(U, V, Om, F, T, record=False):
+        mm.set_filament_velocity(U, V, Om)                                  # A0
+        for k in range(n_mom):
+            if record:
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+            mm.substep(w.moments_every, w.dt)                               # A1-A3 (+A4 fused into the last pass)
+            if record:
+                e1.record(stream)
+                sub_events.append((e0, e1, w.moments_every))
+            mm.moments(F[k], T[k])                                          # A4
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(nsteps, U, V, Om, F, T, record=False):
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = mm.launch_count
+        e0.record(stream)
+        for _ in range(nsteps):
+            step(U, V, Om, F, T, record)
+        e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms, mm.launch_count - l0
+
+    # ---- warm-up, then the timed region (inputs resident in HBM)
+    for _ in range(max(args.warmup, 0)):
+        step(Ud, Vd, Od, Fd, Td)
+    sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else local)
+    sampler.start()
+    ms, launches = timed(args.steps, Ud, Vd, Od, Fd, Td, record=True)
+    clocks = sampler.stop()
+    kname = mm.kernel_name
+    updates_per_step = g.cells * w.n_sub * world
+    value = updates_per_step * args.steps / (ms * 1e-3) / 1e9
+
+    # ---- dominant kernel: average launch duration over the timed region (CUDA events on the library's stream)
+    sub_ms = sum(a.elapsed_time(c) for a, c, _ in sub_events)
+    sub_n = sum(n for _, _, n in sub_events)
+    fuse_t = args.fuse_t or mm.get_option(b.MM_OPT_FUSE_T)
+    launches_per_call = -(-w.moments_every // fuse_t)
+    n_launch = launches_per_call * len(sub_events)
+    peak, peak_src = measured_peaks()
+    alg_bytes = 2.0 * es * g.cells * sub_n                 # 2*sizeof(real) B per cell-update (T=1 count)
+    pass_bytes = 2.0 * es * g.cells * n_launch             # what one fused pass has to move: read once + write once
+    achieved = alg_bytes / (sub_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                "frac": round(achieved / peak, 4), "traffic": None, "peak_source": peak_src,
+                "bytes_per_cell_update": 2 * es, "fuse_T": fuse_t, "launches": n_launch,
+                "avg_launch_ms": round(sub_ms / n_launch, 4),
+                "pass_gbs": round(pass_bytes / (sub_ms * 1e-3) / 1e9, 1),
+                "pass_frac": round(pass_bytes / (sub_ms * 1e-3) / 1e9 / peak, 4),
+                "kernel_share_of_step": round(sub_ms / ms, 4)}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(traffic_file):
+        try:
+            with open(traffic_file) as f:
+                tr = json.load(f).get(f"configs[{idx}]", {})
+            roofline["traffic"] = tr.get("dram_bytes_per_launch")
+            roofline["traffic_source"] = tr.get("source")
+        except Exception:
+            pass
+
+    # ---- the same kernel unfused (T=1) for the T=1 roofline point (outside the timed region)
+    if not args.no_t1 and fuse_t != 1:
+        mm.set_option(b.MM_OPT_FUSE_T, 1)
+        mm.substep(3, w.dt)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        mm.substep(6, w.dt)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        t1 = 2.0 * es * g.cells * 6 / (e0.elapsed_time(e1) * 1e-3) / 1e9
+        roofline["t1_gbs"] = round(t1, 1)
+        roofline["t1_frac"] = round(t1 / peak, 4)
+        roofline["t1_kernel"] = mm.kernel_name
+        mm.set_option(b.MM_OPT_FUSE_T, fuse_t)
+
+    # ---- end to end: pinned host (U,V,Omega) in, moments out to pinned host, every step
+    for _ in range(2):
+        step(Up, Vp, Op, Fp, Tp)
+    ms_e2e, _ = timed(args.steps, Up, Vp, Op, Fp, Tp)
+    e2e = {"value": round(updates_per_step * args.steps / (ms_e2e * 1e-3) / 1e9, 2), "unit": UNIT,
+           "h2d_bytes_per_step": int(3 * g.nc * es), "d2h_bytes_per_step": int(n_mom * 3 * g.nc * 8),
+           "ms_per_step": round(ms_e2e / args.steps, 3),
+           "note": "density is resident state (PAPER.md:133,143); per-step host traffic is (U,V,Omega) in, moments out"}
+    mm.destroy()
+    del b0, b1
+
+    out = {"metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": round(ms / args.steps, 3), "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": w.dtype, "data": "synthetic",
+           "config": {"workload": f"configs[{idx}] {w.name}", "grid": [g.nx, g.ny, g.ntheta, g.ns, g.nxi, g.neta],
+                      "cells_per_gpu": g.cells, "n_sub_per_step": w.n_sub, "moments_every": w.moments_every,
+                      "dt": w.dt, "seed": w.seed, "parallelism": f"configs x{world} (no collective)",
+                      "l2": "inputs larger than L2 (two density buffers of %.1f GB)" % (g.cells * es / 1e9)},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "impl": "cuda"}
+    if rank == 0 and world == 1 and not args.no_cpu:
+        out["cpu_baseline"] = cpu_baseline(w, target_s=args.cpu_seconds, log=log)
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# --------------------------------------------------------------------------------------------- oracle arm
+def oracle_sample(w, n_configs, reps=1):
+    """Oracle (as it stands) on the first n_configs configurations of the workload: full step (n_sub substeps,
+    moments at the cadence).  Returns seconds per step."""
+    from oracle import mm_oracle as orc
+    npdt = np.float64 if w.dtype == "f64" else np.float32
+    st = mi.Stream(w.grid, w.params.R, w.seed, w.omega_max)
+    U, V, Om = st.velocities(npdt)
+    m = st.density(n_configs, npdt).astype(np.float64)
+    st.close()
+    U, V, Om = (np.asarray(x[:n_configs], np.float64) for x in (U, V, Om))
+    times = []
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        for _k in range(w.n_sub // w.moments_every):
+            m = orc.run(w.grid, w.params, U, V, Om, m, w.moments_every, w.dt)
+            orc.moments(w.grid, w.params, m)
+        times.append(time.perf_counter() - t0)
+    return times
+
+
+def cpu_baseline(w, target_s=15.0, log=None):
+    from oracle import mm_oracle as orc
+    cores = orc.threads()
+    probe_n = 2 * cores
+    t = oracle_sample(mi.Workload(w.name, w.grid, w.dtype, w.moments_every, w.moments_every, w.omega_max, w.seed,
+                                  w.params), probe_n)[0]
+    rate = probe_n * w.grid.inner * w.moments_every / t
+    n = int(target_s * rate / (w.grid.inner * w.n_sub))
+    n = max(cores, min(w.grid.nc, n // cores * cores))
+    t = oracle_sample(w, n)[0]
+    val = n * w.grid.inner * w.n_sub / t / 1e9
+    if log:
+        log(f"cpu_baseline: oracle on {n} configurations, {t:.1f} s, {val*1e3:.1f} M cell-updates/s on {cores} threads")
+    return {"value": round(val, 5), "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {n} of {w.grid.nc} configurations of the workload, all {w.n_sub} substeps + moments "
+                      f"every {w.moments_every}; fp64; gcc -O2 -fopenmp over configurations", "seconds": round(t, 2)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank != 0:
+        return
+    free_b = None
+    try:
+        import torch
+        if torch.cuda.is_available():
+            free_b, _ = torch.cuda.mem_get_info()
+    except Exception:
+        pass
+    idx = pick_workload(args.config, free_b)
+    w = mi.CONFIGS[idx]
+    g = w.grid
+    from oracle import mm_oracle as orc
+    cores = orc.threads()
+    # size the per-step sample so that (warmup + steps) steps take about args.cpu_seconds * 4 in total
+    probe_n = 2 * cores
+    t = oracle_sample(mi.Workload(w.name, g, w.dtype, w.moments_every, w.moments_every, w.omega_max, w.seed, w.params),
+                      probe_n)[0]
+    rate = probe_n * g.inner * w.moments_every / t
+    budget = 4.0 * args.cpu_seconds / max(1, args.steps + args.warmup)
+    n = int(budget * rate / (g.inner * w.n_sub))
+    n = max(cores, min(g.nc, n // cores * cores))
+    times = oracle_sample(w, n, reps=args.warmup + args.steps)[args.warmup:]
+    sec = sum(times)
+    val = n * g.inner * w.n_sub * args.steps / sec / 1e9
+    sample = (f"each step = first {n} of {g.nc} configurations of the workload, all {w.n_sub} substeps + moments every "
+              f"{w.moments_every}; fp64 oracle, gcc -O2 -fopenmp over configurations")
+    out = {"impl": "reference", "metric": METRIC, "value": round(val, 5), "unit": UNIT, "n_gpus": world,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(sec / args.steps * 1e3, 3),
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": f"configs[{idx}] {w.name}", "grid": [g.nx, g.ny, g.ntheta, g.ns, g.nxi, g.neta],
+                      "n_sub_per_step": w.n_sub, "moments_every": w.moments_every, "dt": w.dt, "seed": w.seed},
+           "cpu_baseline": {"value": round(val, 5), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": round(val, 5), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=None, help="index into BASELINE.json configs (default: largest that fits)")
+    ap.add_argument("--fuse-t", type=int, default=0, help="override MM_OPT_FUSE_T (0 = library default)")
+    ap.add_argument("--kernel", type=int, default=None, help="override MM_OPT_KERNEL")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-t1", action="store_true", help="skip the unfused (T=1) roofline point")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    args = ap.parse_args()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus != world and world == 1 and args.gpus > 1:
+        raise SystemExit("launch N>1 with: python -m torch.distributed.run --nnodes=1 --nproc-per-node N "
+                         "--master-addr 127.0.0.1 --master-port P bench.py --gpus N ...")
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

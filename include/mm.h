@@ -122,6 +122,7 @@ mm_status mm_substep(mm_ctx *ctx, int32_t n_sub, double dt);
 mm_status mm_moments(mm_ctx *ctx, double *force, double *torque, int dst_on_device);
 
 mm_status mm_set_option(mm_ctx *ctx, mm_option opt, int64_t value);
+mm_status mm_get_option(const mm_ctx *ctx, mm_option opt, int64_t *value); /* current setting; MM_ERR_INVALID_ARG on NULL / unknown */
 
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t mm_launch_count(const mm_ctx *ctx);

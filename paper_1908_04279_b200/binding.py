@@ -17,7 +17,7 @@ MM_OPT_KERNEL, MM_OPT_FUSE_T, MM_OPT_FUSE_MOMENTS = 0, 1, 2
 MM_MAX_FUSE_T = 4
 
 EXPORTS = ["mm_create", "mm_set_density", "mm_get_density", "mm_set_density_range", "mm_get_density_range",
-           "mm_set_filament_velocity", "mm_substep", "mm_moments", "mm_set_option", "mm_launch_count",
+           "mm_set_filament_velocity", "mm_substep", "mm_moments", "mm_set_option", "mm_get_option", "mm_launch_count",
            "mm_kernel_name", "mm_destroy", "mm_status_string", "mm_last_error"]
 
 
@@ -59,6 +59,7 @@ def lib():
         L.mm_substep.argtypes = [vp, i32, dbl]
         L.mm_moments.argtypes = [vp, vp, vp, ctypes.c_int]
         L.mm_set_option.argtypes = [vp, ctypes.c_int, i64]
+        L.mm_get_option.argtypes = [vp, ctypes.c_int, ctypes.POINTER(i64)]
         L.mm_launch_count.argtypes = [vp]
         L.mm_launch_count.restype = i64
         L.mm_kernel_name.argtypes = [vp]
@@ -68,9 +69,6 @@ def lib():
         L.mm_status_string.restype = ctypes.c_char_p
         L.mm_last_error.argtypes = [vp]
         L.mm_last_error.restype = ctypes.c_char_p
-        for n in EXPORTS:
-            if getattr(L, n).restype is ctypes.c_int:
-                pass
         _lib = L
     return _lib
 
@@ -155,6 +153,11 @@ class MM:
 
     def set_option(self, opt: int, value: int):
         self._check(self._L.mm_set_option(self._h, opt, value))
+
+    def get_option(self, opt: int) -> int:
+        v = ctypes.c_int64()
+        self._check(self._L.mm_get_option(self._h, opt, ctypes.byref(v)))
+        return int(v.value)
 
     @property
     def launch_count(self) -> int:

@@ -430,6 +430,17 @@ extern "C" mm_status mm_set_option(mm_ctx *c, mm_option opt, int64_t v)
     return fail(c, MM_ERR_INVALID_ARG, "unknown option");
 }
 
+extern "C" mm_status mm_get_option(const mm_ctx *c, mm_option opt, int64_t *v)
+{
+    if (!c || !v) return MM_ERR_INVALID_ARG;
+    switch (opt) {
+    case MM_OPT_KERNEL: *v = c->opt_kernel; return MM_OK;
+    case MM_OPT_FUSE_T: *v = c->opt_fuse_t; return MM_OK;
+    case MM_OPT_FUSE_MOMENTS: *v = c->opt_fuse_mom; return MM_OK;
+    }
+    return MM_ERR_INVALID_ARG;
+}
+
 extern "C" int64_t mm_launch_count(const mm_ctx *c) { return c ? c->launches : 0; }
 extern "C" const char *mm_kernel_name(const mm_ctx *c) { return c ? c->kname : ""; }
 
