@@ -12,6 +12,7 @@
 
 #include "mm_generic.cuh"
 #include "mm_stream.cuh"
+#include "mm_tile.cuh"
 
 using namespace mm;
 
@@ -37,6 +38,8 @@ struct mm_ctx {
     double checked_dt;              // dt the S8 check last passed with (NaN = none)
     int64_t launches;
     int sm_count;
+    CUtensorMap tmap[2];            // tiled-TMA views of buf[0], buf[1] (tile kernel)
+    bool tile_ok;                   // tensor maps built and grid/flags supported by the tile kernel
     std::string err;
     char kname[64];
 };
@@ -166,6 +169,105 @@ static mm_status launch_stream(mm_ctx *c, int T, bool mom, double dt, const void
                : launch_stream_shape<float, 8, 8, 2>(c, T, mom, dt, in, out);
 }
 
+// ---- tile-kernel dispatch ---------------------------------------------------------------------
+typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static constexpr int TILE_P = 2;   // planes per TMA box
+
+static bool tile_shape_supported(const mm_ctx *c)
+{
+    if (c->p.flags & (MM_FLAG_S_PERIODIC | MM_FLAG_OFFSET_PERIODIC_NOMASK)) return false;
+    return (c->g.nxi == 16 && c->g.neta == 16) || (c->g.nxi == 8 && c->g.neta == 8);
+}
+
+// 4-D view (eta, xi, s, c) of a density buffer; box = one padded plane pair of CPW configurations,
+// out-of-bounds elements read as zero (the ghost cells of S5).
+static mm_status build_tensor_maps(mm_ctx *c)
+{
+    c->tile_ok = false;
+    if (!tile_shape_supported(c)) return MM_OK;
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return fail(c, MM_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
+    }
+    const int cpw = 256 / (c->g.nxi * c->g.neta);
+    const cuuint64_t dims[4] = {(cuuint64_t)c->g.neta, (cuuint64_t)c->g.nxi, (cuuint64_t)c->g.ns, (cuuint64_t)c->nc};
+    const cuuint64_t strides[3] = {(cuuint64_t)c->g.neta * c->esize, (cuuint64_t)c->g.nxi * c->g.neta * c->esize,
+                                   (cuuint64_t)c->inner * c->esize};
+    const cuuint32_t box[4] = {(cuuint32_t)c->g.neta + (cuuint32_t)(32 / c->esize), (cuuint32_t)c->g.nxi + 2, (cuuint32_t)TILE_P, (cuuint32_t)cpw};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    for (int b = 0; b < 2; ++b) {
+        CUresult r = ((encode_tiled_fn)fn)(&c->tmap[b], c->dtype == MM_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64
+                                                                          : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+                                           4, c->buf[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(c, MM_ERR_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
+    }
+    c->tile_ok = true;
+    return MM_OK;
+}
+
+template <typename real, int NXI, int NETA, int CB, int T, bool MOM>
+static mm_status launch_tile_inst(mm_ctx *c, double dt, int in_idx, void *out)
+{
+    constexpr int P = TILE_P, D = (T == 1 ? 4 : 3), WARPS = 4, MINB = 2;
+    using Cfg = TileCfg<real, NXI, NETA, CB, T, P, D, WARPS>;
+    auto kern = substep_tile_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB>;
+    static int blocks_per_sm = 0;
+    if (blocks_per_sm == 0) {
+        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
+        int n = 0;
+        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, Cfg::SMEM_BYTES));
+        if (n < 1) return fail(c, MM_ERR_CUDA, "tile kernel does not fit on an SM");
+        blocks_per_sm = n;
+    }
+    int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
+    const int64_t groups = (c->nc + Cfg::CPW - 1) / Cfg::CPW;
+    const int64_t need = (groups + WARPS - 1) / WARPS;
+    if (grid > need) grid = need;
+    KParams<real> kp = make_kparams<real>(c, dt);
+    kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(kp, c->tmap[in_idx], (real *)out, c->mom_force,
+                                                                      c->mom_torque);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches++;
+    snprintf(c->kname, sizeof c->kname, "tile<%s,%dx%d,T=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA, T,
+             MOM ? ",mom" : "");
+    return MM_OK;
+}
+
+template <typename real, int NXI, int NETA, int CB>
+static mm_status launch_tile_shape(mm_ctx *c, int T, bool mom, double dt, int in_idx, void *out)
+{
+#define MM_CASE(TT)                                                                                     \
+    case TT:                                                                                            \
+        return mom ? launch_tile_inst<real, NXI, NETA, CB, TT, true>(c, dt, in_idx, out)                \
+                   : launch_tile_inst<real, NXI, NETA, CB, TT, false>(c, dt, in_idx, out);
+    switch (T) {
+        MM_CASE(1)
+        MM_CASE(2)
+        MM_CASE(3)
+        MM_CASE(4)
+    }
+#undef MM_CASE
+    return fail(c, MM_ERR_INVALID_ARG, "unsupported fuse depth");
+}
+
+static mm_status launch_tile(mm_ctx *c, int T, bool mom, double dt, int in_idx, void *out)
+{
+    const bool big = c->g.nxi == 16;
+    if (c->dtype == MM_F64)
+        return big ? launch_tile_shape<double, 16, 16, 2>(c, T, mom, dt, in_idx, out)
+                   : launch_tile_shape<double, 8, 8, 2>(c, T, mom, dt, in_idx, out);
+    return big ? launch_tile_shape<float, 16, 16, 4>(c, T, mom, dt, in_idx, out)
+               : launch_tile_shape<float, 8, 8, 4>(c, T, mom, dt, in_idx, out);
+}
+
 template <typename real>
 static mm_status launch_generic(mm_ctx *c, double dt, const void *in, void *out)
 {
@@ -233,7 +335,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->buf[0] = b0; c->buf[1] = b1; c->owns = (b0 == nullptr); c->cur = 0;
     c->U = c->V = c->Om = c->kappa = c->cos_t = c->sin_t = nullptr;
     c->inside = nullptr; c->mom_force = c->mom_torque = nullptr; c->flag_dev = nullptr;
-    c->mom_valid = c->vel_set = false;
+    c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
     c->opt_kernel = 0; c->opt_fuse_t = 1; c->opt_fuse_mom = 1;
     c->checked_dt = NAN; c->launches = 0; c->kname[0] = 0;
@@ -275,6 +377,10 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     CR(cudaGetLastError());
     c->launches++;
 #undef CR
+    {
+        mm_status ts = build_tensor_maps(c);
+        if (ts != MM_OK) { std::string m = c->err; mm_destroy(c); return fail(nullptr, ts, m); }
+    }
     *out = c;
     return MM_OK;
 }
@@ -374,22 +480,25 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         if (flag) return fail(c, MM_ERR_UNSTABLE, "dt violates the positivity bound S8");
         c->checked_dt = dt;
     }
-    const bool want_stream = c->opt_kernel == 2 || (c->opt_kernel == 0 && stream_supported(c));
-    if (c->opt_kernel == 2 && !stream_supported(c))
-        return fail(c, MM_ERR_INVALID_ARG, "streamed kernel does not support this grid/flags");
+    // kernel choice: 0 auto (tile if supported, else generic), 1 generic, 2 warp-streamed (1-D TMA), 3 tile
+    int kind = c->opt_kernel;
+    if (kind == 0) kind = c->tile_ok ? 3 : 1;
+    if (kind == 2 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "streamed kernel does not support this grid/flags");
+    if (kind == 3 && !c->tile_ok) return fail(c, MM_ERR_INVALID_ARG, "tile kernel does not support this grid/flags");
     c->mom_valid = false;
     int remaining = n_sub;
     while (remaining > 0) {
         mm_status s;
         int t = 1;
-        if (want_stream) {
-            t = remaining < c->opt_fuse_t ? remaining : c->opt_fuse_t;
-            const bool mom = c->opt_fuse_mom && remaining == t;
-            s = launch_stream(c, t, mom, dt, c->buf[c->cur], c->buf[c->cur ^ 1]);
-            if (s == MM_OK && mom) c->mom_valid = true;
-        } else {
+        if (kind == 1) {
             s = c->dtype == MM_F64 ? launch_generic<double>(c, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
                                    : launch_generic<float>(c, dt, c->buf[c->cur], c->buf[c->cur ^ 1]);
+        } else {
+            t = remaining < c->opt_fuse_t ? remaining : c->opt_fuse_t;
+            const bool mom = c->opt_fuse_mom && remaining == t;
+            s = kind == 2 ? launch_stream(c, t, mom, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
+                          : launch_tile(c, t, mom, dt, c->cur, c->buf[c->cur ^ 1]);
+            if (s == MM_OK && mom) c->mom_valid = true;
         }
         if (s != MM_OK) return s;
         c->cur ^= 1;
@@ -419,7 +528,7 @@ extern "C" mm_status mm_set_option(mm_ctx *c, mm_option opt, int64_t v)
     if (!c) return MM_ERR_INVALID_ARG;
     switch (opt) {
     case MM_OPT_KERNEL:
-        if (v < 0 || v > 2) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_KERNEL in 0..2");
+        if (v < 0 || v > 3) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_KERNEL in 0..3");
         c->opt_kernel = (int)v; return MM_OK;
     case MM_OPT_FUSE_T:
         if (v < 1 || v > MM_MAX_FUSE_T) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_FUSE_T in 1..MM_MAX_FUSE_T");
