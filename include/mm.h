@@ -78,9 +78,12 @@ typedef struct {
 
 /* Tuning / test options for mm_set_option.  Defaults are what bench.py times. */
 typedef enum {
-    MM_OPT_KERNEL = 0,       /* 0 auto (default); 1 force the generic global-memory kernels;
-                                2 force the warp-streamed TMA kernels (error if the grid is unsupported) */
-    MM_OPT_FUSE_T = 1,       /* max substeps fused per HBM pass by the streamed kernel, 1..MM_MAX_FUSE_T */
+    MM_OPT_KERNEL = 0,       /* 0 auto (default: the fastest measured variant for the dtype and grid, DESIGN.md
+                                "Kernel selection"); 1 force the generic global-memory kernels (any grid, all
+                                flags); 2 force the warp-streamed 1-D-TMA kernels; 3 force the tiled-TMA kernels
+                                (2, 3: MM_ERR_INVALID_ARG from mm_substep if the grid/flags are unsupported) */
+    MM_OPT_FUSE_T = 1,       /* max substeps fused per HBM pass (temporal fusion), 1..MM_MAX_FUSE_T;
+                                default 3 (fp64) / 4 (fp32) */
     MM_OPT_FUSE_MOMENTS = 2  /* 1 (default): the last pass of mm_substep also reduces the moments, so a
                                 following mm_moments is a copy; 0: mm_moments always runs its own pass */
 } mm_option;

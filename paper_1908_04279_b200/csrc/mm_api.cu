@@ -337,7 +337,9 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->inside = nullptr; c->mom_force = c->mom_torque = nullptr; c->flag_dev = nullptr;
     c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
-    c->opt_kernel = 0; c->opt_fuse_t = 1; c->opt_fuse_mom = 1;
+    // measured defaults: fp64 -> tile kernel, 3 substeps per pass;
+    // fp32 -> warp-streamed kernel, 4 substeps per pass
+    c->opt_kernel = 0; c->opt_fuse_t = dtype == MM_F64 ? 3 : 4; c->opt_fuse_mom = 1;
     c->checked_dt = NAN; c->launches = 0; c->kname[0] = 0;
     try { c->dens_cov.assign((size_t)nc, 0); } catch (...) { delete c; return fail(nullptr, MM_ERR_NOMEM, "host allocation failed"); }
 
@@ -480,9 +482,10 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         if (flag) return fail(c, MM_ERR_UNSTABLE, "dt violates the positivity bound S8");
         c->checked_dt = dt;
     }
-    // kernel choice: 0 auto (tile if supported, else generic), 1 generic, 2 warp-streamed (1-D TMA), 3 tile
+    // kernel choice: 0 auto (fp64: tile, fp32: warp-streamed, when the grid is supported; else generic),
+    // 1 generic, 2 warp-streamed (1-D TMA), 3 tile
     int kind = c->opt_kernel;
-    if (kind == 0) kind = c->tile_ok ? 3 : 1;
+    if (kind == 0) kind = (c->dtype == MM_F64 && c->tile_ok) ? 3 : stream_supported(c) ? 2 : 1;
     if (kind == 2 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "streamed kernel does not support this grid/flags");
     if (kind == 3 && !c->tile_ok) return fail(c, MM_ERR_INVALID_ARG, "tile kernel does not support this grid/flags");
     c->mom_valid = false;

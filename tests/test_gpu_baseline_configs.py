@@ -1,0 +1,138 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (default kernel
+selection and fuse depth, borrowed torch buffers, the config's substep count and moment cadence).
+
+The S11 inputs of the whole workload are generated on the host in chunks of configurations and uploaded
+(exactly what bench.py does).  Configurations never interact, so the oracle can compute any
+single configuration of the full-size run on its own: a stratified sample of configurations -- always
+containing c = 0, c = Nc-1 and the configurations that straddle flat offsets 2^31 and 2^32 elements and
+2^32 bytes (SURVEY.md 8(c) "Large configs", H3) -- is compared cell by cell (P1) and moment by moment (P2,
+every cadence point).  configs[0] is small enough to compare ALL configurations.  Over the whole density
+the properties that hold at any size are checked: finite, >= 0, cells outside the disc exactly 0 (C9).
+"""
+import numpy as np
+import pytest
+
+import mm_inputs as mi
+from oracle import mm_oracle as orc
+from util import NPDT, TOL, p1_density, p2_moments
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+ES = {"f64": 8, "f32": 4}
+
+
+def sample_configs(w, n_random=40):
+    g = w.grid
+    if g.nc <= 4096:
+        return list(range(g.nc))
+    pick = {0, 1, g.nc - 2, g.nc - 1}
+    for flat in (2 ** 31, 2 ** 32, 2 ** 32 // ES[w.dtype], 2 ** 33 // ES[w.dtype]):
+        c = flat // g.inner
+        for cc in (c - 1, c):
+            if 0 <= cc < g.nc:
+                pick.add(cc)
+    # stratified: one per equal slice of the configuration range, position inside the slice seeded
+    rng = np.random.default_rng(1234)
+    edges = np.linspace(0, g.nc, n_random + 1).astype(np.int64)
+    for lo, hi in zip(edges[:-1], edges[1:]):
+        pick.add(int(rng.integers(lo, hi)))
+    # one full warp-group neighbourhood (consecutive configurations share a warp / block in the kernels)
+    mid = g.nc // 2
+    pick.update(range(mid, mid + 8))
+    return sorted(pick)
+
+
+@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4])
+def test_full_size_config(idx):
+    import torch
+    from paper_1908_04279_b200 import MM
+
+    w = mi.CONFIGS[idx]
+    g, p = w.grid, w.params
+    free_b, _ = torch.cuda.mem_get_info()
+    if 2 * g.cells * ES[w.dtype] + (3 << 30) > free_b:
+        pytest.skip(f"configs[{idx}] needs {2 * g.cells * ES[w.dtype] / 1e9:.0f} GB of device memory")
+    npdt = NPDT[w.dtype]
+    tdt = torch.float64 if w.dtype == "f64" else torch.float32
+    dev = torch.device("cuda:0")
+    sample = sample_configs(w)
+    sset = set(sample)
+
+    b0 = torch.empty(g.cells, dtype=tdt, device=dev)
+    b1 = torch.empty(g.cells, dtype=tdt, device=dev)
+    mm = MM(g, p, w.dtype, b0, b1)
+
+    # ---- S11 inputs, chunked; keep the sampled configurations' initial densities for the oracle
+    st = mi.Stream(g, p.R, w.seed, w.omega_max)
+    U, V, Om = st.velocities(npdt)
+    chunk = 2048
+    buf = np.empty((min(chunk, g.nc), g.ns, g.nxi, g.neta), npdt)
+    m0 = {}
+    for c0 in range(0, g.nc, chunk):
+        n = min(chunk, g.nc - c0)
+        st.density(n, npdt, out=buf[:n])
+        mm.set_density_range(c0, n, buf[:n])
+        for c in range(c0, c0 + n):
+            if c in sset:
+                m0[c] = buf[c - c0].copy()
+    st.close()
+    mm.set_filament_velocity(U, V, Om)
+
+    # ---- the run bench.py times: n_sub substeps, moments at the cadence (Q20)
+    n_mom = w.n_sub // w.moments_every
+    F = torch.empty((n_mom, g.nc, 2), dtype=torch.float64, device=dev)
+    T = torch.empty((n_mom, g.nc), dtype=torch.float64, device=dev)
+    for k in range(n_mom):
+        mm.substep(w.moments_every, w.dt)
+        mm.moments(F[k], T[k])
+    torch.cuda.synchronize()
+    kname = mm.kernel_name
+    assert not kname.startswith("generic"), kname       # the bandwidth kernels are what is being tested
+    Fh, Th = F.cpu().numpy(), T.cpu().numpy()
+    assert np.isfinite(Fh).all() and np.isfinite(Th).all()
+
+    # ---- whole-density properties (any size): finite, non-negative, exactly 0 outside the disc
+    cur = b0 if (mm.launch_count and _is_current(mm, b0, g, npdt)) else b1
+    view = cur.view(g.nc, g.ns, g.nxi * g.neta)
+    outside = torch.from_numpy(~mi.inside_mask(g.nxi, g.neta).reshape(-1)).to(dev)
+    step = max(1, (1 << 28) // g.inner)
+    for c0 in range(0, g.nc, step):
+        blk = view[c0:c0 + step]
+        assert bool(torch.isfinite(blk).all()) and bool((blk >= 0).all())
+        assert bool((blk[:, :, outside] == 0).all()), "cells outside the disc must be exactly 0"
+        assert bool((blk[:, :, ~outside] > 0).all()), "source term keeps every disc cell positive"
+
+    # ---- sampled configurations against the oracle (runs of consecutive configurations go in one call)
+    tol = TOL[w.dtype]
+    worst = dict(p1=0.0, f=0.0, t=0.0)
+    inside = mi.inside_mask(g.nxi, g.neta)
+    runs, start = [], 0
+    for i in range(1, len(sample) + 1):
+        if i == len(sample) or sample[i] != sample[i - 1] + 1:
+            runs.append((sample[start], i - start))
+            start = i
+    for c, n in runs:
+        m = np.stack([np.asarray(m0[cc], np.float64) for cc in range(c, c + n)])
+        Uc, Vc, Oc = (np.asarray(x[c:c + n], np.float64) for x in (U, V, Om))
+        for k in range(n_mom):
+            m = orc.run(g, p, Uc, Vc, Oc, m, w.moments_every, w.dt, c_first=c)
+            ref = orc.moments(g, p, m, c_first=c)
+            ef, et = p2_moments(Fh[k, c:c + n], Th[k, c:c + n], ref)
+            worst["f"], worst["t"] = max(worst["f"], ef), max(worst["t"], et)
+            assert ef <= tol and et <= tol, f"configs[{idx}] c={c}+{n} moments #{k}: P2 {ef:.3e} {et:.3e} ({kname})"
+        out = np.empty((n, g.ns, g.nxi, g.neta), npdt)
+        mm.get_density_range(c, n, out)
+        e1 = p1_density(out, m)
+        worst["p1"] = max(worst["p1"], e1)
+        assert (out[:, :, ~inside] == 0).all()
+        assert e1 <= tol, f"configs[{idx}] c={c}+{n}: P1 {e1:.3e} ({kname})"
+    mm.destroy()
+    print(f"configs[{idx}] {w.name} {kname}: {len(sample)} configurations vs oracle: "
+          f"P1 {worst['p1']:.2e}  P2 force {worst['f']:.2e} torque {worst['t']:.2e}  (tol {tol})")
+
+
+def _is_current(mm, b0, g, npdt):
+    """True when b0 holds the current density: compare configuration 0 read through the ABI with b0's."""
+    out = np.empty((1, g.ns, g.nxi, g.neta), npdt)
+    mm.get_density_range(0, 1, out)
+    return np.array_equal(out.reshape(-1), b0[:g.inner].cpu().numpy())
