@@ -13,6 +13,7 @@
 #include "mm_generic.cuh"
 #include "mm_stream.cuh"
 #include "mm_tile.cuh"
+#include "mm_coef.cuh"
 
 using namespace mm;
 
@@ -167,6 +168,78 @@ static mm_status launch_stream(mm_ctx *c, int T, bool mom, double dt, const void
                    : launch_stream_shape<double, 8, 8, 2>(c, T, mom, dt, in, out);
     return big ? launch_stream_shape<float, 16, 16, 4>(c, T, mom, dt, in, out)
                : launch_stream_shape<float, 8, 8, 2>(c, T, mom, dt, in, out);
+}
+
+// ---- coefficient-form kernel dispatch -----------------------------------------------------------
+#ifndef MM_COEF_P
+#define MM_COEF_P 2
+#endif
+#ifndef MM_COEF_D
+#define MM_COEF_D 3
+#endif
+#ifndef MM_COEF_WARPS
+#define MM_COEF_WARPS 4
+#endif
+#ifndef MM_COEF_MINB_F32
+#define MM_COEF_MINB_F32 2
+#endif
+#ifndef MM_COEF_MINB_F64
+#define MM_COEF_MINB_F64 2
+#endif
+
+template <typename real, int NXI, int NETA, int CB, int T, bool MOM>
+static mm_status launch_coef_inst(mm_ctx *c, double dt, const void *in, void *out)
+{
+    constexpr int P = MM_COEF_P, D = MM_COEF_D, WARPS = MM_COEF_WARPS;
+    constexpr int MINB = sizeof(real) == 8 ? MM_COEF_MINB_F64 : MM_COEF_MINB_F32;
+    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS>;
+    auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB>;
+    static int blocks_per_sm = 0;
+    if (blocks_per_sm == 0) {
+        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
+        int n = 0;
+        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, Cfg::SMEM_BYTES));
+        if (n < 1) return fail(c, MM_ERR_CUDA, "coefficient-form kernel does not fit on an SM");
+        blocks_per_sm = n;
+    }
+    int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
+    const int64_t need = (c->nc + WARPS - 1) / WARPS;
+    if (grid > need) grid = need;
+    KParams<real> kp = make_kparams<real>(c, dt);
+    kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(kp, (const real *)in, (real *)out, c->mom_force,
+                                                                      c->mom_torque);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches++;
+    snprintf(c->kname, sizeof c->kname, "coef<%s,%dx%d,CB=%d,T=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
+             CB, T, MOM ? ",mom" : "");
+    return MM_OK;
+}
+
+template <typename real, int NXI, int NETA, int CB>
+static mm_status launch_coef_shape(mm_ctx *c, int T, bool mom, double dt, const void *in, void *out)
+{
+#define MM_CASE(TT)                                                                                     \
+    case TT:                                                                                            \
+        return mom ? launch_coef_inst<real, NXI, NETA, CB, TT, true>(c, dt, in, out)                    \
+                   : launch_coef_inst<real, NXI, NETA, CB, TT, false>(c, dt, in, out);
+    switch (T) {
+        MM_CASE(1)
+        MM_CASE(2)
+        MM_CASE(3)
+        MM_CASE(4)
+    }
+#undef MM_CASE
+    return fail(c, MM_ERR_INVALID_ARG, "unsupported fuse depth");
+}
+
+static mm_status launch_coef(mm_ctx *c, int T, bool mom, double dt, const void *in, void *out)
+{
+    const bool big = c->g.nxi == 16;
+    if (c->dtype == MM_F64)
+        return big ? launch_coef_shape<double, 16, 16, 2>(c, T, mom, dt, in, out)
+                   : launch_coef_shape<double, 8, 8, 2>(c, T, mom, dt, in, out);
+    return big ? launch_coef_shape<float, 16, 16, 4>(c, T, mom, dt, in, out)
+               : launch_coef_shape<float, 8, 8, 2>(c, T, mom, dt, in, out);
 }
 
 // ---- tile-kernel dispatch ---------------------------------------------------------------------
@@ -483,10 +556,11 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         c->checked_dt = dt;
     }
     // kernel choice: 0 auto (fp64: tile, fp32: warp-streamed, when the grid is supported; else generic),
-    // 1 generic, 2 warp-streamed (1-D TMA), 3 tile
+    // 1 generic, 2 warp-streamed (1-D TMA), 3 tile, 4 coefficient form (same grids/flags as 2)
     int kind = c->opt_kernel;
     if (kind == 0) kind = (c->dtype == MM_F64 && c->tile_ok) ? 3 : stream_supported(c) ? 2 : 1;
     if (kind == 2 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "streamed kernel does not support this grid/flags");
+    if (kind == 4 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernel does not support this grid/flags");
     if (kind == 3 && !c->tile_ok) return fail(c, MM_ERR_INVALID_ARG, "tile kernel does not support this grid/flags");
     c->mom_valid = false;
     int remaining = n_sub;
@@ -499,8 +573,9 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         } else {
             t = remaining < c->opt_fuse_t ? remaining : c->opt_fuse_t;
             const bool mom = c->opt_fuse_mom && remaining == t;
-            s = kind == 2 ? launch_stream(c, t, mom, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
-                          : launch_tile(c, t, mom, dt, c->cur, c->buf[c->cur ^ 1]);
+            s = kind == 2   ? launch_stream(c, t, mom, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
+                : kind == 4 ? launch_coef(c, t, mom, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
+                            : launch_tile(c, t, mom, dt, c->cur, c->buf[c->cur ^ 1]);
             if (s == MM_OK && mom) c->mom_valid = true;
         }
         if (s != MM_OK) return s;
@@ -531,7 +606,7 @@ extern "C" mm_status mm_set_option(mm_ctx *c, mm_option opt, int64_t v)
     if (!c) return MM_ERR_INVALID_ARG;
     switch (opt) {
     case MM_OPT_KERNEL:
-        if (v < 0 || v > 3) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_KERNEL in 0..3");
+        if (v < 0 || v > 4) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_KERNEL in 0..4");
         c->opt_kernel = (int)v; return MM_OK;
     case MM_OPT_FUSE_T:
         if (v < 1 || v > MM_MAX_FUSE_T) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_FUSE_T in 1..MM_MAX_FUSE_T");

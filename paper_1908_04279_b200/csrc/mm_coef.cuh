@@ -1,0 +1,316 @@
+// mm_coef.cuh -- the issue-lean kernel: fused advect + react (+ moments), T substeps per HBM pass (sm_100a).
+//
+// Same data movement as mm_stream.cuh (one warp streams one configuration through its Ns offset planes; a
+// warp-private ring of shared-memory slots filled by 1-D TMA bulk copies on mbarriers; T levels applied to plane j
+// as soon as it arrives, plane j-1 of every level kept in registers; direct 128-bit stores).  What differs is the
+// arithmetic, rebuilt around the measured issue rates of sm_100a (profiles/r01b_ubench.md): selects, integer
+// compares and predicate traffic are half rate, FMNMX-free absolute values ride as operand modifiers, and a
+// 64-bit max/min is microcoded.  So:
+//  * S5-S7 in COEFFICIENT form.  With the half face velocity h = (dt/2dxi) A the upwind split needs no compare:
+//    max(A,0) dt/dxi = h + |h|, min(A,0) dt/dxi = h - |h|.  Everything that does not depend on the level -- the
+//    five neighbour coefficients of every owned cell, already multiplied by the disc mask and with the ghost
+//    cells' coefficients zeroed -- is built ONCE per plane and reused by all T levels:
+//        c0j = mask (1 - dt W/ds - dt kappa_j - [h_t - h_b] - [h_r - h_l]) - mask (|h_t| + |h_b| + |h_r| + |h_l|)
+//        cxm = mask (h_b + |h_b|)   cxp = mask (|h_t| - h_t)   cem = mask (h_l + |h_l|)   cep = mask (|h_r| - h_r)
+//    ([h_t - h_b] does not depend on s, so it is folded per configuration.)
+//  * One level is then 6 FMAs per cell (self + source, s-upwind plane, four offset neighbours) and one shuffle per
+//    patch-edge value; there is no select, no compare and no boundary flux in the level loop.  Lanes at the box
+//    edge multiply whatever the shuffle returned by an exact 0.
+//  * MOM: the last level adds the three S9 sums per lane; one shuffle reduction and one plain store per
+//    configuration -- no atomics.
+#pragma once
+#include "mm_common.cuh"
+#include "mm_ptx.cuh"
+
+namespace mm {
+
+template <typename real, int N>
+struct alignas(sizeof(real) * N) CVec {
+    real v[N];
+};
+
+__device__ __forceinline__ float rabs(float x) { return fabsf(x); }
+__device__ __forceinline__ double rabs(double x) { return fabs(x); }
+
+template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS>
+struct CoefCfg {
+    static constexpr int LB = NETA / CB;       // lanes per patch row
+    static constexpr int G = 32 / LB;          // patch rows per plane
+    static constexpr int QA = NXI / G;         // rows per patch
+    static constexpr int PLANE = NXI * NETA;
+    static_assert(NETA % CB == 0 && 32 % LB == 0 && LB <= 32 && NXI % G == 0 && QA >= 1, "unsupported patch shape");
+    static constexpr int VW = CB * sizeof(real) >= 16 ? 16 / sizeof(real) : CB;   // elements per shared/global access
+    static_assert((PLANE * sizeof(real)) % 16 == 0 && CB % VW == 0 && (VW * sizeof(real)) % 8 == 0, "16-byte bulk copies, 64/128-bit rows");
+    static constexpr size_t RING_BYTES = (size_t)D * P * PLANE * sizeof(real);
+    static constexpr size_t TABLE_BYTES = (((size_t)PLANE * sizeof(real)) + 127) / 128 * 128;
+    static constexpr size_t SMEM_BYTES = TABLE_BYTES + WARPS * RING_BYTES + (size_t)WARPS * D * sizeof(uint64_t);
+};
+
+template <typename real, int NXI, int NETA, int CB, int T, bool MOM, int P, int D, int WARPS, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB)
+    substep_coef_kernel(const __grid_constant__ KParams<real> kp, const real *__restrict__ in, real *__restrict__ out,
+                        double *__restrict__ force, double *__restrict__ torque)
+{
+    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS>;
+    constexpr int LB = Cfg::LB, G = Cfg::G, QA = Cfg::QA, PLANE = Cfg::PLANE;
+    constexpr int VW = Cfg::VW;
+    using V128 = CVec<real, VW>;
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    real *kap_s = reinterpret_cast<real *>(smem_raw);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    real *ring = reinterpret_cast<real *>(smem_raw + Cfg::TABLE_BYTES + (size_t)warp * Cfg::RING_BYTES);
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + Cfg::TABLE_BYTES + (size_t)WARPS * Cfg::RING_BYTES) +
+                     warp * D;
+
+    for (int i = threadIdx.x; i < PLANE; i += WARPS * 32) kap_s[i] = kp.kappa[i];
+    if (lane == 0) {
+#pragma unroll
+        for (int d = 0; d < D; ++d) mbar_init(&full[d], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    // ---- lane's patch and configuration-independent constants
+    const int g = lane / LB, lb = lane - g * LB;
+    const int a0 = g * QA, b0 = lb * CB;
+    const bool is_g0 = (g == 0), is_gtop = (g == G - 1), is_l0 = (lb == 0), is_lr = (lb == LB - 1);
+    real maskf[QA][CB], srcm[QA][CB], xiq[QA], etab[CB];
+#pragma unroll
+    for (int q = 0; q < QA; ++q) {
+        xiq[q] = -kp.R + (real(a0 + q) + real(0.5)) * kp.dxi;
+#pragma unroll
+        for (int cb = 0; cb < CB; ++cb) {
+            maskf[q][cb] = kp.inside[(a0 + q) * NETA + b0 + cb] ? real(1) : real(0);
+            srcm[q][cb] = maskf[q][cb] * kp.dt_src;   // S6 source, 0 outside the disc
+        }
+    }
+#pragma unroll
+    for (int cb = 0; cb < CB; ++cb) etab[cb] = -kp.R + (real(b0 + cb) + real(0.5)) * kp.deta;
+    const real hdx = real(0.5) * kp.dt_dxi, hde = real(0.5) * kp.dt_deta;
+
+    const int ns = kp.ns;
+    const int64_t inner = (int64_t)ns * PLANE;
+    const int CH = (ns + P - 1) / P;
+    const int64_t gw = (int64_t)blockIdx.x * WARPS + warp, nw = (int64_t)gridDim.x * WARPS;
+    const int64_t my_n = gw < kp.nc ? (kp.nc - gw + nw - 1) / nw : 0;
+    const int64_t total = my_n * CH;
+
+    // producer state (lane 0): next chunk to request
+    int64_t pk = 0;
+    int pch = 0, pslot = 0;
+    auto issue = [&]() {   // lane 0 only: TMA bulk copy of the next stream chunk into its ring slot
+        const int64_t c = gw + pk * nw;
+        const int planes = min(P, ns - pch * P);
+        const uint32_t bytes = (uint32_t)(planes * PLANE * sizeof(real));
+        mbar_expect_tx(&full[pslot], bytes);
+        tma_load_1d(ring + (size_t)pslot * P * PLANE, in + c * inner + (int64_t)pch * P * PLANE, bytes, &full[pslot]);
+        if (++pslot == D) pslot = 0;
+        if (++pch == CH) { pch = 0; ++pk; }
+    };
+    if (lane == 0)
+        for (int64_t i = 0; i < total && i < D; ++i) issue();
+
+    // ---- per-configuration registers (S2-S4, S6 folded; everything that does not depend on s)
+    real h0x[QA + 1][CB];   // (dt/2dxi)  A_xi  at s = 0 on the xi faces below rows a0 .. a0+QA        (S4)
+    real h0e[QA][CB + 1];   // (dt/2deta) A_eta at s = 0 on the eta faces left of columns b0 .. b0+CB
+    real c0m[QA][CB];       // mask (1 - dt W/ds - dt kappa - [h_t - h_b] - [h_r - h_l])
+    real csm[QA][CB];       // mask dt W/ds                                                            (S5, s flux)
+    real hbx = 0, hbe = 0, ct = 0, st = 0;
+    real R[T][QA][CB];      // plane j-1 at levels n .. n+T-1
+    real FX = 0, FY = 0, TQ = 0;
+
+    int64_t k = 0, c = 0;
+    int ch = 0, slot = 0;
+    uint32_t phase = 0;
+    for (int64_t i = 0; i < total; ++i) {
+        if (ch == 0) {
+            c = gw + k * nw;
+            const int kth = (int)(c % kp.ntheta);
+            ct = kp.cos_t[kth];
+            st = kp.sin_t[kth];
+            const real U = kp.U[c], Vv = kp.V[c], Om = kp.Om[c];
+            hbx = -hdx * Om * st;   // d/ds_j of h_xi   (S4: A_xi = U + w cos - s Omega sin)
+            hbe = hde * Om * ct;    // d/ds_j of h_eta  (S4: A_eta = V + w sin + s Omega cos)
+#pragma unroll
+            for (int fq = 0; fq <= QA; ++fq) {
+                const real xif = -kp.R + real(a0 + fq) * kp.dxi;   // face below row a0+fq
+#pragma unroll
+                for (int cb = 0; cb < CB; ++cb)
+                    h0x[fq][cb] = hdx * (U + walk_speed(kp.v0, kp.kload, ct, st, xif, etab[cb]) * ct);
+            }
+#pragma unroll
+            for (int q = 0; q < QA; ++q) {
+#pragma unroll
+                for (int fb = 0; fb <= CB; ++fb) {
+                    const real etaf = -kp.R + real(b0 + fb) * kp.deta;   // face left of column b0+fb
+                    h0e[q][fb] = hde * (Vv + walk_speed(kp.v0, kp.kload, ct, st, xiq[q], etaf) * st);
+                }
+#pragma unroll
+                for (int cb = 0; cb < CB; ++cb) {
+                    const real cs = kp.dt_ds * walk_speed(kp.v0, kp.kload, ct, st, xiq[q], etab[cb]);
+                    const real lin = (h0x[q + 1][cb] - h0x[q][cb]) + (h0e[q][cb + 1] - h0e[q][cb]);
+                    csm[q][cb] = maskf[q][cb] * cs;
+                    c0m[q][cb] = maskf[q][cb] * (real(1) - cs - kp.dt * kap_s[(a0 + q) * NETA + b0 + cb] - lin);
+                }
+            }
+#pragma unroll
+            for (int lv = 0; lv < T; ++lv)
+#pragma unroll
+                for (int q = 0; q < QA; ++q)
+#pragma unroll
+                    for (int cb = 0; cb < CB; ++cb) R[lv][q][cb] = real(0);   // zero inflow at s_lo (S5)
+            FX = FY = TQ = real(0);
+        }
+
+        mbar_wait(&full[slot], phase);
+        const real *sp = ring + (size_t)slot * P * PLANE;
+        real *oc = out + c * inner;
+#pragma unroll 1
+        for (int pl = 0; pl < P; ++pl) {
+            const int j = ch * P + pl;
+            if (j >= ns) break;
+            const real sj = kp.s_lo + (real(j) + real(0.5)) * kp.ds;
+            // ---- level-independent coefficients of this plane
+            real c0j[QA][CB], cxm[QA][CB], cxp[QA][CB], cem[QA][CB], cep[QA][CB];
+            {
+                real hx[QA + 1][CB], he[QA][CB + 1];
+#pragma unroll
+                for (int fq = 0; fq <= QA; ++fq)
+#pragma unroll
+                    for (int cb = 0; cb < CB; ++cb) hx[fq][cb] = fma(sj, hbx, h0x[fq][cb]);
+#pragma unroll
+                for (int q = 0; q < QA; ++q)
+#pragma unroll
+                    for (int fb = 0; fb <= CB; ++fb) he[q][fb] = fma(sj, hbe, h0e[q][fb]);
+#pragma unroll
+                for (int q = 0; q < QA; ++q)
+#pragma unroll
+                    for (int cb = 0; cb < CB; ++cb) {
+                        const real m = maskf[q][cb];
+                        const real sabs = (rabs(hx[q][cb]) + rabs(hx[q + 1][cb])) + (rabs(he[q][cb]) + rabs(he[q][cb + 1]));
+                        c0j[q][cb] = fma(-m, sabs, c0m[q][cb]);
+                        cxm[q][cb] = m * (hx[q][cb] + rabs(hx[q][cb]));               // max(A,0) on the face below
+                        cxp[q][cb] = m * (rabs(hx[q + 1][cb]) - hx[q + 1][cb]);       // -min(A,0) on the face above
+                        cem[q][cb] = m * (he[q][cb] + rabs(he[q][cb]));
+                        cep[q][cb] = m * (rabs(he[q][cb + 1]) - he[q][cb + 1]);
+                    }
+                // ghost cells beyond the box are 0 (S5): their coefficient is an exact 0 on the edge lanes
+#pragma unroll
+                for (int cb = 0; cb < CB; ++cb) {
+                    cxm[0][cb] = is_g0 ? real(0) : cxm[0][cb];
+                    cxp[QA - 1][cb] = is_gtop ? real(0) : cxp[QA - 1][cb];
+                }
+#pragma unroll
+                for (int q = 0; q < QA; ++q) {
+                    cem[q][0] = is_l0 ? real(0) : cem[q][0];
+                    cep[q][CB - 1] = is_lr ? real(0) : cep[q][CB - 1];
+                }
+                if ((j < kp.n_end) || (j >= ns - kp.n_end)) {   // enhanced end detachment (S6)
+#pragma unroll
+                    for (int q = 0; q < QA; ++q)
+#pragma unroll
+                        for (int cb = 0; cb < CB; ++cb)
+                            c0j[q][cb] = fma(-kp.dt_endx * maskf[q][cb], kap_s[(a0 + q) * NETA + b0 + cb], c0j[q][cb]);
+                }
+            }
+            real x[QA][CB];
+#pragma unroll
+            for (int q = 0; q < QA; ++q)
+#pragma unroll
+                for (int v4 = 0; v4 < CB / VW; ++v4) {
+                    const V128 v = *reinterpret_cast<const V128 *>(sp + pl * PLANE + (a0 + q) * NETA + b0 + v4 * VW);
+#pragma unroll
+                    for (int e = 0; e < VW; ++e) x[q][v4 * VW + e] = v.v[e];
+                }
+#pragma unroll
+            for (int lv = 0; lv < T; ++lv) {
+                real up[CB], dn[CB], lf[QA], rt[QA];
+#pragma unroll
+                for (int cb = 0; cb < CB; ++cb) {
+                    up[cb] = shfl_down_r(x[0][cb], LB);
+                    dn[cb] = shfl_up_r(x[QA - 1][cb], LB);
+                }
+#pragma unroll
+                for (int q = 0; q < QA; ++q) {
+                    rt[q] = shfl_down_r(x[q][0], 1);
+                    lf[q] = shfl_up_r(x[q][CB - 1], 1);
+                }
+                real nx[QA][CB];
+#pragma unroll
+                for (int q = 0; q < QA; ++q)
+#pragma unroll
+                    for (int cb = 0; cb < CB; ++cb) {
+                        real acc = fma(c0j[q][cb], x[q][cb], srcm[q][cb]);
+                        acc = fma(csm[q][cb], R[lv][q][cb], acc);
+                        if (q > 0) acc = fma(cxm[q][cb], x[q - 1][cb], acc);
+                        if (q + 1 < QA) acc = fma(cxp[q][cb], x[q + 1][cb], acc);
+                        if (cb > 0) acc = fma(cem[q][cb], x[q][cb - 1], acc);
+                        if (cb + 1 < CB) acc = fma(cep[q][cb], x[q][cb + 1], acc);
+                        if (q == 0) acc = fma(cxm[q][cb], dn[cb], acc);
+                        if (q + 1 == QA) acc = fma(cxp[q][cb], up[cb], acc);
+                        if (cb == 0) acc = fma(cem[q][cb], lf[q], acc);
+                        if (cb + 1 == CB) acc = fma(cep[q][cb], rt[q], acc);
+                        nx[q][cb] = acc;
+                    }
+#pragma unroll
+                for (int q = 0; q < QA; ++q)
+#pragma unroll
+                    for (int cb = 0; cb < CB; ++cb) {
+                        R[lv][q][cb] = x[q][cb];
+                        x[q][cb] = nx[q][cb];
+                    }
+            }
+            // ---- store level T of plane j; S9 partial sums
+#pragma unroll
+            for (int q = 0; q < QA; ++q)
+#pragma unroll
+                for (int v4 = 0; v4 < CB / VW; ++v4) {
+                    V128 v;
+#pragma unroll
+                    for (int e = 0; e < VW; ++e) v.v[e] = x[q][v4 * VW + e];
+                    *reinterpret_cast<V128 *>(oc + (int64_t)j * PLANE + (a0 + q) * NETA + b0 + v4 * VW) = v;
+                }
+            if (MOM) {
+                real fxp = 0, fyp = 0;
+#pragma unroll
+                for (int q = 0; q < QA; ++q) {
+                    real rs = x[q][0];
+#pragma unroll
+                    for (int cb = 1; cb < CB; ++cb) rs += x[q][cb];
+                    fxp = fma(xiq[q], rs, fxp);
+                }
+#pragma unroll
+                for (int cb = 0; cb < CB; ++cb) {
+                    real csum = x[0][cb];
+#pragma unroll
+                    for (int q = 1; q < QA; ++q) csum += x[q][cb];
+                    fyp = fma(etab[cb], csum, fyp);
+                }
+                FX += fxp;
+                FY += fyp;
+                TQ = fma(sj, ct * fyp - st * fxp, TQ);
+            }
+        }
+        // every lane has consumed this slot (its values fed the stores above): refill it
+        __syncwarp();
+        if (lane == 0 && i + D < total) issue();
+        if (++slot == D) { slot = 0; phase ^= 1u; }
+
+        if (++ch == CH) {
+            if (MOM) {
+                // S9: fp64 from the cross-lane reduction on (fp32 contexts: fp32 within a lane)
+                double fx = warp_sum((double)FX), fy = warp_sum((double)FY), tq = warp_sum((double)TQ);
+                if (lane == 0) {
+                    force[2 * c] = kp.mom_scale * fx;
+                    force[2 * c + 1] = kp.mom_scale * fy;
+                    torque[c] = kp.mom_scale * tq;
+                }
+            }
+            ch = 0;
+            ++k;
+        }
+    }
+}
+
+}  // namespace mm

@@ -188,3 +188,73 @@ def test_tile_dirty_masked_input_is_dropped():
     out, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [2], dt, kernel=3, fuse_t=2)
     ref, _ = oracle_run(g, p, U, V, Om, m0, [2], dt)
     assert p1_density(out, ref) < TOL["f64"]
+
+
+# ------------------------------------------------------------------ coefficient-form kernels (mm_coef.cuh)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("T", [1, 2, 3, 4])
+@pytest.mark.parametrize("nxi", [16, 8])
+def test_coef_kernel_parity(dtype, T, nxi):
+    # Ns=7: ragged last chunk (P=2); 700 configurations: several per warp
+    g = Grid(5, 7, 20, 7, nxi, nxi)
+    p = Params()
+    e, info = check_parity(g, p, dtype, [5, 3], _dt(g, p), kernel=4, fuse_t=T)
+    assert info["kernel"].startswith("coef<"), info
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_coef_many_configs_per_warp(dtype):
+    g = Grid(16, 16, 16, 6, 8, 8)   # 4096 configs of 384 cells
+    p = Params()
+    check_parity(g, p, dtype, [4], _dt(g, p), kernel=4, fuse_t=2)
+
+
+def test_coef_equals_generic_and_fusion_invariance():
+    g = Grid(3, 3, 8, 10, 16, 16)
+    p = Params()
+    dt = _dt(g, p)
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    ref, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [7], dt, kernel=1)
+    for T in (1, 2, 3, 4):
+        out, _, info = gpu_run(g, p, "f64", U, V, Om, m0, [7], dt, kernel=4, fuse_t=T)
+        assert p1_density(out, ref) < 1e-13, (T, info)
+    a, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [3, 4], dt, kernel=4, fuse_t=2)
+    b, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [7], dt, kernel=4, fuse_t=2)
+    assert p1_density(a, b) < 1e-13
+
+
+def test_coef_moments_fused_equals_standalone():
+    g = Grid(2, 3, 8, 12, 16, 16)
+    p = Params()
+    dt = _dt(g, p)
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    _, mf, _ = gpu_run(g, p, "f64", U, V, Om, m0, [4, 4], dt, kernel=4, fuse_t=2, fuse_mom=1)
+    _, ms, _ = gpu_run(g, p, "f64", U, V, Om, m0, [4, 4], dt, kernel=4, fuse_t=2, fuse_mom=0)
+    for (f1, t1), (f2, t2) in zip(mf, ms):
+        assert np.allclose(f1, f2, rtol=0, atol=1e-14) and np.allclose(t1, t2, rtol=0, atol=1e-14)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_coef_stall_clamp_wide_ends_and_omega2(dtype):
+    g = Grid(2, 2, 8, 9, 16, 16)
+    p = Params(k_spring=200.0, n_end_cells=2, end_detach_mult=3.0)
+    check_parity(g, p, dtype, [6], 0.25 * _dt(g, p, 2.0), omega_max=2.0, kernel=4, fuse_t=3)
+
+
+def test_coef_zero_rates_and_zero_speed():
+    """Degenerate parameters: no source, no walking (v0 = 0), no springs -- the coefficient folding must not
+    divide by or depend on any of them."""
+    g = Grid(1, 2, 8, 8, 16, 16)
+    p = Params(k_on=0.0, v0=0.0, k_spring=0.0)
+    check_parity(g, p, "f64", [5], _dt(g, Params()), kernel=4, fuse_t=2)
+
+
+def test_coef_dirty_masked_input_is_dropped():
+    g = Grid(1, 2, 4, 6, 16, 16)
+    p = Params()
+    dt = _dt(g, p)
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    m0 = m0.copy(); m0[:, :, ~mi.inside_mask(16, 16)] = 3.0
+    out, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [2], dt, kernel=4, fuse_t=2)
+    ref, _ = oracle_run(g, p, U, V, Om, m0, [2], dt)
+    assert p1_density(out, ref) < TOL["f64"]
