@@ -192,8 +192,10 @@ static mm_status launch_coef_inst(mm_ctx *c, double dt, const void *in, void *ou
 {
     constexpr int P = MM_COEF_P, D = MM_COEF_D, WARPS = MM_COEF_WARPS;
     constexpr int MINB = sizeof(real) == 8 ? MM_COEF_MINB_F64 : MM_COEF_MINB_F32;
-    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS>;
-    auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB>;
+    constexpr bool PM = sizeof(real) == 8;   // post-mask: fp64 only
+    constexpr bool CS = sizeof(real) == 8;   // per-configuration constants in shared memory: fp64 only
+    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
+    auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB, PM, CS>;
     static int blocks_per_sm = 0;
     if (blocks_per_sm == 0) {
         CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));

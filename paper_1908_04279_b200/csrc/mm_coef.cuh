@@ -29,10 +29,15 @@ struct alignas(sizeof(real) * N) CVec {
     real v[N];
 };
 
+__device__ __forceinline__ double and_mask(double v, int m)
+{
+    return __hiloint2double(__double2hiint(v) & m, __double2loint(v) & m);
+}
+__device__ __forceinline__ float and_mask(float v, int m) { return __int_as_float(__float_as_int(v) & m); }
 __device__ __forceinline__ float rabs(float x) { return fabsf(x); }
 __device__ __forceinline__ double rabs(double x) { return fabs(x); }
 
-template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS>
+template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, bool CS>
 struct CoefCfg {
     static constexpr int LB = NETA / CB;       // lanes per patch row
     static constexpr int G = 32 / LB;          // patch rows per plane
@@ -43,24 +48,34 @@ struct CoefCfg {
     static_assert((PLANE * sizeof(real)) % 16 == 0 && CB % VW == 0 && (VW * sizeof(real)) % 8 == 0, "16-byte bulk copies, 64/128-bit rows");
     static constexpr size_t RING_BYTES = (size_t)D * P * PLANE * sizeof(real);
     static constexpr size_t TABLE_BYTES = (((size_t)PLANE * sizeof(real)) + 127) / 128 * 128;
-    static constexpr size_t SMEM_BYTES = TABLE_BYTES + WARPS * RING_BYTES + (size_t)WARPS * D * sizeof(uint64_t);
+    // CS: the per-configuration constants of a lane (h0x, h0e, c0m) live in a warp-private shared-memory block
+    // ([vector][lane] so every 128-bit access is conflict-free) and are re-read once per plane, while the plane's
+    // coefficient registers are dead -- the fp64 choice, where they would not fit beside 40 coefficient doubles.
+    static constexpr int NK = (QA + 1) * CB + QA * (CB + 1) + QA * CB;   // constants per lane
+    static constexpr int NKV = (NK + VW - 1) / VW;                       // ... in vectors
+    static constexpr size_t CST_BYTES = CS ? (size_t)NKV * 32 * VW * sizeof(real) : 0;
+    static constexpr size_t WARP_BYTES = RING_BYTES + CST_BYTES;
+    static constexpr size_t SMEM_BYTES = TABLE_BYTES + WARPS * WARP_BYTES + (size_t)WARPS * D * sizeof(uint64_t);
 };
 
-template <typename real, int NXI, int NETA, int CB, int T, bool MOM, int P, int D, int WARPS, int MINB>
+template <typename real, int NXI, int NETA, int CB, int T, bool MOM, int P, int D, int WARPS, int MINB, bool PM, bool CS>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
     substep_coef_kernel(const __grid_constant__ KParams<real> kp, const real *__restrict__ in, real *__restrict__ out,
                         double *__restrict__ force, double *__restrict__ torque)
 {
-    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS>;
-    constexpr int LB = Cfg::LB, G = Cfg::G, QA = Cfg::QA, PLANE = Cfg::PLANE;
+    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
+    constexpr int LB = Cfg::LB, G = Cfg::G, QA = Cfg::QA, PLANE = Cfg::PLANE, NK = Cfg::NK, NKV = Cfg::NKV;
     constexpr int VW = Cfg::VW;
+    constexpr int UNR = CS ? 1 : P;   // plane-loop unroll: full where registers allow (it removes the R <- x moves)
     using V128 = CVec<real, VW>;
+    constexpr int OX = 0, OE = (QA + 1) * CB, OC = OE + QA * (CB + 1);   // offsets of h0x, h0e, c0m in the block
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     real *kap_s = reinterpret_cast<real *>(smem_raw);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    real *ring = reinterpret_cast<real *>(smem_raw + Cfg::TABLE_BYTES + (size_t)warp * Cfg::RING_BYTES);
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + Cfg::TABLE_BYTES + (size_t)WARPS * Cfg::RING_BYTES) +
+    real *ring = reinterpret_cast<real *>(smem_raw + Cfg::TABLE_BYTES + (size_t)warp * Cfg::WARP_BYTES);
+    real *cst = ring + Cfg::RING_BYTES / sizeof(real) + lane * VW;   // this lane's column of the constants block
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + Cfg::TABLE_BYTES + (size_t)WARPS * Cfg::WARP_BYTES) +
                      warp * D;
 
     for (int i = threadIdx.x; i < PLANE; i += WARPS * 32) kap_s[i] = kp.kappa[i];
@@ -75,13 +90,19 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     const int g = lane / LB, lb = lane - g * LB;
     const int a0 = g * QA, b0 = lb * CB;
     const bool is_g0 = (g == 0), is_gtop = (g == G - 1), is_l0 = (lb == 0), is_lr = (lb == LB - 1);
+    // Disc mask (S1/S7).  PM = false: folded into every coefficient (maskf, srcm), free in the level loop.
+    // PM = true ("post-mask", the fp64 choice): coefficients stay unmasked and every level's result is ANDed with
+    // maskw on the otherwise idle integer pipe -- 32 fewer registers and no mask multiplies on the fp64 pipe.
     real maskf[QA][CB], srcm[QA][CB], xiq[QA], etab[CB];
+    int maskw[QA][CB];
 #pragma unroll
     for (int q = 0; q < QA; ++q) {
         xiq[q] = -kp.R + (real(a0 + q) + real(0.5)) * kp.dxi;
 #pragma unroll
         for (int cb = 0; cb < CB; ++cb) {
-            maskf[q][cb] = kp.inside[(a0 + q) * NETA + b0 + cb] ? real(1) : real(0);
+            const bool in = kp.inside[(a0 + q) * NETA + b0 + cb] != 0;
+            maskw[q][cb] = -(int)kp.inside[(a0 + q) * NETA + b0 + cb];   // 0 / ~0, kept opaque so the AND stays an AND
+            maskf[q][cb] = in ? real(1) : real(0);
             srcm[q][cb] = maskf[q][cb] * kp.dt_src;   // S6 source, 0 outside the disc
         }
     }
@@ -112,9 +133,10 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
         for (int64_t i = 0; i < total && i < D; ++i) issue();
 
     // ---- per-configuration registers (S2-S4, S6 folded; everything that does not depend on s)
-    real h0x[QA + 1][CB];   // (dt/2dxi)  A_xi  at s = 0 on the xi faces below rows a0 .. a0+QA        (S4)
-    real h0e[QA][CB + 1];   // (dt/2deta) A_eta at s = 0 on the eta faces left of columns b0 .. b0+CB
-    real c0m[QA][CB];       // mask (1 - dt W/ds - dt kappa - [h_t - h_b] - [h_r - h_l])
+    // kc[OX + fq*CB + cb]     = h0x: (dt/2dxi)  A_xi  at s = 0 on the xi faces below rows a0 .. a0+QA       (S4)
+    // kc[OE + q*(CB+1) + fb]  = h0e: (dt/2deta) A_eta at s = 0 on the eta faces left of columns b0 .. b0+CB
+    // kc[OC + q*CB + cb]      = c0m: mask (1 - dt W/ds - dt kappa - [h_t - h_b] - [h_r - h_l])
+    real kc[NKV * VW];
     real csm[QA][CB];       // mask dt W/ds                                                            (S5, s flux)
     real hbx = 0, hbe = 0, ct = 0, st = 0;
     real R[T][QA][CB];      // plane j-1 at levels n .. n+T-1
@@ -137,21 +159,32 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 const real xif = -kp.R + real(a0 + fq) * kp.dxi;   // face below row a0+fq
 #pragma unroll
                 for (int cb = 0; cb < CB; ++cb)
-                    h0x[fq][cb] = hdx * (U + walk_speed(kp.v0, kp.kload, ct, st, xif, etab[cb]) * ct);
+                    kc[OX + fq * CB + cb] = hdx * (U + walk_speed(kp.v0, kp.kload, ct, st, xif, etab[cb]) * ct);
             }
 #pragma unroll
             for (int q = 0; q < QA; ++q) {
 #pragma unroll
                 for (int fb = 0; fb <= CB; ++fb) {
                     const real etaf = -kp.R + real(b0 + fb) * kp.deta;   // face left of column b0+fb
-                    h0e[q][fb] = hde * (Vv + walk_speed(kp.v0, kp.kload, ct, st, xiq[q], etaf) * st);
+                    kc[OE + q * (CB + 1) + fb] = hde * (Vv + walk_speed(kp.v0, kp.kload, ct, st, xiq[q], etaf) * st);
                 }
 #pragma unroll
                 for (int cb = 0; cb < CB; ++cb) {
                     const real cs = kp.dt_ds * walk_speed(kp.v0, kp.kload, ct, st, xiq[q], etab[cb]);
-                    const real lin = (h0x[q + 1][cb] - h0x[q][cb]) + (h0e[q][cb + 1] - h0e[q][cb]);
-                    csm[q][cb] = maskf[q][cb] * cs;
-                    c0m[q][cb] = maskf[q][cb] * (real(1) - cs - kp.dt * kap_s[(a0 + q) * NETA + b0 + cb] - lin);
+                    const real lin = (kc[OX + (q + 1) * CB + cb] - kc[OX + q * CB + cb]) +
+                                     (kc[OE + q * (CB + 1) + cb + 1] - kc[OE + q * (CB + 1) + cb]);
+                    const real c0 = real(1) - cs - kp.dt * kap_s[(a0 + q) * NETA + b0 + cb] - lin;
+                    csm[q][cb] = PM ? cs : maskf[q][cb] * cs;
+                    kc[OC + q * CB + cb] = PM ? c0 : maskf[q][cb] * c0;
+                }
+            }
+            if (CS) {
+#pragma unroll
+                for (int v = 0; v < NKV; ++v) {
+                    V128 t;
+#pragma unroll
+                    for (int e = 0; e < VW; ++e) t.v[e] = (v * VW + e < NK) ? kc[v * VW + e] : real(0);
+                    *reinterpret_cast<V128 *>(cst + v * 32 * VW) = t;
                 }
             }
 #pragma unroll
@@ -166,34 +199,55 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
         mbar_wait(&full[slot], phase);
         const real *sp = ring + (size_t)slot * P * PLANE;
         real *oc = out + c * inner;
-#pragma unroll 1
+#pragma unroll UNR
         for (int pl = 0; pl < P; ++pl) {
             const int j = ch * P + pl;
-            if (j >= ns) break;
+            // A ragged last chunk (j >= ns) still runs the arithmetic on whatever the slot holds -- straight-line code
+            // keeps the register rotation of the unrolled planes free of copies -- but stores and sums nothing; R is
+            // re-zeroed at the next configuration.
+            const bool live = j < ns;
             const real sj = kp.s_lo + (real(j) + real(0.5)) * kp.ds;
             // ---- level-independent coefficients of this plane
             real c0j[QA][CB], cxm[QA][CB], cxp[QA][CB], cem[QA][CB], cep[QA][CB];
             {
+                real kl[NKV * VW];
+                if (CS) {
+#pragma unroll
+                    for (int v = 0; v < NKV; ++v) {
+                        const V128 t = *reinterpret_cast<const V128 *>(cst + v * 32 * VW);
+#pragma unroll
+                        for (int e = 0; e < VW; ++e) kl[v * VW + e] = t.v[e];
+                    }
+                } else {
+#pragma unroll
+                    for (int e = 0; e < NK; ++e) kl[e] = kc[e];
+                }
                 real hx[QA + 1][CB], he[QA][CB + 1];
 #pragma unroll
                 for (int fq = 0; fq <= QA; ++fq)
 #pragma unroll
-                    for (int cb = 0; cb < CB; ++cb) hx[fq][cb] = fma(sj, hbx, h0x[fq][cb]);
+                    for (int cb = 0; cb < CB; ++cb) hx[fq][cb] = fma(sj, hbx, kl[OX + fq * CB + cb]);
 #pragma unroll
                 for (int q = 0; q < QA; ++q)
 #pragma unroll
-                    for (int fb = 0; fb <= CB; ++fb) he[q][fb] = fma(sj, hbe, h0e[q][fb]);
+                    for (int fb = 0; fb <= CB; ++fb) he[q][fb] = fma(sj, hbe, kl[OE + q * (CB + 1) + fb]);
 #pragma unroll
                 for (int q = 0; q < QA; ++q)
 #pragma unroll
                     for (int cb = 0; cb < CB; ++cb) {
-                        const real m = maskf[q][cb];
                         const real sabs = (rabs(hx[q][cb]) + rabs(hx[q + 1][cb])) + (rabs(he[q][cb]) + rabs(he[q][cb + 1]));
-                        c0j[q][cb] = fma(-m, sabs, c0m[q][cb]);
-                        cxm[q][cb] = m * (hx[q][cb] + rabs(hx[q][cb]));               // max(A,0) on the face below
-                        cxp[q][cb] = m * (rabs(hx[q + 1][cb]) - hx[q + 1][cb]);       // -min(A,0) on the face above
-                        cem[q][cb] = m * (he[q][cb] + rabs(he[q][cb]));
-                        cep[q][cb] = m * (rabs(he[q][cb + 1]) - he[q][cb + 1]);
+                        const real pb = hx[q][cb] + rabs(hx[q][cb]);               // max(A,0) on the face below
+                        const real nt = rabs(hx[q + 1][cb]) - hx[q + 1][cb];       // -min(A,0) on the face above
+                        const real pl_ = he[q][cb] + rabs(he[q][cb]);
+                        const real nr = rabs(he[q][cb + 1]) - he[q][cb + 1];
+                        if (PM) {
+                            c0j[q][cb] = kl[OC + q * CB + cb] - sabs;
+                            cxm[q][cb] = pb; cxp[q][cb] = nt; cem[q][cb] = pl_; cep[q][cb] = nr;
+                        } else {
+                            const real m = maskf[q][cb];
+                            c0j[q][cb] = fma(-m, sabs, kl[OC + q * CB + cb]);
+                            cxm[q][cb] = m * pb; cxp[q][cb] = m * nt; cem[q][cb] = m * pl_; cep[q][cb] = m * nr;
+                        }
                     }
                 // ghost cells beyond the box are 0 (S5): their coefficient is an exact 0 on the edge lanes
 #pragma unroll
@@ -211,7 +265,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     for (int q = 0; q < QA; ++q)
 #pragma unroll
                         for (int cb = 0; cb < CB; ++cb)
-                            c0j[q][cb] = fma(-kp.dt_endx * maskf[q][cb], kap_s[(a0 + q) * NETA + b0 + cb], c0j[q][cb]);
+                            c0j[q][cb] = fma(PM ? -kp.dt_endx : -kp.dt_endx * maskf[q][cb],
+                                             kap_s[(a0 + q) * NETA + b0 + cb], c0j[q][cb]);
                 }
             }
             real x[QA][CB];
@@ -241,8 +296,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 for (int q = 0; q < QA; ++q)
 #pragma unroll
                     for (int cb = 0; cb < CB; ++cb) {
-                        real acc = fma(c0j[q][cb], x[q][cb], srcm[q][cb]);
-                        acc = fma(csm[q][cb], R[lv][q][cb], acc);
+                        real acc = fma(c0j[q][cb], x[q][cb], PM ? kp.dt_src : srcm[q][cb]);
                         if (q > 0) acc = fma(cxm[q][cb], x[q - 1][cb], acc);
                         if (q + 1 < QA) acc = fma(cxp[q][cb], x[q + 1][cb], acc);
                         if (cb > 0) acc = fma(cem[q][cb], x[q][cb - 1], acc);
@@ -251,7 +305,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                         if (q + 1 == QA) acc = fma(cxp[q][cb], up[cb], acc);
                         if (cb == 0) acc = fma(cem[q][cb], lf[q], acc);
                         if (cb + 1 == CB) acc = fma(cep[q][cb], rt[q], acc);
-                        nx[q][cb] = acc;
+                        acc = fma(csm[q][cb], R[lv][q][cb], acc);   // last: the result may reuse R's register
+                        nx[q][cb] = PM ? and_mask(acc, maskw[q][cb]) : acc;
                     }
 #pragma unroll
                 for (int q = 0; q < QA; ++q)
@@ -262,6 +317,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     }
             }
             // ---- store level T of plane j; S9 partial sums
+            if (live) {
 #pragma unroll
             for (int q = 0; q < QA; ++q)
 #pragma unroll
@@ -271,7 +327,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     for (int e = 0; e < VW; ++e) v.v[e] = x[q][v4 * VW + e];
                     *reinterpret_cast<V128 *>(oc + (int64_t)j * PLANE + (a0 + q) * NETA + b0 + v4 * VW) = v;
                 }
-            if (MOM) {
+            }
+            if (MOM && live) {
                 real fxp = 0, fyp = 0;
 #pragma unroll
                 for (int q = 0; q < QA; ++q) {

@@ -23,6 +23,7 @@
 #pragma once
 #include "mm_common.cuh"
 #include "mm_ptx.cuh"
+#include "mm_coef.cuh"   // and_mask
 
 namespace mm {
 
@@ -57,11 +58,6 @@ struct TileCfg {
 
 __device__ __forceinline__ bool is_neg(double a) { return __double2hiint(a) < 0; }
 __device__ __forceinline__ bool is_neg(float a) { return __float_as_int(a) < 0; }
-__device__ __forceinline__ double and_mask(double v, int m)
-{
-    return __hiloint2double(__double2hiint(v) & m, __double2loint(v) & m);
-}
-__device__ __forceinline__ float and_mask(float v, int m) { return __int_as_float(__float_as_int(v) & m); }
 
 template <typename real, int NXI, int NETA, int CB, int T, bool MOM, int P, int D, int WARPS, int MINB>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
