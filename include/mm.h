@@ -80,10 +80,11 @@ typedef struct {
 typedef enum {
     MM_OPT_KERNEL = 0,       /* 0 auto (default: the fastest measured variant for the dtype and grid, DESIGN.md
                                 "Kernel selection"); 1 force the generic global-memory kernels (any grid, all
-                                flags); 2 force the warp-streamed 1-D-TMA kernels; 3 force the tiled-TMA kernels
-                                (2, 3: MM_ERR_INVALID_ARG from mm_substep if the grid/flags are unsupported) */
+                                flags); 2 force the warp-streamed 1-D-TMA kernels; 3 force the tiled-TMA kernels;
+                                4 force the coefficient-form kernels (the default where supported)
+                                (2, 3, 4: MM_ERR_INVALID_ARG from mm_substep if the grid/flags are unsupported) */
     MM_OPT_FUSE_T = 1,       /* max substeps fused per HBM pass (temporal fusion), 1..MM_MAX_FUSE_T;
-                                default 3 (fp64) / 4 (fp32) */
+                                default 4 */
     MM_OPT_FUSE_MOMENTS = 2  /* 1 (default): the last pass of mm_substep also reduces the moments, so a
                                 following mm_moments is a copy; 0: mm_moments always runs its own pass */
 } mm_option;

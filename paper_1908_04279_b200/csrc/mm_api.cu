@@ -171,11 +171,19 @@ static mm_status launch_stream(mm_ctx *c, int T, bool mom, double dt, const void
 }
 
 // ---- coefficient-form kernel dispatch -----------------------------------------------------------
-#ifndef MM_COEF_P
-#define MM_COEF_P 2
+// Launch shape of the coefficient-form kernel, per dtype (measured sweep in profiles/r01b_README.md):
+// planes per TMA copy, ring depth, warps per CTA, resident CTAs per SM asked of the register allocator.
+#ifndef MM_COEF_P_F32
+#define MM_COEF_P_F32 4
 #endif
-#ifndef MM_COEF_D
-#define MM_COEF_D 3
+#ifndef MM_COEF_D_F32
+#define MM_COEF_D_F32 2
+#endif
+#ifndef MM_COEF_P_F64
+#define MM_COEF_P_F64 2
+#endif
+#ifndef MM_COEF_D_F64
+#define MM_COEF_D_F64 3
 #endif
 #ifndef MM_COEF_WARPS
 #define MM_COEF_WARPS 4
@@ -190,7 +198,8 @@ static mm_status launch_stream(mm_ctx *c, int T, bool mom, double dt, const void
 template <typename real, int NXI, int NETA, int CB, int T, bool MOM>
 static mm_status launch_coef_inst(mm_ctx *c, double dt, const void *in, void *out)
 {
-    constexpr int P = MM_COEF_P, D = MM_COEF_D, WARPS = MM_COEF_WARPS;
+    constexpr int P = sizeof(real) == 8 ? MM_COEF_P_F64 : MM_COEF_P_F32;
+    constexpr int D = sizeof(real) == 8 ? MM_COEF_D_F64 : MM_COEF_D_F32, WARPS = MM_COEF_WARPS;
     constexpr int MINB = sizeof(real) == 8 ? MM_COEF_MINB_F64 : MM_COEF_MINB_F32;
     constexpr bool PM = sizeof(real) == 8;   // post-mask: fp64 only
     constexpr bool CS = sizeof(real) == 8;   // per-configuration constants in shared memory: fp64 only
@@ -412,9 +421,8 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->inside = nullptr; c->mom_force = c->mom_torque = nullptr; c->flag_dev = nullptr;
     c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
-    // measured defaults: fp64 -> tile kernel, 3 substeps per pass;
-    // fp32 -> warp-streamed kernel, 4 substeps per pass
-    c->opt_kernel = 0; c->opt_fuse_t = dtype == MM_F64 ? 3 : 4; c->opt_fuse_mom = 1;
+    // measured defaults: the coefficient-form kernel, 4 substeps per pass
+    c->opt_kernel = 0; c->opt_fuse_t = 4; c->opt_fuse_mom = 1;
     c->checked_dt = NAN; c->launches = 0; c->kname[0] = 0;
     try { c->dens_cov.assign((size_t)nc, 0); } catch (...) { delete c; return fail(nullptr, MM_ERR_NOMEM, "host allocation failed"); }
 
@@ -557,10 +565,10 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         if (flag) return fail(c, MM_ERR_UNSTABLE, "dt violates the positivity bound S8");
         c->checked_dt = dt;
     }
-    // kernel choice: 0 auto (fp64: tile, fp32: warp-streamed, when the grid is supported; else generic),
+    // kernel choice: 0 auto (coefficient form when the grid/flags are supported; else generic),
     // 1 generic, 2 warp-streamed (1-D TMA), 3 tile, 4 coefficient form (same grids/flags as 2)
     int kind = c->opt_kernel;
-    if (kind == 0) kind = (c->dtype == MM_F64 && c->tile_ok) ? 3 : stream_supported(c) ? 2 : 1;
+    if (kind == 0) kind = stream_supported(c) ? 4 : 1;
     if (kind == 2 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "streamed kernel does not support this grid/flags");
     if (kind == 4 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernel does not support this grid/flags");
     if (kind == 3 && !c->tile_ok) return fail(c, MM_ERR_INVALID_ARG, "tile kernel does not support this grid/flags");
