@@ -129,7 +129,9 @@ def pick_workload(idx, free_bytes=None):
 def rank_workload(w: mi.Workload, rank: int):
     """Weak scaling: configurations never interact, so rank r runs its own copy of the workload
     grid -- the r-th x-slab of a world-times-larger periodic domain -- drawn from seed + r.  No data-path collective."""
-    return mi.Workload(w.name, w.grid, w.dtype, w.n_sub, w.moments_every, w.omega_max, w.seed + rank, w.params)
+    from paper_1908_04279_b200 import shard
+    return mi.Workload(w.name, w.grid, w.dtype, w.n_sub, w.moments_every, w.omega_max, shard.rank_seed(w.seed, rank),
+                       w.params)
 
 
 def upload_inputs(mm, w, chunk_configs=2048, log=None):
@@ -154,7 +156,7 @@ def upload_inputs(mm, w, chunk_configs=2048, log=None):
 def run_cuda(args):
     import torch
     import torch.distributed as dist
-    from paper_1908_04279_b200 import MM, binding as b
+    from paper_1908_04279_b200 import MM, binding as b, shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -226,11 +228,7 @@ def run_cuda(args):
             step(U, V, Om, F, T, record)
         e1.record(stream)
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = shard.max_over_ranks(e0.elapsed_time(e1), dev)
         return ms, mm.launch_count - l0
 
     # ---- warm-up, then the timed region (inputs resident in HBM)
@@ -242,7 +240,7 @@ def run_cuda(args):
     clocks = sampler.stop()
     kname = mm.kernel_name
     updates_per_step = g.cells * w.n_sub * world
-    value = updates_per_step * args.steps / (ms * 1e-3) / 1e9
+    value = shard.whole_job_rate(g.cells * w.n_sub, args.steps, world, ms) / 1e9
 
     # ---- dominant kernel: average launch duration over the timed region (CUDA events on the library's stream)
     sub_ms = sum(a.elapsed_time(c) for a, c, _ in sub_events)
