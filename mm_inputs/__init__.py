@@ -55,6 +55,7 @@ def _load():
 FLAG_S_PERIODIC = 1
 FLAG_OFFSET_PERIODIC_NOMASK = 2
 FLAG_CHECK_DT = 4
+FLAG_RK2_SUPERBEE = 8   # the paper's RK2 + Superbee-in-s scheme instead of forward Euler + upwind
 
 
 @dataclass(frozen=True)

@@ -21,6 +21,20 @@
  * C5 brute-force/analytic moments on 2x2x2x4x3x3, C6 single-cell delta column, C7 point
  * symmetry, C8 independence/additivity, C9 positivity/affinity.  No function is unpinned.
  *
+ * Second scheme (flag MMO_RK2_SUPERBEE): the paper's own integrator --
+ * Runge-Kutta 2 through the half step (Alg. 2 l.9-10: "Compute M_b(t^* + dt^* / 2)",
+ * "Compute M_b(t^* + dt^*)"; "We instead use Runge-Kutta 2, which only requires the M_b array at
+ * t^{n+1} and t^n") with the Superbee flux limiter in the arclength dimension
+ * ("applies a Superbee flux limiter"; "The Superbee flux limiter operates
+ * in the arclength s dimension ... neighborhood access pattern of (s-2,s-1,s,s+1,s+2)").  The paper
+ * prints neither formula; the readings (Q27-Q30) are: midpoint RK2 as a method of lines,
+ *     m* = m^n + (dt/2) L(m^n),   m^{n+1} = m^n + dt L(m*),
+ * L(m) = -div F(m) + src - kappa m, both stages masked to the disc; the s flux on face j+1/2 is
+ * W (m_j + sigma_j / 2) with the Superbee-limited slope in its division-free form
+ *     sigma_j = maxmod( minmod(2a, b), minmod(a, 2b) ),  a = m_j - m_{j-1},  b = m_{j+1} - m_j
+ * (= phi(r) b with phi(r) = max(0, min(2r,1), min(r,2)), r = a/b); ghosts beyond both ends of s
+ * are 0 as in S5; (xi, eta) stay first-order upwind.  Pins R1-R7 in tests/test_oracle_rk2_pins.py.
+ *
  * Parallelism: `#pragma omp parallel for` over configurations only (they never interact).
  */
 #include <math.h>
@@ -42,6 +56,7 @@ typedef struct {
 
 #define MMO_S_PERIODIC 1u
 #define MMO_OFFSET_PERIODIC_NOMASK 2u
+#define MMO_RK2_SUPERBEE 8u   /* bit 2 (4u) is the product's CHECK_DT flag; unused here */
 
 static const double MMO_PI = 3.14159265358979323846264338327950288;
 
@@ -65,12 +80,30 @@ static double walk_speed(const mmo_params *p, double ct, double st, double xi, d
 static double dmax(double a, double b) { return a > b ? a : b; }
 static double dmin(double a, double b) { return a < b ? a : b; }
 
-/* One explicit substep (S2..S7) of ONE configuration.
- * m, mnew: [ns][nxi][neta], b fastest.  scratch: 3 flux arrays (sizes below). */
-static void substep_config(const mmo_grid *g, const mmo_params *p, int itheta,
-                           double U, double V, double Om, double dt,
-                           const double *m, double *mnew,
-                           double *Fs, double *Fxi, double *Feta)
+/* Superbee-limited slope (division-free form; LeVeque's maxmod/minmod statement of the limiter the
+ * paper names at PAPER.md:89, 175).  a = backward difference, b = forward difference. */
+static double minmod(double a, double b)
+{
+    if (a * b <= 0.0) return 0.0;
+    return a > 0.0 ? dmin(a, b) : dmax(a, b);
+}
+static double maxmod(double a, double b)
+{
+    if (a * b <= 0.0) return 0.0;
+    return a > 0.0 ? dmax(a, b) : dmin(a, b);
+}
+static double superbee_slope(double a, double b) { return maxmod(minmod(2.0 * a, b), minmod(a, 2.0 * b)); }
+
+/* One explicit stage (S2..S7) of ONE configuration:
+ *     mnew = inside ? mbase + dt * L(m) : 0,    L(m) = -div F(m) + src - kappa m.
+ * Forward Euler (the north_star scheme) is the single stage mbase = m.  RK2 calls it twice
+ * (mbase = m^n both times; m = m^n with dt/2, then m = m* with dt).  `limited` switches the s flux
+ * from first-order upwind to the Superbee-limited one.
+ * m, mbase, mnew: [ns][nxi][neta], b fastest.  scratch: 3 flux arrays (sizes below). */
+static void stage_config(const mmo_grid *g, const mmo_params *p, int itheta,
+                         double U, double V, double Om, double dt,
+                         const double *mbase, const double *m, double *mnew, int limited,
+                         double *Fs, double *Fxi, double *Feta)
 {
     const int ns = g->ns, nxi = g->nxi, neta = g->neta;
     const int per_s = (p->flags & MMO_S_PERIODIC) != 0;
@@ -87,7 +120,18 @@ static void substep_config(const mmo_grid *g, const mmo_params *p, int itheta,
         for (int b = 0; b < neta; ++b) {
             double xi = -R + (a + 0.5) * dxi, eta = -R + (b + 0.5) * deta;
             double W = walk_speed(p, ct, st, xi, eta);            /* S4: W[c,a,b] */
-            for (int jf = 1; jf <= ns; ++jf) FS(jf, a, b) = W * M(jf - 1, a, b);
+            if (!limited) {
+                for (int jf = 1; jf <= ns; ++jf) FS(jf, a, b) = W * M(jf - 1, a, b);
+            } else {
+                /* Superbee in s: face jf takes cell j = jf-1 plus half its limited slope */
+                for (int jf = 1; jf <= ns; ++jf) {
+                    int j = jf - 1;
+                    double mc = M(j, a, b);
+                    double mm1 = j >= 1 ? M(j - 1, a, b) : (per_s ? M(ns - 1, a, b) : 0.0);
+                    double mp1 = j + 1 < ns ? M(j + 1, a, b) : (per_s ? M(0, a, b) : 0.0);
+                    FS(jf, a, b) = W * (mc + 0.5 * superbee_slope(mc - mm1, mp1 - mc));
+                }
+            }
             FS(0, a, b) = per_s ? FS(ns, a, b) : 0.0;             /* zero inflow at s = s_lo (Q9) */
         }
     /* S5, xi-faces.  index af = 0..nxi is the face xi_{af - 1/2} = -R + af*dxi. */
@@ -144,7 +188,8 @@ static void substep_config(const mmo_grid *g, const mmo_params *p, int itheta,
                 double div = (FS(j + 1, a, b) - FS(j, a, b)) / ds
                            + (FXI(j, a + 1, b) - FXI(j, a, b)) / dxi
                            + (FETA(j, a, b + 1) - FETA(j, a, b)) / deta;
-                double mp = mc - dt * div + dt * (src - kappa * mc);
+                double mb = mbase[((size_t)j * nxi + a) * neta + b];
+                double mp = mb - dt * div + dt * (src - kappa * mc);
                 mnew[((size_t)j * nxi + a) * neta + b] = in ? mp : 0.0;
             }
     }
@@ -157,7 +202,7 @@ static void substep_config(const mmo_grid *g, const mmo_params *p, int itheta,
 static size_t scratch_doubles(const mmo_grid *g)
 {
     size_t ns = g->ns, nxi = g->nxi, neta = g->neta;
-    return (ns + 1) * nxi * neta + ns * (nxi + 1) * neta + ns * nxi * (neta + 1) + ns * nxi * neta;
+    return (ns + 1) * nxi * neta + ns * (nxi + 1) * neta + ns * nxi * (neta + 1) + 2 * ns * nxi * neta;
 }
 
 /* Advance configurations [0, n_configs) by n_sub substeps of size dt, in place.
@@ -177,10 +222,17 @@ int mmo_run(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_c
         double *Fxi = Fs + (size_t)(g->ns + 1) * g->nxi * g->neta;
         double *Feta = Fxi + (size_t)g->ns * (g->nxi + 1) * g->neta;
         double *tmp = Feta + (size_t)g->ns * g->nxi * (g->neta + 1);
+        double *half = tmp + inner;
         double *cur = m + (size_t)c * inner;
         int itheta = (int)((c_first + c) % g->ntheta);
         for (int n = 0; n < n_sub; ++n) {
-            substep_config(g, p, itheta, U[c], V[c], Om[c], dt, cur, tmp, Fs, Fxi, Feta);
+            if (p->flags & MMO_RK2_SUPERBEE) {
+                /* Alg. 2 l.9: M_b at t + dt/2;  l.10: M_b at t + dt */
+                stage_config(g, p, itheta, U[c], V[c], Om[c], 0.5 * dt, cur, cur, half, 1, Fs, Fxi, Feta);
+                stage_config(g, p, itheta, U[c], V[c], Om[c], dt, cur, half, tmp, 1, Fs, Fxi, Feta);
+            } else {
+                stage_config(g, p, itheta, U[c], V[c], Om[c], dt, cur, cur, tmp, 0, Fs, Fxi, Feta);
+            }
             memcpy(cur, tmp, sizeof(double) * inner);   /* "swap buffers" */
         }
         free(scr);

@@ -20,6 +20,7 @@ _lib = None
 
 S_PERIODIC = 1
 OFFSET_PERIODIC_NOMASK = 2
+RK2_SUPERBEE = 8
 
 
 class OGrid(ctypes.Structure):
