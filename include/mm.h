@@ -59,6 +59,11 @@ typedef struct {
 #define MM_FLAG_S_PERIODIC 1u              /* test-only: s wraps (default: zero inflow at s_lo, walk-off at s_hi) */
 #define MM_FLAG_OFFSET_PERIODIC_NOMASK 2u  /* test-only: (xi, eta) wrap and the disc mask is off */
 #define MM_FLAG_CHECK_DT 4u                /* mm_substep returns MM_ERR_UNSTABLE when dt breaks the S8 bound */
+#define MM_FLAG_RK2_SUPERBEE 8u            /* second scheme: every substep is the paper's Runge-
+                                              Kutta 2 through the half step (Alg. 2 l.9-10)
+                                              with the Superbee flux limiter in s instead of forward
+                                              Euler + first-order upwind; (xi, eta) stay first-order upwind.  Formulas:
+                                              DESIGN.md Q27-Q30.  The S8 bound of MM_FLAG_CHECK_DT is the Euler one. */
 
 /* Model parameters (BASELINE.json configs[0] gives the benchmark values in brackets). */
 typedef struct {

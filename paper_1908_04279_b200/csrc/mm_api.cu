@@ -14,6 +14,7 @@
 #include "mm_stream.cuh"
 #include "mm_tile.cuh"
 #include "mm_coef.cuh"
+#include "mm_rk2.cuh"
 
 using namespace mm;
 
@@ -366,6 +367,23 @@ static mm_status launch_generic(mm_ctx *c, double dt, const void *in, void *out)
     return MM_OK;
 }
 
+// One RK2 + Superbee substep with the generic stage kernel: m* into the spare buffer, m^{n+1} in place.
+template <typename real>
+static mm_status launch_rk2_generic(mm_ctx *c, double dt)
+{
+    int64_t blocks = (c->cells + 255) / 256;
+    const int64_t cap = (int64_t)c->sm_count * 64;
+    if (blocks > cap) blocks = cap;
+    real *A = (real *)c->buf[c->cur], *B = (real *)c->buf[c->cur ^ 1];
+    rk2_stage_generic_kernel<real><<<(unsigned)blocks, 256, 0, c->stream>>>(make_kparams<real>(c, 0.5 * dt), A, A, B);
+    CUDA_TRY(c, cudaGetLastError());
+    rk2_stage_generic_kernel<real><<<(unsigned)blocks, 256, 0, c->stream>>>(make_kparams<real>(c, dt), A, B, A);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches += 2;
+    snprintf(c->kname, sizeof c->kname, "rk2_generic<%s>", sizeof(real) == 8 ? "f64" : "f32");
+    return MM_OK;
+}
+
 template <typename real>
 static mm_status launch_moments(mm_ctx *c)
 {
@@ -400,7 +418,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
         return fail(nullptr, MM_ERR_INVALID_ARG, "parameter out of range or not finite");
     if (p.n_end_cells < 0 || 2 * (int64_t)p.n_end_cells > g.ns)
         return fail(nullptr, MM_ERR_INVALID_ARG, "need 0 <= 2*n_end_cells <= ns");
-    if (p.flags & ~(MM_FLAG_S_PERIODIC | MM_FLAG_OFFSET_PERIODIC_NOMASK | MM_FLAG_CHECK_DT))
+    if (p.flags & ~(MM_FLAG_S_PERIODIC | MM_FLAG_OFFSET_PERIODIC_NOMASK | MM_FLAG_CHECK_DT | MM_FLAG_RK2_SUPERBEE))
         return fail(nullptr, MM_ERR_INVALID_ARG, "unknown flag");
     if ((b0 == nullptr) != (b1 == nullptr)) return fail(nullptr, MM_ERR_INVALID_ARG, "pass both density buffers or neither");
     if (b0 && (b0 == b1 || ((uintptr_t)b0 & 15) || ((uintptr_t)b1 & 15)))
@@ -573,6 +591,14 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
     if (kind == 4 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernel does not support this grid/flags");
     if (kind == 3 && !c->tile_ok) return fail(c, MM_ERR_INVALID_ARG, "tile kernel does not support this grid/flags");
     c->mom_valid = false;
+    if (c->p.flags & MM_FLAG_RK2_SUPERBEE) {
+        if (kind != 1 && c->opt_kernel != 0) return fail(c, MM_ERR_INVALID_ARG, "RK2 + Superbee runs on kernel 0 (auto) or 1 (generic)");
+        for (int n = 0; n < n_sub; ++n) {
+            mm_status s = c->dtype == MM_F64 ? launch_rk2_generic<double>(c, dt) : launch_rk2_generic<float>(c, dt);
+            if (s != MM_OK) return s;
+        }
+        return MM_OK;
+    }
     int remaining = n_sub;
     while (remaining > 0) {
         mm_status s;
