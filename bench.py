@@ -134,6 +134,16 @@ def rank_workload(w: mi.Workload, rank: int):
                        w.params)
 
 
+def with_scheme(w: mi.Workload, scheme: str):
+    """--scheme rk2: the same workload advanced by the paper's RK2 + Superbee-in-s scheme (SURVEY.md 8(f) NEXT-1,
+    MM_FLAG_RK2_SUPERBEE) instead of forward Euler + first-order upwind."""
+    if scheme != "rk2":
+        return w
+    import dataclasses
+    params = dataclasses.replace(w.params, flags=w.params.flags | mi.FLAG_RK2_SUPERBEE)
+    return mi.Workload(w.name + "+rk2_superbee", w.grid, w.dtype, w.n_sub, w.moments_every, w.omega_max, w.seed, params)
+
+
 def upload_inputs(mm, w, chunk_configs=2048, log=None):
     """S11 inputs for the whole workload, generated on the host in chunks of configurations and uploaded."""
     npdt = np.float64 if w.dtype == "f64" else np.float32
@@ -174,7 +184,7 @@ def run_cuda(args):
 
     free_b, _ = torch.cuda.mem_get_info()
     idx = pick_workload(args.config, free_b)
-    w = rank_workload(mi.CONFIGS[idx], rank)
+    w = with_scheme(rank_workload(mi.CONFIGS[idx], rank), args.scheme)
     g, es = w.grid, ES[w.dtype]
     tdt = torch.float64 if w.dtype == "f64" else torch.float32
     log(f"workload configs[{idx}] {w.name}: Nc={g.nc} cells={g.cells} dtype={w.dtype} n_sub={w.n_sub} "
@@ -245,7 +255,7 @@ def run_cuda(args):
     # ---- dominant kernel: average launch duration over the timed region (CUDA events on the library's stream)
     sub_ms = sum(a.elapsed_time(c) for a, c, _ in sub_events)
     sub_n = sum(n for _, _, n in sub_events)
-    fuse_t = args.fuse_t or mm.get_option(b.MM_OPT_FUSE_T)
+    fuse_t = 1 if args.scheme == "rk2" else (args.fuse_t or mm.get_option(b.MM_OPT_FUSE_T))
     launches_per_call = -(-w.moments_every // fuse_t)
     n_launch = launches_per_call * len(sub_events)
     peak, peak_src = measured_peaks()
@@ -364,7 +374,7 @@ def run_reference(args):
     except Exception:
         pass
     idx = pick_workload(args.config, free_b)
-    w = mi.CONFIGS[idx]
+    w = with_scheme(mi.CONFIGS[idx], args.scheme)
     g = w.grid
     from oracle import mm_oracle as orc
     cores = orc.threads()
@@ -401,6 +411,8 @@ def main():
     ap.add_argument("--config", type=int, default=None, help="index into BASELINE.json configs (default: largest that fits)")
     ap.add_argument("--fuse-t", type=int, default=0, help="override MM_OPT_FUSE_T (0 = library default)")
     ap.add_argument("--kernel", type=int, default=None, help="override MM_OPT_KERNEL")
+    ap.add_argument("--scheme", default="euler", choices=["euler", "rk2"],
+                    help="euler = forward Euler + upwind (north_star, default); rk2 = RK2 + Superbee in s (NEXT-1)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-t1", action="store_true", help="skip the unfused (T=1) roofline point")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")

@@ -384,6 +384,42 @@ static mm_status launch_rk2_generic(mm_ctx *c, double dt)
     return MM_OK;
 }
 
+// One RK2 + Superbee substep in one HBM pass (rk2_fused_kernel): reads buf[cur], writes buf[cur^1].
+template <typename real, int NXI, int NETA, int CB>
+static mm_status launch_rk2_fused(mm_ctx *c, double dt)
+{
+    constexpr int P = 2, D = 3, WARPS = 4, MINB = 2;
+    constexpr bool PM = sizeof(real) == 8, CS = sizeof(real) == 8;
+    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
+    auto kern = rk2_fused_kernel<real, NXI, NETA, CB, P, D, WARPS, MINB, PM, CS>;
+    static int blocks_per_sm = 0;
+    if (blocks_per_sm == 0) {
+        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
+        int n = 0;
+        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, Cfg::SMEM_BYTES));
+        if (n < 1) return fail(c, MM_ERR_CUDA, "fused RK2 kernel does not fit on an SM");
+        blocks_per_sm = n;
+    }
+    int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
+    const int64_t need = (c->nc + WARPS - 1) / WARPS;
+    if (grid > need) grid = need;
+    kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(make_kparams<real>(c, dt), (const real *)c->buf[c->cur],
+                                                                      (real *)c->buf[c->cur ^ 1]);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches++;
+    c->cur ^= 1;
+    snprintf(c->kname, sizeof c->kname, "rk2_fused<%s,%dx%d,CB=%d>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA, CB);
+    return MM_OK;
+}
+
+static mm_status launch_rk2_fused_any(mm_ctx *c, double dt)
+{
+    const bool big = c->g.nxi == 16;
+    if (c->dtype == MM_F64)
+        return big ? launch_rk2_fused<double, 16, 16, 2>(c, dt) : launch_rk2_fused<double, 8, 8, 2>(c, dt);
+    return big ? launch_rk2_fused<float, 16, 16, 4>(c, dt) : launch_rk2_fused<float, 8, 8, 2>(c, dt);
+}
+
 template <typename real>
 static mm_status launch_moments(mm_ctx *c)
 {
@@ -592,9 +628,13 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
     if (kind == 3 && !c->tile_ok) return fail(c, MM_ERR_INVALID_ARG, "tile kernel does not support this grid/flags");
     c->mom_valid = false;
     if (c->p.flags & MM_FLAG_RK2_SUPERBEE) {
-        if (kind != 1 && c->opt_kernel != 0) return fail(c, MM_ERR_INVALID_ARG, "RK2 + Superbee runs on kernel 0 (auto) or 1 (generic)");
+        // kernel 0 (auto): the fused one-pass kernel where the grid is supported, else the generic stages; 1: generic
+        if (c->opt_kernel != 0 && c->opt_kernel != 1)
+            return fail(c, MM_ERR_INVALID_ARG, "RK2 + Superbee runs on kernel 0 (auto) or 1 (generic)");
+        const bool fused = c->opt_kernel == 0 && stream_supported(c);
         for (int n = 0; n < n_sub; ++n) {
-            mm_status s = c->dtype == MM_F64 ? launch_rk2_generic<double>(c, dt) : launch_rk2_generic<float>(c, dt);
+            mm_status s = fused ? launch_rk2_fused_any(c, dt)
+                                : c->dtype == MM_F64 ? launch_rk2_generic<double>(c, dt) : launch_rk2_generic<float>(c, dt);
             if (s != MM_OK) return s;
         }
         return MM_OK;
