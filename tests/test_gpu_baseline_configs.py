@@ -44,11 +44,24 @@ def sample_configs(w, n_random=40):
 
 @pytest.mark.parametrize("idx", [0, 1, 2, 3, 4])
 def test_full_size_config(idx):
+    _full_size(idx, "euler")
+
+
+@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4])
+def test_full_size_config_rk2_superbee(idx):
+    """The same five workloads advanced by the paper's RK2 + Superbee scheme, fused kernel."""
+    _full_size(idx, "rk2")
+
+
+def _full_size(idx, scheme):
+    import dataclasses
     import torch
     from paper_1908_04279_b200 import MM
 
     w = mi.CONFIGS[idx]
     g, p = w.grid, w.params
+    if scheme == "rk2":
+        p = dataclasses.replace(p, flags=p.flags | mi.FLAG_RK2_SUPERBEE)
     free_b, _ = torch.cuda.mem_get_info()
     if 2 * g.cells * ES[w.dtype] + (3 << 30) > free_b:
         pytest.skip(f"configs[{idx}] needs {2 * g.cells * ES[w.dtype] / 1e9:.0f} GB of device memory")
@@ -127,7 +140,7 @@ def test_full_size_config(idx):
         assert (out[:, :, ~inside] == 0).all()
         assert e1 <= tol, f"configs[{idx}] c={c}+{n}: P1 {e1:.3e} ({kname})"
     mm.destroy()
-    print(f"configs[{idx}] {w.name} {kname}: {len(sample)} configurations vs oracle: "
+    print(f"configs[{idx}] {w.name} {scheme} {kname}: {len(sample)} configurations vs oracle: "
           f"P1 {worst['p1']:.2e}  P2 force {worst['f']:.2e} torque {worst['t']:.2e}  (tol {tol})")
 
 
