@@ -22,6 +22,10 @@
 #include "mm_common.cuh"
 #include "mm_ptx.cuh"
 
+#ifndef MM_COEF_PACKED
+#define MM_COEF_PACKED 0   // measured: 21 % fewer issue slots, same time (profiles/r01c_README.md) -- kept selectable
+#endif
+
 namespace mm {
 
 template <typename real, int N>
@@ -66,6 +70,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
     constexpr int LB = Cfg::LB, G = Cfg::G, QA = Cfg::QA, PLANE = Cfg::PLANE, NK = Cfg::NK, NKV = Cfg::NKV;
     constexpr int VW = Cfg::VW;
+    constexpr bool PK = sizeof(real) == 4 && CB % 2 == 0 && !PM && MM_COEF_PACKED;   // packed f32x2 level loop
     constexpr int UNR = CS ? 1 : P;   // plane-loop unroll: full where registers allow (it removes the R <- x moves)
     using V128 = CVec<real, VW>;
     constexpr int OX = 0, OE = (QA + 1) * CB, OC = OE + QA * (CB + 1);   // offsets of h0x, h0e, c0m in the block
@@ -223,6 +228,53 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     for (int e = 0; e < NK; ++e) kl[e] = kc[e];
                 }
                 real hx[QA + 1][CB], he[QA][CB + 1];
+                if constexpr (PK) {
+                    // packed build: face velocities and the mask products two columns at a time
+                    const float2 sj2 = make_float2(sj, sj), bx2 = make_float2(hbx, hbx), be2 = make_float2(hbe, hbe);
+#pragma unroll
+                    for (int fq = 0; fq <= QA; ++fq)
+#pragma unroll
+                        for (int h = 0; h < CB / 2; ++h) {
+                            const float2 t = __ffma2_rn(sj2, bx2, make_float2(kl[OX + fq * CB + 2 * h], kl[OX + fq * CB + 2 * h + 1]));
+                            hx[fq][2 * h] = t.x;
+                            hx[fq][2 * h + 1] = t.y;
+                        }
+#pragma unroll
+                    for (int q = 0; q < QA; ++q) {
+#pragma unroll
+                        for (int h = 0; h < CB / 2; ++h) {
+                            const float2 t = __ffma2_rn(sj2, be2, make_float2(kl[OE + q * (CB + 1) + 2 * h], kl[OE + q * (CB + 1) + 2 * h + 1]));
+                            he[q][2 * h] = t.x;
+                            he[q][2 * h + 1] = t.y;
+                        }
+                        he[q][CB] = fmaf(sj, hbe, kl[OE + q * (CB + 1) + CB]);
+                    }
+#pragma unroll
+                    for (int q = 0; q < QA; ++q)
+#pragma unroll
+                        for (int h = 0; h < CB / 2; ++h) {
+                            float2 ns2, pb2, nt2, pl2, nr2;
+#pragma unroll
+                            for (int e = 0; e < 2; ++e) {
+                                const int cb = 2 * h + e;
+                                const float nsab = (-rabs(hx[q][cb]) - rabs(hx[q + 1][cb])) + (-rabs(he[q][cb]) - rabs(he[q][cb + 1]));
+                                const float pb = hx[q][cb] + rabs(hx[q][cb]);
+                                const float nt = rabs(hx[q + 1][cb]) - hx[q + 1][cb];
+                                const float pl_ = he[q][cb] + rabs(he[q][cb]);
+                                const float nr = rabs(he[q][cb + 1]) - he[q][cb + 1];
+                                if (e == 0) { ns2.x = nsab; pb2.x = pb; nt2.x = nt; pl2.x = pl_; nr2.x = nr; }
+                                else { ns2.y = nsab; pb2.y = pb; nt2.y = nt; pl2.y = pl_; nr2.y = nr; }
+                            }
+                            const float2 m2 = make_float2(maskf[q][2 * h], maskf[q][2 * h + 1]);
+                            const float2 c2 = __ffma2_rn(m2, ns2, make_float2(kl[OC + q * CB + 2 * h], kl[OC + q * CB + 2 * h + 1]));
+                            const float2 a2 = __fmul2_rn(m2, pb2), b2 = __fmul2_rn(m2, nt2), d2 = __fmul2_rn(m2, pl2), e2 = __fmul2_rn(m2, nr2);
+                            c0j[q][2 * h] = c2.x; c0j[q][2 * h + 1] = c2.y;
+                            cxm[q][2 * h] = a2.x; cxm[q][2 * h + 1] = a2.y;
+                            cxp[q][2 * h] = b2.x; cxp[q][2 * h + 1] = b2.y;
+                            cem[q][2 * h] = d2.x; cem[q][2 * h + 1] = d2.y;
+                            cep[q][2 * h] = e2.x; cep[q][2 * h + 1] = e2.y;
+                        }
+                } else {
 #pragma unroll
                 for (int fq = 0; fq <= QA; ++fq)
 #pragma unroll
@@ -249,6 +301,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                             cxm[q][cb] = m * pb; cxp[q][cb] = m * nt; cem[q][cb] = m * pl_; cep[q][cb] = m * nr;
                         }
                     }
+                }
                 // ghost cells beyond the box are 0 (S5): their coefficient is an exact 0 on the edge lanes
 #pragma unroll
                 for (int cb = 0; cb < CB; ++cb) {
@@ -292,6 +345,32 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     lf[q] = shfl_up_r(x[q][CB - 1], 1);
                 }
                 real nx[QA][CB];
+                if constexpr (PK) {
+                    // fp32: the four aligned terms of a column pair go through the packed FFMA2 pipe form (same FMA
+                    // lanes, half the issue slots -- profiles/r01b_README.md section 0); the two eta neighbours are
+                    // misaligned by one column and stay scalar FFMAs on the halves of the pair.
+#pragma unroll
+                    for (int q = 0; q < QA; ++q)
+#pragma unroll
+                        for (int h = 0; h < CB / 2; ++h) {
+                            const int e0 = 2 * h, e1 = 2 * h + 1;
+                            float2 acc = __ffma2_rn(make_float2(c0j[q][e0], c0j[q][e1]), make_float2(x[q][e0], x[q][e1]),
+                                                    make_float2(srcm[q][e0], srcm[q][e1]));
+                            const float2 below = q > 0 ? make_float2(x[q > 0 ? q - 1 : 0][e0], x[q > 0 ? q - 1 : 0][e1])
+                                                       : make_float2(dn[e0], dn[e1]);
+                            const float2 above = q + 1 < QA ? make_float2(x[q + 1 < QA ? q + 1 : 0][e0], x[q + 1 < QA ? q + 1 : 0][e1])
+                                                            : make_float2(up[e0], up[e1]);
+                            acc = __ffma2_rn(make_float2(cxm[q][e0], cxm[q][e1]), below, acc);
+                            acc = __ffma2_rn(make_float2(cxp[q][e0], cxp[q][e1]), above, acc);
+                            acc.x = fmaf(cem[q][e0], e0 > 0 ? x[q][e0 > 0 ? e0 - 1 : 0] : lf[q], acc.x);
+                            acc.y = fmaf(cem[q][e1], x[q][e0], acc.y);
+                            acc.x = fmaf(cep[q][e0], x[q][e1], acc.x);
+                            acc.y = fmaf(cep[q][e1], e1 + 1 < CB ? x[q][e1 + 1 < CB ? e1 + 1 : 0] : rt[q], acc.y);
+                            acc = __ffma2_rn(make_float2(csm[q][e0], csm[q][e1]), make_float2(R[lv][q][e0], R[lv][q][e1]), acc);
+                            nx[q][e0] = acc.x;
+                            nx[q][e1] = acc.y;
+                        }
+                } else {
 #pragma unroll
                 for (int q = 0; q < QA; ++q)
 #pragma unroll
@@ -308,6 +387,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                         acc = fma(csm[q][cb], R[lv][q][cb], acc);   // last: the result may reuse R's register
                         nx[q][cb] = PM ? and_mask(acc, maskw[q][cb]) : acc;
                     }
+                }
 #pragma unroll
                 for (int q = 0; q < QA; ++q)
 #pragma unroll
