@@ -240,6 +240,77 @@ int mmo_run(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_c
     return fail ? -1 : 0;
 }
 
+/* ---- local adaptive time step per independent unit ------------------------------------
+ * "We instead compute a local dt* for each r0 at the beginning of each inner time step and update M_b at each r0
+ * asynchronously"; Alg. 2 l.2-5: "Set t*_end = t + dt; for r0 in grid: while
+ * t* < t*_end: compute adaptive dt*"; "the inner time step dt* restricted by the motor speed and binding/unbinding
+ * rates in Eq. (4)".  The paper prints no formula; readings Q31-Q33:
+ *  - the unit is the configuration c (this path's independent unit, as r0 is the paper's);
+ *  - its stability rate is the S8 positivity rate maximised over the cells of the unit that are evolved
+ *    (inside the disc):  lambda_c = max_{j,a,b} [ W/ds + (max(Axi[a+1/2],0) - min(Axi[a-1/2],0))/dxi
+ *                                              + (max(Aeta[b+1/2],0) - min(Aeta[b-1/2],0))/deta + kappa_ab E_j ];
+ *    the rates do not depend on m, so dt* is constant over the macro step;
+ *  - n_c = max(1, ceil(dt lambda_c / cfl)) local steps of equal size dt*_c = dt / n_c (<= cfl / lambda_c), which
+ *    land exactly on t + dt. */
+int mmo_rate_bound(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
+                   const double *U, const double *V, const double *Om, double *lambda)
+{
+    const int ns = g->ns, nxi = g->nxi, neta = g->neta;
+    const double R = p->R;
+    const double ds = (p->s_hi - p->s_lo) / ns, dxi = 2.0 * R / nxi, deta = 2.0 * R / neta;
+#pragma omp parallel for schedule(static)
+    for (int64_t c = 0; c < n_configs; ++c) {
+        int itheta = (int)((c_first + c) % g->ntheta);
+        double theta = 2.0 * MMO_PI * (double)itheta / (double)g->ntheta;
+        double ct = cos(theta), st = sin(theta);
+        double lam = 0.0;
+        for (int j = 0; j < ns; ++j) {
+            double sj = p->s_lo + (j + 0.5) * ds;
+            double E = (j < p->n_end_cells || j >= ns - p->n_end_cells) ? p->end_detach_mult : 1.0;
+            for (int a = 0; a < nxi; ++a)
+                for (int b = 0; b < neta; ++b) {
+                    if (!inside(g, p, a, b)) continue;
+                    double xi = -R + (a + 0.5) * dxi, eta = -R + (b + 0.5) * deta;
+                    double W = walk_speed(p, ct, st, xi, eta);
+                    double Axh = U[c] + walk_speed(p, ct, st, -R + (a + 1) * dxi, eta) * ct - sj * Om[c] * st;
+                    double Axl = U[c] + walk_speed(p, ct, st, -R + a * dxi, eta) * ct - sj * Om[c] * st;
+                    double Aeh = V[c] + walk_speed(p, ct, st, xi, -R + (b + 1) * deta) * st + sj * Om[c] * ct;
+                    double Ael = V[c] + walk_speed(p, ct, st, xi, -R + b * deta) * st + sj * Om[c] * ct;
+                    double r = sqrt(xi * xi + eta * eta);
+                    double kappa = p->k_off0 * exp(p->k_spring * r / p->f_detach) * E;
+                    double rate = W / ds + (dmax(Axh, 0.0) - dmin(Axl, 0.0)) / dxi
+                                + (dmax(Aeh, 0.0) - dmin(Ael, 0.0)) / deta + kappa;
+                    lam = dmax(lam, rate);
+                }
+        }
+        lambda[c] = lam;
+    }
+    return 0;
+}
+
+/* Advance every configuration from t to t + dt with its own n_c equal local steps (see above); the scheme of each
+ * local step is the one the flags select.  n_steps (may be NULL) receives n_c. */
+int mmo_advance_local(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
+                      const double *U, const double *V, const double *Om,
+                      double *m, double dt, double cfl, int32_t *n_steps)
+{
+    const size_t inner = (size_t)g->ns * g->nxi * g->neta;
+    double *lambda = (double *)malloc(sizeof(double) * (size_t)(n_configs > 0 ? n_configs : 1));
+    if (!lambda) return -1;
+    mmo_rate_bound(g, p, c_first, n_configs, U, V, Om, lambda);
+    int fail = 0;
+#pragma omp parallel for schedule(dynamic)
+    for (int64_t c = 0; c < n_configs; ++c) {
+        double need = ceil(dt * lambda[c] / cfl);
+        int32_t n_c = need < 1.0 ? 1 : (int32_t)need;
+        if (n_steps) n_steps[c] = n_c;
+        if (mmo_run(g, p, c_first + c, 1, U + c, V + c, Om + c, m + (size_t)c * inner, n_c, dt / (double)n_c) != 0)
+            fail = 1;
+    }
+    free(lambda);
+    return fail ? -1 : 0;
+}
+
 /* S9: per-configuration moments; force [n][2], torque [n]; optional (may be NULL) test-only
  * cancellation-free scales N0 = dV sum m, SF = k dV sum r m, Stau = k dV sum |s| r m. */
 int mmo_moments(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,

@@ -51,6 +51,10 @@ def _load():
         lib.mmo_run.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, dbl]
         lib.mmo_moments.restype = ctypes.c_int
         lib.mmo_moments.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp, vp]
+        lib.mmo_rate_bound.restype = ctypes.c_int
+        lib.mmo_rate_bound.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp]
+        lib.mmo_advance_local.restype = ctypes.c_int
+        lib.mmo_advance_local.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, dbl, dbl, vp]
         lib.mmo_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -95,6 +99,34 @@ def run(grid, params, U, V, Om, m, n_sub: int, dt: float, c_first: int = 0) -> n
     if rc != 0:
         raise MemoryError("oracle scratch allocation failed")
     return out.reshape(n, grid.ns, grid.nxi, grid.neta)
+
+
+def rate_bound(grid, params, U, V, Om, c_first: int = 0) -> np.ndarray:
+    """lambda_c of SURVEY.md 8(f) NEXT-3 (reading Q32): the S8 positivity rate maximised over the disc cells."""
+    lib = _load()
+    g, p = _grid(grid), _params(params)
+    U, V, Om = _f64(U), _f64(V, U.size if hasattr(U, "size") else None), _f64(Om)
+    lam = np.empty(U.size)
+    lib.mmo_rate_bound(ctypes.byref(g), ctypes.byref(p), c_first, U.size, U.ctypes.data, V.ctypes.data,
+                       Om.ctypes.data, lam.ctypes.data)
+    return lam
+
+
+def advance_local(grid, params, U, V, Om, m, dt: float, cfl: float, c_first: int = 0):
+    """Every configuration from t to t + dt with its own n_c = max(1, ceil(dt lambda_c / cfl)) equal local steps
+    (Alg. 2 l.2-5; readings Q31-Q33).  Returns (new fp64 density, n_c int32 array)."""
+    lib = _load()
+    g, p = _grid(grid), _params(params)
+    inner = grid.ns * grid.nxi * grid.neta
+    out = np.array(m, dtype=np.float64, order="C", copy=True)
+    n = out.size // inner
+    U, V, Om = _f64(U, n), _f64(V, n), _f64(Om, n)
+    nst = np.empty(n, np.int32)
+    rc = lib.mmo_advance_local(ctypes.byref(g), ctypes.byref(p), c_first, n, U.ctypes.data, V.ctypes.data,
+                               Om.ctypes.data, out.ctypes.data, dt, cfl, nst.ctypes.data)
+    if rc != 0:
+        raise MemoryError("oracle scratch allocation failed")
+    return out.reshape(n, grid.ns, grid.nxi, grid.neta), nst
 
 
 def moments(grid, params, m, c_first: int = 0):
