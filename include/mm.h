@@ -126,6 +126,19 @@ mm_status mm_set_filament_velocity(mm_ctx *ctx, const void *U, const void *V, co
  * when n_sub > 0.  MM_ERR_STATE unless density and velocities have been set. */
 mm_status mm_substep(mm_ctx *ctx, int32_t n_sub, double dt);
 
+/* local adaptive time step per independent unit ("We instead compute a local
+ * dt* for each r0 ... and update M_b at each r0 asynchronously"; Alg. 2 l.2-5).
+ * Advances EVERY configuration c from t to t + dt with its own n_c = max(1, ceil(dt lambda_c / cfl)) forward-Euler
+ * steps of equal size dt / n_c, where lambda_c is the S8 positivity rate maximised over the disc cells of c
+ * (readings Q31-Q33 in DESIGN.md).  lambda_c and n_c are computed on the device in fp64 in every dtype; the number
+ * of passes (max_c n_c) is read back once per call (one 4-byte copy; the call synchronises the stream for it).
+ * dt > 0, cfl > 0, finite; MM_ERR_STATE unless density and velocities have been set; MM_ERR_INVALID_ARG with
+ * MM_FLAG_RK2_SUPERBEE (not supported on this call yet). */
+mm_status mm_advance_local(mm_ctx *ctx, double dt, double cfl);
+/* n_c [Nc] (int32) and lambda_c [Nc] (fp64) of the last mm_advance_local; either pointer may be NULL.
+ * MM_ERR_STATE before the first mm_advance_local or after new velocities were set. */
+mm_status mm_local_steps(mm_ctx *ctx, int32_t *n_steps, double *lambda, int dst_on_device);
+
 /* Moments (S9) of the current density: force [Nc][2] = (Fx, Fy), torque [Nc]; always fp64
  * (macroscale data stays double precision).  Either pointer may be NULL to skip it. */
 mm_status mm_moments(mm_ctx *ctx, double *force, double *torque, int dst_on_device);

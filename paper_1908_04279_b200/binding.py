@@ -18,7 +18,7 @@ MM_MAX_FUSE_T = 4
 
 EXPORTS = ["mm_create", "mm_set_density", "mm_get_density", "mm_set_density_range", "mm_get_density_range",
            "mm_set_filament_velocity", "mm_substep", "mm_moments", "mm_set_option", "mm_get_option", "mm_launch_count",
-           "mm_kernel_name", "mm_destroy", "mm_status_string", "mm_last_error"]
+           "mm_kernel_name", "mm_destroy", "mm_status_string", "mm_last_error", "mm_advance_local", "mm_local_steps"]
 
 
 class mm_grid(ctypes.Structure):
@@ -58,6 +58,8 @@ def lib():
         L.mm_set_filament_velocity.argtypes = [vp, vp, vp, vp, ctypes.c_int]
         L.mm_substep.argtypes = [vp, i32, dbl]
         L.mm_moments.argtypes = [vp, vp, vp, ctypes.c_int]
+        L.mm_advance_local.argtypes = [vp, dbl, dbl]
+        L.mm_local_steps.argtypes = [vp, vp, vp, ctypes.c_int]
         L.mm_set_option.argtypes = [vp, ctypes.c_int, i64]
         L.mm_get_option.argtypes = [vp, ctypes.c_int, ctypes.POINTER(i64)]
         L.mm_launch_count.argtypes = [vp]
@@ -144,6 +146,14 @@ class MM:
 
     def substep(self, n_sub: int, dt: float):
         self._check(self._L.mm_substep(self._h, int(n_sub), float(dt)))
+
+    def advance_local(self, dt: float, cfl: float):
+        self._check(self._L.mm_advance_local(self._h, float(dt), float(cfl)))
+
+    def local_steps(self, n_steps, lam):
+        (pn, d0), (pl, d1) = _ptr(n_steps), _ptr(lam)
+        self._check(self._L.mm_local_steps(self._h, pn, pl, d0 if n_steps is not None else d1))
+        return n_steps, lam
 
     def moments(self, force, torque):
         (pf, d0), (pt, d1) = _ptr(force), _ptr(torque)

@@ -15,6 +15,7 @@
 #include "mm_tile.cuh"
 #include "mm_coef.cuh"
 #include "mm_rk2.cuh"
+#include "mm_local.cuh"
 
 using namespace mm;
 
@@ -40,6 +41,10 @@ struct mm_ctx {
     double checked_dt;              // dt the S8 check last passed with (NaN = none)
     int64_t launches;
     int sm_count;
+    double *loc_lambda;             // NEXT-3: per-configuration rate bound, step count, local dt, max step count
+    int32_t *loc_n, *loc_nmax;
+    void *loc_dt;
+    bool loc_valid;
     CUtensorMap tmap[2];            // tiled-TMA views of buf[0], buf[1] (tile kernel)
     bool tile_ok;                   // tensor maps built and grid/flags supported by the tile kernel
     std::string err;
@@ -473,6 +478,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->buf[0] = b0; c->buf[1] = b1; c->owns = (b0 == nullptr); c->cur = 0;
     c->U = c->V = c->Om = c->kappa = c->cos_t = c->sin_t = nullptr;
     c->inside = nullptr; c->mom_force = c->mom_torque = nullptr; c->flag_dev = nullptr;
+    c->loc_lambda = nullptr; c->loc_n = c->loc_nmax = nullptr; c->loc_dt = nullptr; c->loc_valid = false;
     c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
     // measured defaults: the coefficient-form kernel, 4 substeps per pass
@@ -532,6 +538,7 @@ extern "C" mm_status mm_destroy(mm_ctx *c)
     cudaFree(c->U); cudaFree(c->V); cudaFree(c->Om);
     cudaFree(c->kappa); cudaFree(c->cos_t); cudaFree(c->sin_t); cudaFree(c->inside);
     cudaFree(c->mom_force); cudaFree(c->mom_torque); cudaFree(c->flag_dev);
+    cudaFree(c->loc_lambda); cudaFree(c->loc_n); cudaFree(c->loc_nmax); cudaFree(c->loc_dt);
     delete c;
     return MM_OK;
 }
@@ -596,6 +603,7 @@ extern "C" mm_status mm_set_filament_velocity(mm_ctx *c, const void *U, const vo
     if (!on_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     c->vel_set = true;
     c->checked_dt = NAN;
+    c->loc_valid = false;
     return MM_OK;
 }
 
@@ -658,6 +666,75 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         c->cur ^= 1;
         remaining -= t;
     }
+    return MM_OK;
+}
+
+// ---- NEXT-3: local adaptive time step per configuration (mm_local.cuh) ------------------------------------
+template <typename real>
+static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
+{
+    const mm_grid &g = c->g;
+    const mm_params &p = c->p;
+    LocalParams lp;
+    lp.v0 = p.v0; lp.f_stall = p.f_stall; lp.R = p.R;
+    lp.dxi = 2.0 * p.R / g.nxi; lp.deta = 2.0 * p.R / g.neta; lp.ds = (p.s_hi - p.s_lo) / g.ns; lp.s_lo = p.s_lo;
+    lp.k_spring = p.k_spring; lp.k_off0 = p.k_off0; lp.f_detach = p.f_detach; lp.end_mult = p.end_detach_mult;
+    lp.dt = dt; lp.cfl = cfl;
+    lp.ns = g.ns; lp.nxi = g.nxi; lp.neta = g.neta; lp.ntheta = g.ntheta; lp.n_end = p.n_end_cells;
+    CUDA_TRY(c, cudaMemsetAsync(c->loc_nmax, 0, sizeof(int32_t), c->stream));
+    int64_t blocks = (c->nc + 7) / 8;
+    const int64_t cap = (int64_t)c->sm_count * 16;
+    if (blocks > cap) blocks = cap;
+    local_rate_kernel<real><<<(unsigned)blocks, 256, 0, c->stream>>>(lp, c->nc, (const real *)c->U, (const real *)c->V,
+                                                                     (const real *)c->Om, c->inside, c->loc_lambda,
+                                                                     c->loc_n, (real *)c->loc_dt, c->loc_nmax);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches++;
+    int32_t nmax = 0;   // the number of passes is a host decision: one small read at the macro cadence
+    CUDA_TRY(c, cudaMemcpyAsync(&nmax, c->loc_nmax, sizeof nmax, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->loc_valid = true;
+    c->mom_valid = false;
+    KParams<real> kp = make_kparams<real>(c, 1.0);   // per unit dt; the kernels scale by dt_c
+    int64_t gblocks = (c->cells + 255) / 256;
+    const int64_t gcap = (int64_t)c->sm_count * 64;
+    if (gblocks > gcap) gblocks = gcap;
+    for (int32_t step = 0; step < nmax; ++step) {
+        substep_generic_local_kernel<real><<<(unsigned)gblocks, 256, 0, c->stream>>>(
+            kp, (const real *)c->buf[c->cur], (real *)c->buf[c->cur ^ 1], c->loc_n, (const real *)c->loc_dt, step);
+        CUDA_TRY(c, cudaGetLastError());
+        c->launches++;
+        c->cur ^= 1;
+    }
+    snprintf(c->kname, sizeof c->kname, "local_generic<%s>", sizeof(real) == 8 ? "f64" : "f32");
+    return MM_OK;
+}
+
+extern "C" mm_status mm_advance_local(mm_ctx *c, double dt, double cfl)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    if (!(std::isfinite(dt) && dt > 0) || !(std::isfinite(cfl) && cfl > 0))
+        return fail(c, MM_ERR_INVALID_ARG, "dt and cfl must be finite and > 0");
+    if (c->p.flags & MM_FLAG_RK2_SUPERBEE)
+        return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local drives the forward-Euler scheme only (no MM_FLAG_RK2_SUPERBEE yet)");
+    if (c->dens_cov_count != c->nc || !c->vel_set) return fail(c, MM_ERR_STATE, "set density and filament velocity first");
+    if (!c->loc_n) {
+        CUDA_TRY(c, cudaMalloc(&c->loc_lambda, (size_t)c->nc * sizeof(double)));
+        CUDA_TRY(c, cudaMalloc(&c->loc_n, (size_t)c->nc * sizeof(int32_t)));
+        CUDA_TRY(c, cudaMalloc(&c->loc_dt, (size_t)c->nc * c->esize));
+        CUDA_TRY(c, cudaMalloc(&c->loc_nmax, sizeof(int32_t)));
+    }
+    return c->dtype == MM_F64 ? advance_local_impl<double>(c, dt, cfl) : advance_local_impl<float>(c, dt, cfl);
+}
+
+extern "C" mm_status mm_local_steps(mm_ctx *c, int32_t *n_steps, double *lambda, int on_device)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    if (!c->loc_valid) return fail(c, MM_ERR_STATE, "no mm_advance_local call yet");
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (n_steps) CUDA_TRY(c, cudaMemcpyAsync(n_steps, c->loc_n, (size_t)c->nc * sizeof(int32_t), kind, c->stream));
+    if (lambda) CUDA_TRY(c, cudaMemcpyAsync(lambda, c->loc_lambda, (size_t)c->nc * sizeof(double), kind, c->stream));
+    if (!on_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return MM_OK;
 }
 

@@ -1,0 +1,85 @@
+"""GPU parity of the local adaptive time step (mm_advance_local) against the oracle:
+the integer step counts n_c bit-exactly, the rate bound lambda_c to rounding, the density and moments at the
+usual tolerances."""
+import numpy as np
+import pytest
+
+import mm_inputs as mi
+from mm_inputs import Grid, Params
+from oracle import mm_oracle as orc
+from util import NPDT, TOL, p1_density, p2_moments, random_inputs
+
+pytestmark = pytest.mark.gpu
+
+
+def run_local(g, p, dtype, U, V, Om, m0, dt, cfl, kernel=0):
+    import torch
+    from paper_1908_04279_b200 import MM, binding as b
+    mm = MM(g, p, dtype)
+    mm.set_option(b.MM_OPT_KERNEL, kernel)
+    npdt = NPDT[dtype]
+    mm.set_density(np.ascontiguousarray(m0, npdt))
+    mm.set_filament_velocity(*(np.ascontiguousarray(x, npdt) for x in (U, V, Om)))
+    mm.advance_local(dt, cfl)
+    n, lam = np.empty(g.nc, np.int32), np.empty(g.nc)
+    mm.local_steps(n, lam)
+    f, t = np.empty((g.nc, 2)), np.empty(g.nc)
+    mm.moments(f, t)
+    out = np.empty((g.nc, g.ns, g.nxi, g.neta), npdt)
+    mm.get_density(out)
+    name = mm.kernel_name
+    mm.destroy()
+    return out, n, lam, f, t, name
+
+
+def check_local(g, p, dtype, dt_mult, cfl=0.4, omega_max=1.0, kernel=0):
+    U, V, Om, m0 = random_inputs(g, p, dtype, omega_max=omega_max)
+    lam_o = orc.rate_bound(g, p, U, V, Om)          # from the velocities as stored (fp32 contexts: rounded, Q18)
+    dt = dt_mult / lam_o.mean()
+    out, n, lam, f, t, name = run_local(g, p, dtype, U, V, Om, m0, dt, cfl, kernel)
+    ref, n_o = orc.advance_local(g, p, U, V, Om, m0, dt, cfl)
+    assert np.max(np.abs(lam - lam_o) / lam_o) < 1e-14, name
+    assert np.array_equal(n, n_o), name                                  # integer work: bit-exact
+    tol = TOL[dtype]
+    e1 = p1_density(out, ref)
+    assert e1 <= tol, (e1, name)
+    rm = orc.moments(g, p, ref)
+    ef, et = p2_moments(f, t, rm)
+    assert ef <= tol and et <= tol, (ef, et, name)
+    return n, name
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", [(2, 2, 4, 6, 5, 4), (1, 3, 5, 7, 16, 16), (3, 3, 8, 9, 8, 8)])
+def test_local_generic_parity(dtype, shape):
+    g = Grid(*shape)
+    p = Params()
+    n, name = check_local(g, p, dtype, 6.3, kernel=1)
+    assert name.startswith("local_generic<") and len(set(n.tolist())) > 1
+
+
+def test_local_single_step_and_wide_ends():
+    g = Grid(1, 2, 8, 12, 8, 8)
+    p = Params(k_spring=200.0, n_end_cells=3, end_detach_mult=4.0)
+    n, _ = check_local(g, p, "f64", 0.2, kernel=1)
+    assert (n == 1).all()
+    check_local(g, p, "f64", 9.0, omega_max=2.0, kernel=1)
+
+
+def test_local_errors():
+    from paper_1908_04279_b200 import MM, MMError
+    g = Grid(1, 1, 2, 4, 4, 4)
+    mm = MM(g, Params(), "f64")
+    with pytest.raises(MMError):
+        mm.advance_local(0.1, 0.4)            # nothing set yet
+    with pytest.raises(MMError):
+        mm.local_steps(np.empty(g.nc, np.int32), None)
+    mm.destroy()
+    mm = MM(g, Params(flags=mi.FLAG_RK2_SUPERBEE), "f64")
+    U, V, Om, m0 = random_inputs(g, Params(), "f64")
+    mm.set_density(m0); mm.set_filament_velocity(U, V, Om)
+    with pytest.raises(MMError):
+        mm.advance_local(0.1, 0.4)            # RK2 not supported on this call yet
+    with pytest.raises(MMError):
+        MM(g, Params(), "f64").advance_local(-1.0, 0.4)
+    mm.destroy()
