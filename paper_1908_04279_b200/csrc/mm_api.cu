@@ -224,7 +224,7 @@ static mm_status launch_coef_inst(mm_ctx *c, double dt, const void *in, void *ou
     if (grid > need) grid = need;
     KParams<real> kp = make_kparams<real>(c, dt);
     kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(kp, (const real *)in, (real *)out, c->mom_force,
-                                                                      c->mom_torque);
+                                                                      c->mom_torque, nullptr, nullptr, 0);
     CUDA_TRY(c, cudaGetLastError());
     c->launches++;
     snprintf(c->kname, sizeof c->kname, "coef<%s,%dx%d,CB=%d,T=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
@@ -247,6 +247,48 @@ static mm_status launch_coef_shape(mm_ctx *c, int T, bool mom, double dt, const 
     }
 #undef MM_CASE
     return fail(c, MM_ERR_INVALID_ARG, "unsupported fuse depth");
+}
+
+// NEXT-3: one pass of the local-step variant (T = MM_MAX_FUSE_T levels at most per configuration)
+template <typename real, int NXI, int NETA, int CB, bool MOM>
+static mm_status launch_coef_local_inst(mm_ctx *c, const void *in, void *out, int32_t done)
+{
+    constexpr int T = MM_MAX_FUSE_T;
+    constexpr int P = sizeof(real) == 8 ? MM_COEF_P_F64 : MM_COEF_P_F32;
+    constexpr int D = sizeof(real) == 8 ? MM_COEF_D_F64 : MM_COEF_D_F32, WARPS = MM_COEF_WARPS;
+    constexpr int MINB = sizeof(real) == 8 ? MM_COEF_MINB_F64 : MM_COEF_MINB_F32;
+    constexpr bool PM = sizeof(real) == 8, CS = sizeof(real) == 8;
+    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
+    auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB, PM, CS, true>;
+    static int blocks_per_sm = 0;
+    if (blocks_per_sm == 0) {
+        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
+        int n = 0;
+        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, Cfg::SMEM_BYTES));
+        if (n < 1) return fail(c, MM_ERR_CUDA, "local-step kernel does not fit on an SM");
+        blocks_per_sm = n;
+    }
+    int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
+    const int64_t need = (c->nc + WARPS - 1) / WARPS;
+    if (grid > need) grid = need;
+    KParams<real> kp = make_kparams<real>(c, 1.0);   // per unit dt
+    kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(kp, (const real *)in, (real *)out, c->mom_force,
+                                                                      c->mom_torque, c->loc_n, (const real *)c->loc_dt, done);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches++;
+    snprintf(c->kname, sizeof c->kname, "coef_local<%s,%dx%d,CB=%d,T<=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
+             CB, T, MOM ? ",mom" : "");
+    return MM_OK;
+}
+
+static mm_status launch_coef_local(mm_ctx *c, bool mom, const void *in, void *out, int32_t done)
+{
+    const bool big = c->g.nxi == 16;
+#define MM_LOC(R_, N_, CB_) (mom ? launch_coef_local_inst<R_, N_, N_, CB_, true>(c, in, out, done) \
+                                 : launch_coef_local_inst<R_, N_, N_, CB_, false>(c, in, out, done))
+    if (c->dtype == MM_F64) return big ? MM_LOC(double, 16, 2) : MM_LOC(double, 8, 2);
+    return big ? MM_LOC(float, 16, 4) : MM_LOC(float, 8, 2);
+#undef MM_LOC
 }
 
 static mm_status launch_coef(mm_ctx *c, int T, bool mom, double dt, const void *in, void *out)
@@ -695,6 +737,22 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     c->loc_valid = true;
     c->mom_valid = false;
+    // kernel choice: 0 auto = the coefficient-form local-step kernel where the grid is supported, else (or 1) generic
+    if (c->opt_kernel != 0 && c->opt_kernel != 1 && c->opt_kernel != 4)
+        return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local runs on kernel 0 (auto), 1 (generic) or 4 (coefficient form)");
+    if (c->opt_kernel == 4 && !stream_supported(c))
+        return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernel does not support this grid/flags");
+    if (c->opt_kernel != 1 && stream_supported(c)) {
+        const int32_t passes = (nmax + MM_MAX_FUSE_T - 1) / MM_MAX_FUSE_T;
+        for (int32_t ps = 0; ps < passes; ++ps) {
+            const bool mom = c->opt_fuse_mom && ps == passes - 1;
+            mm_status s = launch_coef_local(c, mom, c->buf[c->cur], c->buf[c->cur ^ 1], ps * MM_MAX_FUSE_T);
+            if (s != MM_OK) return s;
+            if (mom) c->mom_valid = true;
+            c->cur ^= 1;
+        }
+        return MM_OK;
+    }
     KParams<real> kp = make_kparams<real>(c, 1.0);   // per unit dt; the kernels scale by dt_c
     int64_t gblocks = (c->cells + 255) / 256;
     const int64_t gcap = (int64_t)c->sm_count * 64;

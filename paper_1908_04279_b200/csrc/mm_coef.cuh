@@ -62,10 +62,16 @@ struct CoefCfg {
     static constexpr size_t SMEM_BYTES = TABLE_BYTES + WARPS * WARP_BYTES + (size_t)WARPS * D * sizeof(uint64_t);
 };
 
-template <typename real, int NXI, int NETA, int CB, int T, bool MOM, int P, int D, int WARPS, int MINB, bool PM, bool CS>
+// LOC (mm_advance_local): every configuration takes its own local step dt_c and only the
+// levels it still owes this pass (n_steps[c] - done, clamped to 0..T; finished configurations are copied through);
+// `kp` then carries the factors per unit dt and they are scaled by dt_c once per configuration.
+template <typename real, int NXI, int NETA, int CB, int T, bool MOM, int P, int D, int WARPS, int MINB, bool PM, bool CS,
+          bool LOC = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
     substep_coef_kernel(const __grid_constant__ KParams<real> kp, const real *__restrict__ in, real *__restrict__ out,
-                        double *__restrict__ force, double *__restrict__ torque)
+                        double *__restrict__ force, double *__restrict__ torque,
+                        const int32_t *__restrict__ n_steps = nullptr, const real *__restrict__ dt_c = nullptr,
+                        int32_t done = 0)
 {
     using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
     constexpr int LB = Cfg::LB, G = Cfg::G, QA = Cfg::QA, PLANE = Cfg::PLANE, NK = Cfg::NK, NKV = Cfg::NKV;
@@ -113,7 +119,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     }
 #pragma unroll
     for (int cb = 0; cb < CB; ++cb) etab[cb] = -kp.R + (real(b0 + cb) + real(0.5)) * kp.deta;
-    const real hdx = real(0.5) * kp.dt_dxi, hde = real(0.5) * kp.dt_deta;
+    real hdx = real(0.5) * kp.dt_dxi, hde = real(0.5) * kp.dt_deta;
+    real dtc = real(1), dsrc = kp.dt_src;   // LOC: this configuration's local step and source increment
+    int nlev = T;                           // LOC: levels this configuration takes in this pass
 
     const int ns = kp.ns;
     const int64_t inner = (int64_t)ns * PLANE;
@@ -157,6 +165,18 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             ct = kp.cos_t[kth];
             st = kp.sin_t[kth];
             const real U = kp.U[c], Vv = kp.V[c], Om = kp.Om[c];
+            if (LOC) {
+                dtc = dt_c[c];
+                const int owed = n_steps[c] - done;
+                nlev = owed < 0 ? 0 : (owed > T ? T : owed);
+                hdx = real(0.5) * kp.dt_dxi * dtc;
+                hde = real(0.5) * kp.dt_deta * dtc;
+                dsrc = kp.dt_src * dtc;
+#pragma unroll
+                for (int q = 0; q < QA; ++q)
+#pragma unroll
+                    for (int cb = 0; cb < CB; ++cb) srcm[q][cb] = maskf[q][cb] * dsrc;
+            }
             hbx = -hdx * Om * st;   // d/ds_j of h_xi   (S4: A_xi = U + w cos - s Omega sin)
             hbe = hde * Om * ct;    // d/ds_j of h_eta  (S4: A_eta = V + w sin + s Omega cos)
 #pragma unroll
@@ -175,10 +195,10 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 }
 #pragma unroll
                 for (int cb = 0; cb < CB; ++cb) {
-                    const real cs = kp.dt_ds * walk_speed(kp.v0, kp.kload, ct, st, xiq[q], etab[cb]);
+                    const real cs = (LOC ? kp.dt_ds * dtc : kp.dt_ds) * walk_speed(kp.v0, kp.kload, ct, st, xiq[q], etab[cb]);
                     const real lin = (kc[OX + (q + 1) * CB + cb] - kc[OX + q * CB + cb]) +
                                      (kc[OE + q * (CB + 1) + cb + 1] - kc[OE + q * (CB + 1) + cb]);
-                    const real c0 = real(1) - cs - kp.dt * kap_s[(a0 + q) * NETA + b0 + cb] - lin;
+                    const real c0 = real(1) - cs - (LOC ? kp.dt * dtc : kp.dt) * kap_s[(a0 + q) * NETA + b0 + cb] - lin;
                     csm[q][cb] = PM ? cs : maskf[q][cb] * cs;
                     kc[OC + q * CB + cb] = PM ? c0 : maskf[q][cb] * c0;
                 }
@@ -318,7 +338,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     for (int q = 0; q < QA; ++q)
 #pragma unroll
                         for (int cb = 0; cb < CB; ++cb)
-                            c0j[q][cb] = fma(PM ? -kp.dt_endx : -kp.dt_endx * maskf[q][cb],
+                            c0j[q][cb] = fma(PM ? -(LOC ? kp.dt_endx * dtc : kp.dt_endx)
+                                                : -(LOC ? kp.dt_endx * dtc : kp.dt_endx) * maskf[q][cb],
                                              kap_s[(a0 + q) * NETA + b0 + cb], c0j[q][cb]);
                 }
             }
@@ -333,6 +354,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 }
 #pragma unroll
             for (int lv = 0; lv < T; ++lv) {
+                if (LOC && lv >= nlev) continue;   // warp-uniform: this configuration owes fewer levels
                 real up[CB], dn[CB], lf[QA], rt[QA];
 #pragma unroll
                 for (int cb = 0; cb < CB; ++cb) {
@@ -375,7 +397,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 for (int q = 0; q < QA; ++q)
 #pragma unroll
                     for (int cb = 0; cb < CB; ++cb) {
-                        real acc = fma(c0j[q][cb], x[q][cb], PM ? kp.dt_src : srcm[q][cb]);
+                        real acc = fma(c0j[q][cb], x[q][cb], PM ? dsrc : srcm[q][cb]);
                         if (q > 0) acc = fma(cxm[q][cb], x[q - 1][cb], acc);
                         if (q + 1 < QA) acc = fma(cxp[q][cb], x[q + 1][cb], acc);
                         if (cb > 0) acc = fma(cem[q][cb], x[q][cb - 1], acc);

@@ -83,3 +83,31 @@ def test_local_errors():
     with pytest.raises(MMError):
         MM(g, Params(), "f64").advance_local(-1.0, 0.4)
     mm.destroy()
+
+
+# ------------------------------------------------------------------ coefficient-form local-step kernel
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("nxi", [16, 8])
+@pytest.mark.parametrize("dt_mult", [0.3, 2.9, 11.0])
+def test_local_coef_parity(dtype, nxi, dt_mult):
+    # 700 configurations, ragged Ns = 7; dt_mult 0.3: one step everywhere, 2.9: fewer than T levels in the only pass,
+    # 11: several passes with configurations finishing in different passes (copy-through)
+    g = Grid(5, 7, 20, 7, nxi, nxi)
+    p = Params()
+    n, name = check_local(g, p, dtype, dt_mult, omega_max=2.0)
+    assert name.startswith("coef_local<"), name
+    if dt_mult > 1:
+        assert len(set(n.tolist())) > 1
+
+
+def test_local_coef_equals_generic_and_moments_standalone():
+    from paper_1908_04279_b200 import binding as b
+    g = Grid(2, 3, 8, 12, 16, 16)
+    p = Params(k_spring=120.0, n_end_cells=2, end_detach_mult=3.0)
+    U, V, Om, m0 = random_inputs(g, p, "f64", omega_max=2.0)
+    dt = 7.7 / orc.rate_bound(g, p, U, V, Om).mean()
+    a = run_local(g, p, "f64", U, V, Om, m0, dt, 0.4, kernel=0)
+    c = run_local(g, p, "f64", U, V, Om, m0, dt, 0.4, kernel=1)
+    assert a[5].startswith("coef_local<") and c[5].startswith("local_generic<")
+    assert np.array_equal(a[1], c[1]) and p1_density(a[0], c[0]) < 1e-12
+    assert np.allclose(a[3], c[3], rtol=0, atol=1e-13) and np.allclose(a[4], c[4], rtol=0, atol=1e-13)
