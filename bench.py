@@ -218,7 +218,10 @@ def run_cuda(args):
             if record:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
-            mm.substep(w.moments_every, w.dt)                               # A1-A3 (+A4 fused into the last pass)
+            if args.local_dt:   # NEXT-3: same macro interval, every configuration with its own local steps
+                mm.advance_local(w.moments_every * w.dt, args.cfl)
+            else:
+                mm.substep(w.moments_every, w.dt)                           # A1-A3 (+A4 fused into the last pass)
             if record:
                 e1.record(stream)
                 sub_events.append((e0, e1, w.moments_every))
@@ -249,17 +252,33 @@ def run_cuda(args):
     ms, launches = timed(args.steps, Ud, Vd, Od, Fd, Td, record=True)
     clocks = sampler.stop()
     kname = mm.kernel_name
-    updates_per_step = g.cells * w.n_sub * world
-    value = shard.whole_job_rate(g.cells * w.n_sub, args.steps, world, ms) / 1e9
+    units_rank_step = g.cells * w.n_sub          # cell-updates one rank performs per step
+    local_info = None
+    if args.local_dt:
+        n_c = torch.empty(g.nc, dtype=torch.int32, device=dev)
+        mm.local_steps(n_c, None)
+        n_sum, n_max = int(n_c.sum().item()), int(n_c.max().item())
+        units_rank_step = g.inner * n_sum * n_mom
+        local_info = {"macro_dt": w.moments_every * w.dt, "cfl": args.cfl, "n_c_mean": round(n_sum / g.nc, 3),
+                      "n_c_max": n_max, "n_c_min": int(n_c.min().item()),
+                      "global_step_equivalent": round(g.cells * w.n_sub * world * args.steps / (ms * 1e-3) / 1e9, 2),
+                      "note": "value counts the cell-updates actually performed (sum of n_c); global_step_equivalent "
+                              "= rate at which the same physical time would need the global-dt substeps"}
+    updates_per_step = units_rank_step * world
+    value = shard.whole_job_rate(units_rank_step, args.steps, world, ms) / 1e9
 
     # ---- dominant kernel: average launch duration over the timed region (CUDA events on the library's stream)
     sub_ms = sum(a.elapsed_time(c) for a, c, _ in sub_events)
     sub_n = sum(n for _, _, n in sub_events)
     fuse_t = 1 if args.scheme == "rk2" else (args.fuse_t or mm.get_option(b.MM_OPT_FUSE_T))
     launches_per_call = -(-w.moments_every // fuse_t)
+    if args.local_dt:
+        launches_per_call = -(-local_info["n_c_max"] // b.MM_MAX_FUSE_T)
     n_launch = launches_per_call * len(sub_events)
     peak, peak_src = measured_peaks()
     alg_bytes = 2.0 * es * g.cells * sub_n                 # 2*sizeof(real) B per cell-update (T=1 count)
+    if args.local_dt:
+        alg_bytes = 2.0 * es * units_rank_step / n_mom * len(sub_events)
     pass_bytes = 2.0 * es * g.cells * n_launch             # what one fused pass has to move: read once + write once
     achieved = alg_bytes / (sub_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": kname, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
@@ -280,7 +299,7 @@ def run_cuda(args):
             pass
 
     # ---- the same kernel unfused (T=1) for the T=1 roofline point (outside the timed region)
-    if not args.no_t1 and fuse_t != 1:
+    if not args.no_t1 and fuse_t != 1 and not args.local_dt:
         mm.set_option(b.MM_OPT_FUSE_T, 1)
         mm.substep(3, w.dt)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -314,7 +333,10 @@ def run_cuda(args):
                       "dt": w.dt, "seed": w.seed, "parallelism": f"configs x{world} (no collective)",
                       "l2": "inputs larger than L2 (two density buffers of %.1f GB)" % (g.cells * es / 1e9)},
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "impl": "cuda"}
-    if rank == 0 and world == 1 and not args.no_cpu:
+    if local_info:
+        out["config"]["workload"] += "+local_dt"
+        out["local_dt"] = local_info
+    if rank == 0 and world == 1 and not args.no_cpu and not args.local_dt:
         out["cpu_baseline"] = cpu_baseline(w, target_s=args.cpu_seconds, log=log)
     if rank == 0:
         print(json.dumps(out), flush=True)
@@ -413,6 +435,9 @@ def main():
     ap.add_argument("--kernel", type=int, default=None, help="override MM_OPT_KERNEL")
     ap.add_argument("--scheme", default="euler", choices=["euler", "rk2"],
                     help="euler = forward Euler + upwind (north_star, default); rk2 = RK2 + Superbee in s (NEXT-1)")
+    ap.add_argument("--local-dt", action="store_true",
+                    help="NEXT-3: advance each macro interval with mm_advance_local (per-configuration local steps)")
+    ap.add_argument("--cfl", type=float, default=0.4, help="CFL number of --local-dt")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-t1", action="store_true", help="skip the unfused (T=1) roofline point")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
