@@ -1,6 +1,7 @@
 // mm_api.cu -- the C ABI of libmm (include/mm.h): context, validation, buffer ownership, kernel dispatch.
-// All arithmetic of the hot path lives in the kernels (mm_stream.cuh, mm_generic.cuh); this file only
-// marshals arguments and launches.  There is no CPU fallback.
+// All arithmetic of the hot path lives in the kernels (mm_coef.cuh = default; mm_stream.cuh, mm_tile.cuh,
+// mm_generic.cuh = variants / fallback for other grids; mm_rk2.cuh, mm_local.cuh = SURVEY.md 8(f) NEXT-1, NEXT-3);
+// this file only validates, marshals arguments and launches.  There is no CPU fallback.
 #include "../../include/mm.h"
 
 #include <cmath>
