@@ -439,7 +439,8 @@ static mm_status launch_rk2_fused(mm_ctx *c, double dt)
     constexpr int P = 2, D = 3, WARPS = 4, MINB = 2;
     constexpr bool PM = sizeof(real) == 8, CS = sizeof(real) == 8;
     using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
-    auto kern = rk2_fused_kernel<real, NXI, NETA, CB, P, D, WARPS, MINB, PM, CS>;
+    constexpr bool KEEPC = sizeof(real) == 4;
+    auto kern = rk2_fused_kernel<real, NXI, NETA, CB, P, D, WARPS, MINB, PM, CS, KEEPC>;
     static int blocks_per_sm = 0;
     if (blocks_per_sm == 0) {
         CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));

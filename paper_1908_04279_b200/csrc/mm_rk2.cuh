@@ -127,7 +127,9 @@ template <typename real> __device__ __forceinline__ real superbee_half_slope(rea
     return (rcopysign(real(0.25), a) + rcopysign(real(0.25), b)) * t;   // sigma / 2
 }
 
-template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, int MINB, bool PM, bool CS>
+// KEEPC: keep the coefficient set of plane i-1 in registers for stage 2 of the next iteration (fp32); when false
+// (fp64, where 40 more doubles do not fit) stage 2 rebuilds the set of plane i-2 from the constants block.
+template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, int MINB, bool PM, bool CS, bool KEEPC>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
     rk2_fused_kernel(const __grid_constant__ KParams<real> kp, const real *__restrict__ in, real *__restrict__ out)
 {
@@ -201,15 +203,15 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     real hbx = 0, hbe = 0;
     // ---- state carried from one plane to the next (see the header comment)
     real x1[QA][CB], a1[QA][CB], Flo1[QA][CB], base2[QA][CB], xs[QA][CB], as_[QA][CB], Flo2[QA][CB];
-    real Cp[5][QA][CB];     // offset coefficients of plane i-2: c0L, cxm, cxp, cem, cep
+    real Cp[KEEPC ? 5 : 1][QA][CB];     // offset coefficients of plane i-2: c0L, cxm, cxp, cem, cep (KEEPC only)
 
     real *oc = out;
     // one skewed iteration: plane i of m arrives as y (zeros for the two ghost iterations)
     auto iter = [&](const int i, const real (&y)[QA][CB]) {
         const int j1 = i - 1, j2 = i - 2;
-        const real sj = kp.s_lo + (real(j1) + real(0.5)) * kp.ds;
-        real Cn[5][QA][CB];
-        {
+        // level-independent offset coefficients of plane jp (as in mm_coef.cuh, for the operator D = dt L)
+        auto build = [&](const int jp, real (&Cn)[5][QA][CB]) {
+            const real sj = kp.s_lo + (real(jp) + real(0.5)) * kp.ds;
             real kl[NKV * VW];
             if (CS) {
 #pragma unroll
@@ -231,7 +233,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             for (int q = 0; q < QA; ++q)
 #pragma unroll
                 for (int fb = 0; fb <= CB; ++fb) he[q][fb] = fma(sj, hbe, kl[OE + q * (CB + 1) + fb]);
-            const bool endp = (j1 < kp.n_end) || (j1 >= ns - kp.n_end);
+            const bool endp = (jp < kp.n_end) || (jp >= ns - kp.n_end);
 #pragma unroll
             for (int q = 0; q < QA; ++q)
 #pragma unroll
@@ -260,7 +262,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 Cn[3][q][0] = is_l0 ? real(0) : Cn[3][q][0];
                 Cn[4][q][CB - 1] = is_lr ? real(0) : Cn[4][q][CB - 1];
             }
-        }
+        };
+        real Cn[5][QA][CB];
+        build(j1, Cn);
         // D(v) - (F_hi - F_lo) part: offset neighbours + self + source, for state v with coefficient set C
         auto offsets = [&](const real (&v)[QA][CB], const real (&C)[5][QA][CB], real (&acc)[QA][CB]) {
             real up[CB], dn[CB], lf[QA], rt[QA];
@@ -308,7 +312,13 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
         real bs[QA][CB], Fh2[QA][CB], o[QA][CB];
         {
             real acc[QA][CB];
-            offsets(xs, Cp, acc);
+            if constexpr (KEEPC) {
+                offsets(xs, Cp, acc);
+            } else {
+                real C2[5][QA][CB];
+                build(j2, C2);
+                offsets(xs, C2, acc);
+            }
 #pragma unroll
             for (int q = 0; q < QA; ++q)
 #pragma unroll
@@ -342,8 +352,10 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 xs[q][cb] = ms[q][cb];
                 as_[q][cb] = bs[q][cb];
                 Flo2[q][cb] = Fh2[q][cb];
+                if constexpr (KEEPC) {
 #pragma unroll
-                for (int e = 0; e < 5; ++e) Cp[e][q][cb] = Cn[e][q][cb];
+                    for (int e = 0; e < 5; ++e) Cp[e][q][cb] = Cn[e][q][cb];
+                }
             }
     };
 
@@ -399,7 +411,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     x1[q][cb] = a1[q][cb] = Flo1[q][cb] = base2[q][cb] = real(0);   // ghosts below s_lo are 0 (S5)
                     xs[q][cb] = as_[q][cb] = Flo2[q][cb] = real(0);
 #pragma unroll
-                    for (int e = 0; e < 5; ++e) Cp[e][q][cb] = real(0);
+                    for (int e = 0; e < (KEEPC ? 5 : 1); ++e) Cp[e][q][cb] = real(0);
                 }
         }
 
