@@ -473,11 +473,25 @@ template <typename real>
 static mm_status launch_moments(mm_ctx *c)
 {
     KParams<real> kp = make_kparams<real>(c, 1.0);
-    int64_t blocks = c->nc;
-    const int64_t cap = (int64_t)c->sm_count * 16;
-    if (blocks > cap) blocks = cap;
-    moments_generic_kernel<real><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, (const real *)c->buf[c->cur], c->mom_force,
-                                                                          c->mom_torque);
+    const int plane = c->g.nxi * c->g.neta;
+    constexpr int VWF = 16 / sizeof(real);
+    const real *dens = (const real *)c->buf[c->cur];
+    // planes that tile a warp: one warp per configuration with vector loads; otherwise one block per configuration
+    const int vw = plane % (32 * VWF) == 0 ? VWF : (VWF > 2 && plane % (32 * 2) == 0 ? 2 : 0);
+    if (vw && plane <= 32 * vw * 4) {
+        int64_t blocks = (c->nc + 7) / 8;
+        const int64_t cap = (int64_t)c->sm_count * 8;
+        if (blocks > cap) blocks = cap;
+        if (vw == VWF)
+            moments_warp_kernel<real, VWF><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, dens, c->mom_force, c->mom_torque);
+        else
+            moments_warp_kernel<real, 2><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, dens, c->mom_force, c->mom_torque);
+    } else {
+        int64_t blocks = c->nc;
+        const int64_t cap = (int64_t)c->sm_count * 16;
+        if (blocks > cap) blocks = cap;
+        moments_generic_kernel<real><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, dens, c->mom_force, c->mom_torque);
+    }
     CUDA_TRY(c, cudaGetLastError());
     c->launches++;
     return MM_OK;

@@ -133,4 +133,59 @@ __global__ void __launch_bounds__(256) moments_generic_kernel(const __grid_const
     }
 }
 
+// S9 moments for planes that tile a warp (nxi*neta a multiple of 32*VW: the 16x16 and 8x8 BASELINE shapes): one
+// WARP per configuration, VW-element (64/128-bit) coalesced loads straight from HBM, a lane's (xi, eta) weights fixed
+// once, per-plane partial sums, one fp64 shuffle reduction and one plain store per configuration.  Used when the
+// moments are not fused into a substep pass (MM_OPT_FUSE_MOMENTS = 0, and the RK2 / generic paths).
+template <typename real, int VW>
+__global__ void __launch_bounds__(256) moments_warp_kernel(const __grid_constant__ KParams<real> kp,
+                                                           const real *__restrict__ dens, double *__restrict__ force,
+                                                           double *__restrict__ torque)
+{
+    struct alignas(sizeof(real) * VW) Vec { real v[VW]; };
+    constexpr int MAXK = 4;                       // vectors per lane per plane (host guarantees plane <= 32*VW*MAXK)
+    const int plane = kp.nxi * kp.neta, nk = plane / (32 * VW);
+    const int lane = threadIdx.x & 31;
+    const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    real wx[MAXK][VW], wy[MAXK][VW];
+#pragma unroll
+    for (int k = 0; k < MAXK; ++k)
+#pragma unroll
+        for (int e = 0; e < VW; ++e) {
+            const int i = (k * 32 + lane) * VW + e;
+            const int a = i / kp.neta, b = i - a * kp.neta;
+            wx[k][e] = -kp.R + (real(a) + real(0.5)) * kp.dxi;
+            wy[k][e] = -kp.R + (real(b) + real(0.5)) * kp.deta;
+        }
+    for (int64_t c = warp0; c < kp.nc; c += nwarps) {
+        const Vec *mc = reinterpret_cast<const Vec *>(dens + c * (int64_t)plane * kp.ns);
+        const int kth = (int)(c % kp.ntheta);
+        const real ct = kp.cos_t[kth], st = kp.sin_t[kth];
+        real FX = 0, FY = 0, TQ = 0;
+#pragma unroll 4
+        for (int j = 0; j < kp.ns; ++j) {
+            const real sj = kp.s_lo + (real(j) + real(0.5)) * kp.ds;
+            real px = 0, py = 0;
+#pragma unroll
+            for (int k = 0; k < MAXK; ++k)
+                if (k < nk) {
+                    const Vec v = mc[(int64_t)j * (plane / VW) + k * 32 + lane];
+#pragma unroll
+                    for (int e = 0; e < VW; ++e) {
+                        px = fma(wx[k][e], v.v[e], px);
+                        py = fma(wy[k][e], v.v[e], py);
+                    }
+                }
+            FX += px;
+            FY += py;
+            TQ = fma(sj, ct * py - st * px, TQ);
+        }
+        const double fx = warp_sum((double)FX), fy = warp_sum((double)FY), tq = warp_sum((double)TQ);
+        if (lane == 0) {
+            if (force) { force[2 * c] = kp.mom_scale * fx; force[2 * c + 1] = kp.mom_scale * fy; }
+            if (torque) torque[c] = kp.mom_scale * tq;
+        }
+    }
+}
+
 }  // namespace mm
