@@ -22,6 +22,9 @@
 #include "mm_common.cuh"
 #include "mm_ptx.cuh"
 
+#ifndef MM_COEF_XSTATIONARY
+#define MM_COEF_XSTATIONARY 0   // measured: ptxas reschedules the FMAs anyway, no .reuse gained (profiles/r01e_README.md)
+#endif
 #ifndef MM_COEF_PACKED
 #define MM_COEF_PACKED 0   // measured: 21 % fewer issue slots, same time (profiles/r01c_README.md) -- kept selectable
 #endif
@@ -38,6 +41,15 @@ __device__ __forceinline__ double and_mask(double v, int m)
     return __hiloint2double(__double2hiint(v) & m, __double2loint(v) & m);
 }
 __device__ __forceinline__ float and_mask(float v, int m) { return __int_as_float(__float_as_int(v) & m); }
+// fma whose position in the instruction stream is pinned relative to its neighbours (volatile asm): used where the
+// ORDER of independent FMAs matters for operand reuse (x-stationary level update)
+__device__ __forceinline__ float ofma(float a, float b, float c)
+{
+    float d;
+    asm volatile("fma.rn.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
+}
+__device__ __forceinline__ double ofma(double a, double b, double c) { return fma(a, b, c); }
 __device__ __forceinline__ float rabs(float x) { return fabsf(x); }
 __device__ __forceinline__ double rabs(double x) { return fabs(x); }
 
@@ -76,6 +88,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
     constexpr int LB = Cfg::LB, G = Cfg::G, QA = Cfg::QA, PLANE = Cfg::PLANE, NK = Cfg::NK, NKV = Cfg::NKV;
     constexpr int VW = Cfg::VW;
+    constexpr bool XS = MM_COEF_XSTATIONARY != 0;   // operand-reuse-friendly order of the level update
     constexpr bool PK = sizeof(real) == 4 && CB % 2 == 0 && !PM && MM_COEF_PACKED;   // packed f32x2 level loop
     constexpr int UNR = CS ? 1 : P;   // plane-loop unroll: full where registers allow (it removes the R <- x moves)
     using V128 = CVec<real, VW>;
@@ -393,6 +406,42 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                             nx[q][e1] = acc.y;
                         }
                 } else {
+                if constexpr (XS) {
+                    // x-stationary order: a 3-register FFMA issues at half rate unless an operand comes from the reuse
+                    // cache (profiles/r01e_README.md: 1.9 vs 3.0 FFMA/clk/SM), so every owned value feeds its (up to 5)
+                    // accumulators back to back; the halo values -- still in flight from the shuffles -- come last.
+#pragma unroll
+                    for (int q = 0; q < QA; ++q)
+#pragma unroll
+                        for (int cb = 0; cb < CB; ++cb) nx[q][cb] = ofma(csm[q][cb], R[lv][q][cb], PM ? dsrc : srcm[q][cb]);
+#pragma unroll
+                    for (int q = 0; q < QA; ++q)
+#pragma unroll
+                        for (int cb = 0; cb < CB; ++cb) {
+                            const real v = x[q][cb];
+                            nx[q][cb] = ofma(c0j[q][cb], v, nx[q][cb]);
+                            if (q + 1 < QA) nx[q + 1 < QA ? q + 1 : 0][cb] = ofma(cxm[q + 1 < QA ? q + 1 : 0][cb], v, nx[q + 1 < QA ? q + 1 : 0][cb]);
+                            if (q > 0) nx[q > 0 ? q - 1 : 0][cb] = ofma(cxp[q > 0 ? q - 1 : 0][cb], v, nx[q > 0 ? q - 1 : 0][cb]);
+                            if (cb + 1 < CB) nx[q][cb + 1 < CB ? cb + 1 : 0] = ofma(cem[q][cb + 1 < CB ? cb + 1 : 0], v, nx[q][cb + 1 < CB ? cb + 1 : 0]);
+                            if (cb > 0) nx[q][cb > 0 ? cb - 1 : 0] = ofma(cep[q][cb > 0 ? cb - 1 : 0], v, nx[q][cb > 0 ? cb - 1 : 0]);
+                        }
+#pragma unroll
+                    for (int cb = 0; cb < CB; ++cb) {
+                        nx[0][cb] = ofma(cxm[0][cb], dn[cb], nx[0][cb]);
+                        nx[QA - 1][cb] = ofma(cxp[QA - 1][cb], up[cb], nx[QA - 1][cb]);
+                    }
+#pragma unroll
+                    for (int q = 0; q < QA; ++q) {
+                        nx[q][0] = ofma(cem[q][0], lf[q], nx[q][0]);
+                        nx[q][CB - 1] = ofma(cep[q][CB - 1], rt[q], nx[q][CB - 1]);
+                    }
+                    if (PM) {
+#pragma unroll
+                        for (int q = 0; q < QA; ++q)
+#pragma unroll
+                            for (int cb = 0; cb < CB; ++cb) nx[q][cb] = and_mask(nx[q][cb], maskw[q][cb]);
+                    }
+                } else {
 #pragma unroll
                 for (int q = 0; q < QA; ++q)
 #pragma unroll
@@ -409,6 +458,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                         acc = fma(csm[q][cb], R[lv][q][cb], acc);   // last: the result may reuse R's register
                         nx[q][cb] = PM ? and_mask(acc, maskw[q][cb]) : acc;
                     }
+                }
                 }
 #pragma unroll
                 for (int q = 0; q < QA; ++q)
