@@ -354,6 +354,75 @@ int mmo_moments(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t
     return 0;
 }
 
+/* ---- motor-force spreading onto the fluid grid ----------------------------------------
+ * Eq. 10: F_2(x) = F iiint f ds dr0 dy dtheta, f = p delta(y + (l/L) s p - x) Psi M_b: the force the
+ * bound motors exert is weighted by the filament density Psi and spread to the fluid point under the motor head
+ * with a delta function; "use independent GPU threads to compute the integral ... limiting the use of atomic
+ * operations to the final reduction".  The paper does not print the discrete delta or the quadrature;
+ * readings Q34-Q37:
+ *  - the force carried by plane j of configuration c is the spring force of S9 before the sum over j,
+ *        f_j(c) = -k dxi deta sum_ab (xi_a, eta_b) m[c,j,a,b]      (so that ds sum_j f_j(c) = the S9 force);
+ *  - configuration c = (ix, iy, itheta) sits at the node x_c = (ix/nx, iy/ny) of the periodic unit square; the head
+ *    of plane j is at X = x_c + s_j p_c  (l/L = 1, Q4);
+ *  - delta_h = Peskin's 4-point kernel phi in each direction, delta_h(r) = phi(r_x/h_x) phi(r_y/h_y) / (h_x h_y),
+ *        phi(r) = (3 - 2|r| + sqrt(1 + 4|r| - 4 r^2))/8 for |r| <= 1, (5 - 2|r| - sqrt(-7 + 12|r| - 4 r^2))/8 for
+ *        1 <= |r| <= 2, 0 beyond; the grid is periodic;
+ *  - quadrature: F_2[g] = sum_c sum_j Psi_c f_j(c) delta_h(X_g - X_cj) ds (h_x h_y dtheta)
+ *                       = dtheta ds sum_{c,j} Psi_c f_j(c) phi(.) phi(.).
+ * F2: [nx][ny][2], ACCUMULATED into (the caller zeroes it); configurations [c_first, c_first + n_configs). */
+static double peskin4(double r)
+{
+    double a = fabs(r);
+    if (a <= 1.0) return (3.0 - 2.0 * a + sqrt(1.0 + 4.0 * a - 4.0 * a * a)) / 8.0;
+    if (a <= 2.0) return (5.0 - 2.0 * a - sqrt(-7.0 + 12.0 * a - 4.0 * a * a)) / 8.0;
+    return 0.0;
+}
+
+int mmo_spread_force(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
+                     const double *m, const double *psi, double *F2)
+{
+    const int ns = g->ns, nxi = g->nxi, neta = g->neta, nx = g->nx, ny = g->ny;
+    const double R = p->R, k = p->k_spring;
+    const double ds = (p->s_hi - p->s_lo) / ns, dxi = 2.0 * R / nxi, deta = 2.0 * R / neta;
+    const double dtheta = 2.0 * MMO_PI / (double)g->ntheta;
+    const size_t inner = (size_t)ns * nxi * neta;
+    for (int64_t cc = 0; cc < n_configs; ++cc) {            /* serial: plain sums in a fixed order */
+        int64_t c = c_first + cc;
+        int itheta = (int)(c % g->ntheta);
+        int iy = (int)((c / g->ntheta) % ny), ix = (int)(c / ((int64_t)g->ntheta * ny));
+        double theta = 2.0 * MMO_PI * (double)itheta / (double)g->ntheta;
+        double ct = cos(theta), st = sin(theta);
+        const double *mc = m + (size_t)cc * inner;
+        for (int j = 0; j < ns; ++j) {
+            double sj = p->s_lo + (j + 0.5) * ds;
+            double fx = 0.0, fy = 0.0;
+            for (int a = 0; a < nxi; ++a)
+                for (int b = 0; b < neta; ++b) {
+                    double xi = -R + (a + 0.5) * dxi, eta = -R + (b + 0.5) * deta;
+                    double v = mc[((size_t)j * nxi + a) * neta + b];
+                    fx += xi * v;
+                    fy += eta * v;
+                }
+            fx *= -k * dxi * deta;
+            fy *= -k * dxi * deta;
+            /* head position in grid units */
+            double gx = ((double)ix / nx + sj * ct) * nx, gy = ((double)iy / ny + sj * st) * ny;
+            double bx = floor(gx), by = floor(gy);
+            for (int u = -1; u <= 2; ++u)
+                for (int v = -1; v <= 2; ++v) {
+                    double wx = peskin4(gx - (bx + u)), wy = peskin4(gy - (by + v));
+                    long jx = ((long)bx + u) % nx, jy = ((long)by + v) % ny;
+                    if (jx < 0) jx += nx;
+                    if (jy < 0) jy += ny;
+                    double w = dtheta * ds * psi[cc] * wx * wy;
+                    F2[((size_t)jx * ny + jy) * 2 + 0] += w * fx;
+                    F2[((size_t)jx * ny + jy) * 2 + 1] += w * fy;
+                }
+        }
+    }
+    return 0;
+}
+
 int mmo_threads(void)
 {
 #ifdef _OPENMP

@@ -55,6 +55,8 @@ def _load():
         lib.mmo_rate_bound.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp]
         lib.mmo_advance_local.restype = ctypes.c_int
         lib.mmo_advance_local.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, dbl, dbl, vp]
+        lib.mmo_spread_force.restype = ctypes.c_int
+        lib.mmo_spread_force.argtypes = [vp, vp, i64, i64, vp, vp, vp]
         lib.mmo_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -127,6 +129,22 @@ def advance_local(grid, params, U, V, Om, m, dt: float, cfl: float, c_first: int
     if rc != 0:
         raise MemoryError("oracle scratch allocation failed")
     return out.reshape(n, grid.ns, grid.nxi, grid.neta), nst
+
+
+def spread_force(grid, params, m, psi, c_first: int = 0, F2=None) -> np.ndarray:
+    """Motor-force spreading (Eq. 10; readings Q34-Q37): F2[nx][ny][2] += contributions of the
+    configurations held in ``m`` (Psi-weighted plane forces spread with Peskin's 4-point delta at x_c + s_j p_c)."""
+    lib = _load()
+    g, p = _grid(grid), _params(params)
+    inner = grid.ns * grid.nxi * grid.neta
+    m = _f64(m)
+    n = m.size // inner
+    psi = _f64(psi, n)
+    if F2 is None:
+        F2 = np.zeros((grid.nx, grid.ny, 2))
+    assert F2.dtype == np.float64 and F2.flags.c_contiguous and F2.shape == (grid.nx, grid.ny, 2)
+    lib.mmo_spread_force(ctypes.byref(g), ctypes.byref(p), c_first, n, m.ctypes.data, psi.ctypes.data, F2.ctypes.data)
+    return F2
 
 
 def moments(grid, params, m, c_first: int = 0):
