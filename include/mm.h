@@ -139,6 +139,19 @@ mm_status mm_advance_local(mm_ctx *ctx, double dt, double cfl);
  * MM_ERR_STATE before the first mm_advance_local or after new velocities were set. */
 mm_status mm_local_steps(mm_ctx *ctx, int32_t *n_steps, double *lambda, int dst_on_device);
 
+/* motor-force spreading onto the fluid grid (Eq. 10: F_2(x) = F iiint p
+ * delta(y + (l/L) s p - x) Psi M_b ds dr0 dy dtheta).  Readings Q34-Q37 in DESIGN.md: plane j of
+ * configuration c = (ix, iy, itheta) carries the S9 spring force before the sum over j, f_j(c) = -k dxi deta sum_ab
+ * (xi_a, eta_b) m[c,j,a,b]; its head is at X = (ix/nx, iy/ny) + s_j p_c on the periodic unit square; the delta is
+ * Peskin's 4-point kernel phi per direction:
+ *     F2[gx][gy][.] = dtheta ds sum_{c,j} Psi_c f_j(c) phi(nx (X - X_g)_x) phi(ny (X - X_g)_y).
+ * mm_set_psi : Psi [Nc], fp64 (macroscale data stays double), copied.
+ * mm_spread_force : F2 [nx][ny][2] fp64, OVERWRITTEN with the spread force of the current density; fp64 atomic adds,
+ *                   so the summation order (not the value beyond rounding) varies from call to call.
+ *                   MM_ERR_STATE unless density and Psi have been set. */
+mm_status mm_set_psi(mm_ctx *ctx, const double *psi, int src_on_device);
+mm_status mm_spread_force(mm_ctx *ctx, double *F2, int dst_on_device);
+
 /* Moments (S9) of the current density: force [Nc][2] = (Fx, Fy), torque [Nc]; always fp64
  * (macroscale data stays double precision).  Either pointer may be NULL to skip it. */
 mm_status mm_moments(mm_ctx *ctx, double *force, double *torque, int dst_on_device);

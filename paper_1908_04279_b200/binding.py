@@ -18,7 +18,8 @@ MM_MAX_FUSE_T = 4
 
 EXPORTS = ["mm_create", "mm_set_density", "mm_get_density", "mm_set_density_range", "mm_get_density_range",
            "mm_set_filament_velocity", "mm_substep", "mm_moments", "mm_set_option", "mm_get_option", "mm_launch_count",
-           "mm_kernel_name", "mm_destroy", "mm_status_string", "mm_last_error", "mm_advance_local", "mm_local_steps"]
+           "mm_kernel_name", "mm_destroy", "mm_status_string", "mm_last_error", "mm_advance_local", "mm_local_steps", "mm_set_psi",
+           "mm_spread_force"]
 
 
 class mm_grid(ctypes.Structure):
@@ -60,6 +61,8 @@ def lib():
         L.mm_moments.argtypes = [vp, vp, vp, ctypes.c_int]
         L.mm_advance_local.argtypes = [vp, dbl, dbl]
         L.mm_local_steps.argtypes = [vp, vp, vp, ctypes.c_int]
+        L.mm_set_psi.argtypes = [vp, vp, ctypes.c_int]
+        L.mm_spread_force.argtypes = [vp, vp, ctypes.c_int]
         L.mm_set_option.argtypes = [vp, ctypes.c_int, i64]
         L.mm_get_option.argtypes = [vp, ctypes.c_int, ctypes.POINTER(i64)]
         L.mm_launch_count.argtypes = [vp]
@@ -154,6 +157,15 @@ class MM:
         (pn, d0), (pl, d1) = _ptr(n_steps), _ptr(lam)
         self._check(self._L.mm_local_steps(self._h, pn, pl, d0 if n_steps is not None else d1))
         return n_steps, lam
+
+    def set_psi(self, psi):
+        pp, dev = _ptr(psi)
+        self._check(self._L.mm_set_psi(self._h, pp, dev))
+
+    def spread_force(self, F2):
+        pf, dev = _ptr(F2)
+        self._check(self._L.mm_spread_force(self._h, pf, dev))
+        return F2
 
     def moments(self, force, torque):
         (pf, d0), (pt, d1) = _ptr(force), _ptr(torque)

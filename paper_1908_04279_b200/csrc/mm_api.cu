@@ -17,6 +17,7 @@
 #include "mm_coef.cuh"
 #include "mm_rk2.cuh"
 #include "mm_local.cuh"
+#include "mm_spread.cuh"
 
 using namespace mm;
 
@@ -46,6 +47,8 @@ struct mm_ctx {
     int32_t *loc_n, *loc_nmax;
     void *loc_dt;
     bool loc_valid;
+    double *psi, *fline, *F2;       // NEXT-4: filament density weights [nc], plane forces [nc][ns][2], fluid-grid force
+    bool psi_set;
     CUtensorMap tmap[2];            // tiled-TMA views of buf[0], buf[1] (tile kernel)
     bool tile_ok;                   // tensor maps built and grid/flags supported by the tile kernel
     std::string err;
@@ -537,6 +540,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->U = c->V = c->Om = c->kappa = c->cos_t = c->sin_t = nullptr;
     c->inside = nullptr; c->mom_force = c->mom_torque = nullptr; c->flag_dev = nullptr;
     c->loc_lambda = nullptr; c->loc_n = c->loc_nmax = nullptr; c->loc_dt = nullptr; c->loc_valid = false;
+    c->psi = c->fline = c->F2 = nullptr; c->psi_set = false;
     c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
     // measured defaults: the coefficient-form kernel, 4 substeps per pass
@@ -597,6 +601,7 @@ extern "C" mm_status mm_destroy(mm_ctx *c)
     cudaFree(c->kappa); cudaFree(c->cos_t); cudaFree(c->sin_t); cudaFree(c->inside);
     cudaFree(c->mom_force); cudaFree(c->mom_torque); cudaFree(c->flag_dev);
     cudaFree(c->loc_lambda); cudaFree(c->loc_n); cudaFree(c->loc_nmax); cudaFree(c->loc_dt);
+    cudaFree(c->psi); cudaFree(c->fline); cudaFree(c->F2);
     delete c;
     return MM_OK;
 }
@@ -808,6 +813,63 @@ extern "C" mm_status mm_local_steps(mm_ctx *c, int32_t *n_steps, double *lambda,
     const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     if (n_steps) CUDA_TRY(c, cudaMemcpyAsync(n_steps, c->loc_n, (size_t)c->nc * sizeof(int32_t), kind, c->stream));
     if (lambda) CUDA_TRY(c, cudaMemcpyAsync(lambda, c->loc_lambda, (size_t)c->nc * sizeof(double), kind, c->stream));
+    if (!on_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MM_OK;
+}
+
+// ---- NEXT-4: motor-force spreading onto the fluid grid (mm_spread.cuh) -----------------------------------------
+extern "C" mm_status mm_set_psi(mm_ctx *c, const double *psi, int on_device)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    if (!psi) return fail(c, MM_ERR_INVALID_ARG, "NULL psi");
+    if (!c->psi) CUDA_TRY(c, cudaMalloc(&c->psi, (size_t)c->nc * sizeof(double)));
+    CUDA_TRY(c, cudaMemcpyAsync(c->psi, psi, (size_t)c->nc * sizeof(double),
+                                on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    if (!on_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->psi_set = true;
+    return MM_OK;
+}
+
+template <typename real>
+static mm_status spread_impl(mm_ctx *c)
+{
+    KParams<real> kp = make_kparams<real>(c, 1.0);
+    const int plane = c->g.nxi * c->g.neta;
+    constexpr int VWF = 16 / sizeof(real);
+    const real *dens = (const real *)c->buf[c->cur];
+    int64_t blocks = (c->nc + 7) / 8;
+    const int64_t cap = (int64_t)c->sm_count * 8;
+    if (blocks > cap) blocks = cap;
+    if (plane % VWF == 0)
+        plane_force_kernel<real, VWF><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, dens, c->fline);
+    else
+        plane_force_kernel<real, 1><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, dens, c->fline);
+    CUDA_TRY(c, cudaGetLastError());
+    CUDA_TRY(c, cudaMemsetAsync(c->F2, 0, (size_t)c->g.nx * c->g.ny * 2 * sizeof(double), c->stream));
+    const int64_t total = c->nc * c->g.ns * 4;
+    int64_t sb = (total + 255) / 256;
+    const int64_t scap = (int64_t)c->sm_count * 32;
+    if (sb > scap) sb = scap;
+    spread_kernel<<<(unsigned)sb, 256, 0, c->stream>>>(c->nc, c->g.ns, c->g.nx, c->g.ny, c->g.ntheta, c->p.s_lo,
+                                                       (c->p.s_hi - c->p.s_lo) / c->g.ns, c->psi, c->fline, c->F2);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches += 2;
+    return MM_OK;
+}
+
+extern "C" mm_status mm_spread_force(mm_ctx *c, double *F2, int on_device)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    if (!F2) return fail(c, MM_ERR_INVALID_ARG, "NULL destination");
+    if (c->dens_cov_count != c->nc || !c->psi_set) return fail(c, MM_ERR_STATE, "set density and psi first");
+    if (!c->fline) {
+        CUDA_TRY(c, cudaMalloc(&c->fline, (size_t)c->nc * c->g.ns * 2 * sizeof(double)));
+        CUDA_TRY(c, cudaMalloc(&c->F2, (size_t)c->g.nx * c->g.ny * 2 * sizeof(double)));
+    }
+    mm_status s = c->dtype == MM_F64 ? spread_impl<double>(c) : spread_impl<float>(c);
+    if (s != MM_OK) return s;
+    CUDA_TRY(c, cudaMemcpyAsync(F2, c->F2, (size_t)c->g.nx * c->g.ny * 2 * sizeof(double),
+                                on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
     if (!on_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return MM_OK;
 }
