@@ -314,6 +314,25 @@ def run_cuda(args):
         roofline["t1_kernel"] = mm.kernel_name
         mm.set_option(b.MM_OPT_FUSE_T, fuse_t)
 
+    # ---- optional: NEXT-4 motor-force spreading of the current density (macro cadence; outside the timed region)
+    spread_info = None
+    if args.spread:
+        psi = torch.rand(g.nc, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(7))
+        F2 = torch.empty((g.nx, g.ny, 2), dtype=torch.float64, device=dev)
+        mm.set_psi(psi)
+        mm.spread_force(F2)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(3):
+            mm.spread_force(F2)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        sms = e0.elapsed_time(e1) / 3
+        spread_info = {"ms_per_call": round(sms, 3), "density_read_gbs": round(g.cells * es / (sms * 1e-3) / 1e9, 1),
+                       "point_forces_per_call": g.nc * g.ns, "atomic_adds_per_call": g.nc * g.ns * 32,
+                       "grid": [g.nx, g.ny]}
+
     # ---- end to end: pinned host (U,V,Omega) in, moments out to pinned host, every step
     for _ in range(2):
         step(Up, Vp, Op, Fp, Tp)
@@ -333,6 +352,8 @@ def run_cuda(args):
                       "dt": w.dt, "seed": w.seed, "parallelism": f"configs x{world} (no collective)",
                       "l2": "inputs larger than L2 (two density buffers of %.1f GB)" % (g.cells * es / 1e9)},
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "impl": "cuda"}
+    if spread_info:
+        out["spread_force"] = spread_info
     if local_info:
         out["config"]["workload"] += "+local_dt"
         out["local_dt"] = local_info
@@ -437,6 +458,8 @@ def main():
                     help="euler = forward Euler + upwind (north_star, default); rk2 = RK2 + Superbee in s (NEXT-1)")
     ap.add_argument("--local-dt", action="store_true",
                     help="NEXT-3: advance each macro interval with mm_advance_local (per-configuration local steps)")
+    ap.add_argument("--spread", action="store_true",
+                    help="NEXT-4: also time mm_spread_force (motor-force spreading, Eq. 10) on the final density")
     ap.add_argument("--cfl", type=float, default=0.4, help="CFL number of --local-dt")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-t1", action="store_true", help="skip the unfused (T=1) roofline point")
