@@ -258,8 +258,9 @@ template <typename real, int NXI, int NETA, int CB, bool MOM>
 static mm_status launch_coef_local_inst(mm_ctx *c, const void *in, void *out, int32_t done)
 {
     constexpr int T = MM_MAX_FUSE_T;
-    constexpr int P = sizeof(real) == 8 ? MM_COEF_P_F64 : MM_COEF_P_F32;
-    constexpr int D = sizeof(real) == 8 ? MM_COEF_D_F64 : MM_COEF_D_F32, WARPS = MM_COEF_WARPS;
+    // 2 planes x 3 slots for both dtypes: the kernel holds T+1 straight-line instances of the chunk body (one per
+    // level count), so the chunk is kept short to stay inside the instruction cache
+    constexpr int P = 2, D = 3, WARPS = MM_COEF_WARPS;
     constexpr int MINB = sizeof(real) == 8 ? MM_COEF_MINB_F64 : MM_COEF_MINB_F32;
     constexpr bool PM = sizeof(real) == 8, CS = sizeof(real) == 8;
     using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;

@@ -19,6 +19,7 @@
 //  * MOM: the last level adds the three S9 sums per lane; one shuffle reduction and one plain store per
 //    configuration -- no atomics.
 #pragma once
+#include <type_traits>
 #include "mm_common.cuh"
 #include "mm_ptx.cuh"
 
@@ -237,6 +238,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
         mbar_wait(&full[slot], phase);
         const real *sp = ring + (size_t)slot * P * PLANE;
         real *oc = out + c * inner;
+        // The planes of one chunk for a compile-time number NL of levels.  NL = T except in the LOC variant, where the
+        // warp-uniform level count of the configuration selects one of the T+1 straight-line instances below (a
+        // run-time `lv < nlev` test inside the unrolled planes would break their copy-free register rotation).
+        auto chunk = [&](auto NLC) {
+        constexpr int NL = decltype(NLC)::value;
 #pragma unroll UNR
         for (int pl = 0; pl < P; ++pl) {
             const int j = ch * P + pl;
@@ -366,8 +372,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     for (int e = 0; e < VW; ++e) x[q][v4 * VW + e] = v.v[e];
                 }
 #pragma unroll
-            for (int lv = 0; lv < T; ++lv) {
-                if (LOC && lv >= nlev) continue;   // warp-uniform: this configuration owes fewer levels
+            for (int lv = 0; lv < NL; ++lv) {
                 real up[CB], dn[CB], lf[QA], rt[QA];
 #pragma unroll
                 for (int cb = 0; cb < CB; ++cb) {
@@ -500,6 +505,19 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 FY += fyp;
                 TQ = fma(sj, ct * fyp - st * fxp, TQ);
             }
+        }
+        };
+        if constexpr (LOC) {
+            static_assert(T == 4, "the LOC dispatch below lists the level counts 0..4");
+            switch (nlev) {
+            case 0: chunk(std::integral_constant<int, 0>{}); break;
+            case 1: chunk(std::integral_constant<int, 1>{}); break;
+            case 2: chunk(std::integral_constant<int, 2>{}); break;
+            case 3: chunk(std::integral_constant<int, 3>{}); break;
+            default: chunk(std::integral_constant<int, 4>{}); break;
+            }
+        } else {
+            chunk(std::integral_constant<int, T>{});
         }
         // every lane has consumed this slot (its values fed the stores above): refill it
         __syncwarp();
