@@ -44,7 +44,7 @@ struct mm_ctx {
     int64_t launches;
     int sm_count;
     double *loc_lambda;             // NEXT-3: per-configuration rate bound, step count, local dt, max step count
-    int32_t *loc_n, *loc_nmax;
+    int32_t *loc_n, *loc_nmax, *loc_list, *loc_count;
     void *loc_dt;
     bool loc_valid;
     double *psi, *fline, *F2;       // NEXT-4: filament density weights [nc], plane forces [nc][ns][2], fluid-grid force
@@ -228,7 +228,7 @@ static mm_status launch_coef_inst(mm_ctx *c, double dt, const void *in, void *ou
     if (grid > need) grid = need;
     KParams<real> kp = make_kparams<real>(c, dt);
     kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(kp, (const real *)in, (real *)out, c->mom_force,
-                                                                      c->mom_torque, nullptr, nullptr, 0);
+                                                                      c->mom_torque, nullptr, nullptr, 0, nullptr, nullptr);
     CUDA_TRY(c, cudaGetLastError());
     c->launches++;
     snprintf(c->kname, sizeof c->kname, "coef<%s,%dx%d,CB=%d,T=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
@@ -255,7 +255,7 @@ static mm_status launch_coef_shape(mm_ctx *c, int T, bool mom, double dt, const 
 
 // NEXT-3: one pass of the local-step variant (T = MM_MAX_FUSE_T levels at most per configuration)
 template <typename real, int NXI, int NETA, int CB, bool MOM>
-static mm_status launch_coef_local_inst(mm_ctx *c, const void *in, void *out, int32_t done)
+static mm_status launch_coef_local_inst(mm_ctx *c, const void *in, void *out, int32_t done, bool use_list)
 {
     constexpr int T = MM_MAX_FUSE_T;
     // 2 planes x 3 slots for both dtypes: the kernel holds T+1 straight-line instances of the chunk body (one per
@@ -277,8 +277,11 @@ static mm_status launch_coef_local_inst(mm_ctx *c, const void *in, void *out, in
     const int64_t need = (c->nc + WARPS - 1) / WARPS;
     if (grid > need) grid = need;
     KParams<real> kp = make_kparams<real>(c, 1.0);   // per unit dt
+    // in may equal out (in-place pass, see the LOC note in mm_coef.cuh)
     kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(kp, (const real *)in, (real *)out, c->mom_force,
-                                                                      c->mom_torque, c->loc_n, (const real *)c->loc_dt, done);
+                                                                      c->mom_torque, c->loc_n, (const real *)c->loc_dt, done,
+                                                                      use_list ? c->loc_list : nullptr,
+                                                                      use_list ? c->loc_count : nullptr);
     CUDA_TRY(c, cudaGetLastError());
     c->launches++;
     snprintf(c->kname, sizeof c->kname, "coef_local<%s,%dx%d,CB=%d,T<=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
@@ -286,11 +289,11 @@ static mm_status launch_coef_local_inst(mm_ctx *c, const void *in, void *out, in
     return MM_OK;
 }
 
-static mm_status launch_coef_local(mm_ctx *c, bool mom, const void *in, void *out, int32_t done)
+static mm_status launch_coef_local(mm_ctx *c, bool mom, const void *in, void *out, int32_t done, bool use_list)
 {
     const bool big = c->g.nxi == 16;
-#define MM_LOC(R_, N_, CB_) (mom ? launch_coef_local_inst<R_, N_, N_, CB_, true>(c, in, out, done) \
-                                 : launch_coef_local_inst<R_, N_, N_, CB_, false>(c, in, out, done))
+#define MM_LOC(R_, N_, CB_) (mom ? launch_coef_local_inst<R_, N_, N_, CB_, true>(c, in, out, done, use_list) \
+                                 : launch_coef_local_inst<R_, N_, N_, CB_, false>(c, in, out, done, use_list))
     if (c->dtype == MM_F64) return big ? MM_LOC(double, 16, 2) : MM_LOC(double, 8, 2);
     return big ? MM_LOC(float, 16, 4) : MM_LOC(float, 8, 2);
 #undef MM_LOC
@@ -540,7 +543,8 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->buf[0] = b0; c->buf[1] = b1; c->owns = (b0 == nullptr); c->cur = 0;
     c->U = c->V = c->Om = c->kappa = c->cos_t = c->sin_t = nullptr;
     c->inside = nullptr; c->mom_force = c->mom_torque = nullptr; c->flag_dev = nullptr;
-    c->loc_lambda = nullptr; c->loc_n = c->loc_nmax = nullptr; c->loc_dt = nullptr; c->loc_valid = false;
+    c->loc_lambda = nullptr; c->loc_n = c->loc_nmax = c->loc_list = c->loc_count = nullptr; c->loc_dt = nullptr;
+    c->loc_valid = false;
     c->psi = c->fline = c->F2 = nullptr; c->psi_set = false;
     c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
@@ -602,6 +606,7 @@ extern "C" mm_status mm_destroy(mm_ctx *c)
     cudaFree(c->kappa); cudaFree(c->cos_t); cudaFree(c->sin_t); cudaFree(c->inside);
     cudaFree(c->mom_force); cudaFree(c->mom_torque); cudaFree(c->flag_dev);
     cudaFree(c->loc_lambda); cudaFree(c->loc_n); cudaFree(c->loc_nmax); cudaFree(c->loc_dt);
+    cudaFree(c->loc_list); cudaFree(c->loc_count);
     cudaFree(c->psi); cudaFree(c->fline); cudaFree(c->F2);
     delete c;
     return MM_OK;
@@ -745,7 +750,10 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
     lp.k_spring = p.k_spring; lp.k_off0 = p.k_off0; lp.f_detach = p.f_detach; lp.end_mult = p.end_detach_mult;
     lp.dt = dt; lp.cfl = cfl;
     lp.ns = g.ns; lp.nxi = g.nxi; lp.neta = g.neta; lp.ntheta = g.ntheta; lp.n_end = p.n_end_cells;
-    CUDA_TRY(c, cudaMemsetAsync(c->loc_nmax, 0, sizeof(int32_t), c->stream));
+    {
+        const int32_t init[2] = {0, INT32_MIN};   // running max of n_c and of -n_c
+        CUDA_TRY(c, cudaMemcpyAsync(c->loc_nmax, init, sizeof init, cudaMemcpyHostToDevice, c->stream));
+    }
     int64_t blocks = (c->nc + 7) / 8;
     const int64_t cap = (int64_t)c->sm_count * 16;
     if (blocks > cap) blocks = cap;
@@ -754,9 +762,10 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
                                                                      c->loc_n, (real *)c->loc_dt, c->loc_nmax);
     CUDA_TRY(c, cudaGetLastError());
     c->launches++;
-    int32_t nmax = 0;   // the number of passes is a host decision: one small read at the macro cadence
-    CUDA_TRY(c, cudaMemcpyAsync(&nmax, c->loc_nmax, sizeof nmax, cudaMemcpyDeviceToHost, c->stream));
+    int32_t nmm[2] = {0, 0};   // the number of passes is a host decision: one small read at the macro cadence
+    CUDA_TRY(c, cudaMemcpyAsync(nmm, c->loc_nmax, sizeof nmm, cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    const int32_t nmax = nmm[0], nmin = -nmm[1];
     c->loc_valid = true;
     c->mom_valid = false;
     // kernel choice: 0 auto = the coefficient-form local-step kernel where the grid is supported, else (or 1) generic
@@ -765,14 +774,34 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
     if (c->opt_kernel == 4 && !stream_supported(c))
         return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernel does not support this grid/flags");
     if (c->opt_kernel != 1 && stream_supported(c)) {
+        // fp32: passes run IN PLACE on the current buffer and, from the second pass on, visit only the unfinished
+        // configurations (compact list built on the device); a configuration writes its moments when it finishes.
+        // fp64 (measured: in-place is slower there): ping-pong passes over all configurations,
+        // finished ones copied through, moments in the last pass.
         const int32_t passes = (nmax + MM_MAX_FUSE_T - 1) / MM_MAX_FUSE_T;
+        const bool inplace = sizeof(real) == 4;
         for (int32_t ps = 0; ps < passes; ++ps) {
-            const bool mom = c->opt_fuse_mom && ps == passes - 1;
-            mm_status s = launch_coef_local(c, mom, c->buf[c->cur], c->buf[c->cur ^ 1], ps * MM_MAX_FUSE_T);
+            const int32_t done = ps * MM_MAX_FUSE_T;
+            mm_status s;
+            if (inplace) {
+                // moments are only compiled into the passes in which some configuration can finish
+                const bool mom = c->opt_fuse_mom != 0 && nmin <= done + MM_MAX_FUSE_T;
+                if (ps > 0) {
+                    CUDA_TRY(c, cudaMemsetAsync(c->loc_count, 0, sizeof(int32_t), c->stream));
+                    int64_t lb = (c->nc + 255) / 256;
+                    if (lb > (int64_t)c->sm_count * 8) lb = (int64_t)c->sm_count * 8;
+                    local_list_kernel<<<(unsigned)lb, 256, 0, c->stream>>>(c->nc, c->loc_n, done, c->loc_list, c->loc_count);
+                    CUDA_TRY(c, cudaGetLastError());
+                    c->launches++;
+                }
+                s = launch_coef_local(c, mom, c->buf[c->cur], c->buf[c->cur], done, ps > 0);
+            } else {
+                s = launch_coef_local(c, c->opt_fuse_mom != 0 && ps == passes - 1, c->buf[c->cur], c->buf[c->cur ^ 1], done, false);
+                if (s == MM_OK) c->cur ^= 1;
+            }
             if (s != MM_OK) return s;
-            if (mom) c->mom_valid = true;
-            c->cur ^= 1;
         }
+        if (c->opt_fuse_mom) c->mom_valid = true;
         return MM_OK;
     }
     KParams<real> kp = make_kparams<real>(c, 1.0);   // per unit dt; the kernels scale by dt_c
@@ -802,7 +831,9 @@ extern "C" mm_status mm_advance_local(mm_ctx *c, double dt, double cfl)
         CUDA_TRY(c, cudaMalloc(&c->loc_lambda, (size_t)c->nc * sizeof(double)));
         CUDA_TRY(c, cudaMalloc(&c->loc_n, (size_t)c->nc * sizeof(int32_t)));
         CUDA_TRY(c, cudaMalloc(&c->loc_dt, (size_t)c->nc * c->esize));
-        CUDA_TRY(c, cudaMalloc(&c->loc_nmax, sizeof(int32_t)));
+        CUDA_TRY(c, cudaMalloc(&c->loc_nmax, 2 * sizeof(int32_t)));
+        CUDA_TRY(c, cudaMalloc(&c->loc_list, (size_t)c->nc * sizeof(int32_t)));
+        CUDA_TRY(c, cudaMalloc(&c->loc_count, sizeof(int32_t)));
     }
     return c->dtype == MM_F64 ? advance_local_impl<double>(c, dt, cfl) : advance_local_impl<float>(c, dt, cfl);
 }

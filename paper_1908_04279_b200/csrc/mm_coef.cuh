@@ -76,15 +76,20 @@ struct CoefCfg {
 };
 
 // LOC (mm_advance_local): every configuration takes its own local step dt_c and only the
-// levels it still owes this pass (n_steps[c] - done, clamped to 0..T; finished configurations are copied through);
-// `kp` then carries the factors per unit dt and they are scaled by dt_c once per configuration.
+// levels it still owes this pass (n_steps[c] - done, clamped to 0..T); `kp` then carries the factors per unit dt and
+// they are scaled by dt_c once per configuration.  A LOC pass runs IN PLACE (in == out): plane j of the output
+// depends on input planes <= j only, each already copied to shared memory by the time plane j is stored, and a
+// configuration is touched by one warp only -- so a pass visits just the configurations in `list` (those still
+// unfinished; NULL = all) and the finished ones cost no traffic.  With MOM the moments of a configuration are
+// written in the pass in which it finishes.
 template <typename real, int NXI, int NETA, int CB, int T, bool MOM, int P, int D, int WARPS, int MINB, bool PM, bool CS,
           bool LOC = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
     substep_coef_kernel(const __grid_constant__ KParams<real> kp, const real *__restrict__ in, real *__restrict__ out,
                         double *__restrict__ force, double *__restrict__ torque,
                         const int32_t *__restrict__ n_steps = nullptr, const real *__restrict__ dt_c = nullptr,
-                        int32_t done = 0)
+                        int32_t done = 0, const int32_t *__restrict__ list = nullptr,
+                        const int32_t *__restrict__ list_count = nullptr)
 {
     using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
     constexpr int LB = Cfg::LB, G = Cfg::G, QA = Cfg::QA, PLANE = Cfg::PLANE, NK = Cfg::NK, NKV = Cfg::NKV;
@@ -136,19 +141,21 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     real hdx = real(0.5) * kp.dt_dxi, hde = real(0.5) * kp.dt_deta;
     real dtc = real(1), dsrc = kp.dt_src;   // LOC: this configuration's local step and source increment
     int nlev = T;                           // LOC: levels this configuration takes in this pass
+    bool last_pass = true;                  // LOC: the configuration finishes in this pass (moments are due)
 
     const int ns = kp.ns;
     const int64_t inner = (int64_t)ns * PLANE;
     const int CH = (ns + P - 1) / P;
     const int64_t gw = (int64_t)blockIdx.x * WARPS + warp, nw = (int64_t)gridDim.x * WARPS;
-    const int64_t my_n = gw < kp.nc ? (kp.nc - gw + nw - 1) / nw : 0;
+    const int64_t nact = (LOC && list) ? (int64_t)*list_count : kp.nc;   // configurations this pass visits
+    const int64_t my_n = gw < nact ? (nact - gw + nw - 1) / nw : 0;
     const int64_t total = my_n * CH;
 
     // producer state (lane 0): next chunk to request
     int64_t pk = 0;
     int pch = 0, pslot = 0;
     auto issue = [&]() {   // lane 0 only: TMA bulk copy of the next stream chunk into its ring slot
-        const int64_t c = gw + pk * nw;
+        const int64_t c = (LOC && list) ? (int64_t)list[gw + pk * nw] : gw + pk * nw;
         const int planes = min(P, ns - pch * P);
         const uint32_t bytes = (uint32_t)(planes * PLANE * sizeof(real));
         mbar_expect_tx(&full[pslot], bytes);
@@ -174,7 +181,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     uint32_t phase = 0;
     for (int64_t i = 0; i < total; ++i) {
         if (ch == 0) {
-            c = gw + k * nw;
+            c = (LOC && list) ? (int64_t)list[gw + k * nw] : gw + k * nw;
             const int kth = (int)(c % kp.ntheta);
             ct = kp.cos_t[kth];
             st = kp.sin_t[kth];
@@ -183,6 +190,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 dtc = dt_c[c];
                 const int owed = n_steps[c] - done;
                 nlev = owed < 0 ? 0 : (owed > T ? T : owed);
+                last_pass = owed <= T;
                 hdx = real(0.5) * kp.dt_dxi * dtc;
                 hde = real(0.5) * kp.dt_deta * dtc;
                 dsrc = kp.dt_src * dtc;
@@ -525,7 +533,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
         if (++slot == D) { slot = 0; phase ^= 1u; }
 
         if (++ch == CH) {
-            if (MOM) {
+            if (MOM && (!LOC || last_pass)) {
                 // S9: fp64 from the cross-lane reduction on (fp32 contexts: fp32 within a lane)
                 double fx = warp_sum((double)FX), fy = warp_sum((double)FY), tq = warp_sum((double)TQ);
                 if (lane == 0) {

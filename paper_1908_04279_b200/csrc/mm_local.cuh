@@ -32,7 +32,7 @@ __global__ void __launch_bounds__(256) local_rate_kernel(const LocalParams p, in
                                                          const real *__restrict__ V, const real *__restrict__ Om,
                                                          const uint8_t *__restrict__ inside, double *__restrict__ lambda,
                                                          int32_t *__restrict__ n_steps, real *__restrict__ dt_c,
-                                                         int32_t *__restrict__ n_max)
+                                                         int32_t *__restrict__ n_max /* [2]: max, -min */)
 {
     const int lane = threadIdx.x & 31;
     const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
@@ -81,8 +81,17 @@ __global__ void __launch_bounds__(256) local_rate_kernel(const LocalParams p, in
             n_steps[c] = n;
             dt_c[c] = (real)(p.dt / (double)n);
             atomicMax(n_max, n);   // once per configuration, at the macro cadence -- not on the hot loop
+            atomicMax(n_max + 1, -n);
         }
     }
+}
+
+// Compact list of the configurations that still owe steps after `done` (order irrelevant: units are independent).
+__global__ void __launch_bounds__(256) local_list_kernel(int64_t nc, const int32_t *__restrict__ n_steps, int32_t done,
+                                                         int32_t *__restrict__ list, int32_t *__restrict__ count)
+{
+    for (int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += (int64_t)gridDim.x * blockDim.x)
+        if (n_steps[c] > done) list[atomicAdd(count, 1)] = (int32_t)c;   // macro cadence, not the hot loop
 }
 
 // One local Euler step (S2-S7) for the configurations that still have steps to take (step < n_c), a copy for the
