@@ -90,8 +90,13 @@ typedef enum {
                                 (2, 3, 4: MM_ERR_INVALID_ARG from mm_substep if the grid/flags are unsupported) */
     MM_OPT_FUSE_T = 1,       /* max substeps fused per HBM pass (temporal fusion), 1..MM_MAX_FUSE_T;
                                 default 4 */
-    MM_OPT_FUSE_MOMENTS = 2  /* 1 (default): the last pass of mm_substep also reduces the moments, so a
+    MM_OPT_FUSE_MOMENTS = 2, /* 1 (default): the last pass of mm_substep also reduces the moments, so a
                                 following mm_moments is a copy; 0: mm_moments always runs its own pass */
+    MM_OPT_INPLACE = 3       /* 1: the coefficient-form, fused RK2 and local-step kernels update the current density
+                                buffer IN PLACE (plane j of the result depends on input planes <= j only, each already
+                                staged on the SM when plane j is stored, and one warp owns a configuration), the other
+                                buffer is not touched; same results, same speed, half the memory.  Default 0; always 1
+                                for a context created with ONE density buffer (mm_create, dens_buf1 = NULL) */
 } mm_option;
 #define MM_MAX_FUSE_T 4
 
@@ -101,7 +106,10 @@ typedef enum {
  *  dens_buf0/1  : device pointers to two density buffers of >= cells*sizeof(real) bytes each,
  *                 16-byte aligned, BORROWED (must outlive the context; e.g. torch tensors).  Pass
  *                 NULL, NULL and the library allocates and owns them (MM_ERR_NOMEM on failure).
- *                 Passing exactly one NULL is invalid.
+ *                 dens_buf0 alone (dens_buf1 = NULL) creates a SINGLE-BUFFER context: half the memory, every
+ *                 pass in place (MM_OPT_INPLACE), and only the in-place kernels are available -- mm_substep /
+ *                 mm_advance_local return MM_ERR_INVALID_ARG for grids or flags that need the generic kernels.
+ *                 dens_buf0 = NULL with dens_buf1 != NULL is invalid.
  *  cuda_stream  : a cudaStream_t (NULL = the legacy default stream).
  *  out          : receives the handle.  On error *out is NULL. */
 mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_dtype dtype,

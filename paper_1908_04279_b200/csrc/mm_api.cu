@@ -39,7 +39,8 @@ struct mm_ctx {
     bool mom_valid, vel_set;
     std::vector<uint8_t> dens_cov;  // per configuration: density uploaded
     int64_t dens_cov_count;
-    int opt_kernel, opt_fuse_t, opt_fuse_mom;
+    int opt_kernel, opt_fuse_t, opt_fuse_mom, opt_inplace;
+    bool single;                    // created with ONE density buffer: only the in-place kernels can run
     double checked_dt;              // dt the S8 check last passed with (NaN = none)
     int64_t launches;
     int sm_count;
@@ -327,7 +328,7 @@ static bool tile_shape_supported(const mm_ctx *c)
 static mm_status build_tensor_maps(mm_ctx *c)
 {
     c->tile_ok = false;
-    if (!tile_shape_supported(c)) return MM_OK;
+    if (!tile_shape_supported(c) || c->single) return MM_OK;
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
@@ -459,11 +460,13 @@ static mm_status launch_rk2_fused(mm_ctx *c, double dt)
     int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
     const int64_t need = (c->nc + WARPS - 1) / WARPS;
     if (grid > need) grid = need;
+    // in place when asked: stage 2 stores plane i-2 when plane i has arrived, every input plane is read once
+    const int dst = c->opt_inplace ? c->cur : c->cur ^ 1;
     kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(make_kparams<real>(c, dt), (const real *)c->buf[c->cur],
-                                                                      (real *)c->buf[c->cur ^ 1]);
+                                                                      (real *)c->buf[dst]);
     CUDA_TRY(c, cudaGetLastError());
     c->launches++;
-    c->cur ^= 1;
+    c->cur = dst;
     snprintf(c->kname, sizeof c->kname, "rk2_fused<%s,%dx%d,CB=%d>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA, CB);
     return MM_OK;
 }
@@ -526,7 +529,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
         return fail(nullptr, MM_ERR_INVALID_ARG, "need 0 <= 2*n_end_cells <= ns");
     if (p.flags & ~(MM_FLAG_S_PERIODIC | MM_FLAG_OFFSET_PERIODIC_NOMASK | MM_FLAG_CHECK_DT | MM_FLAG_RK2_SUPERBEE))
         return fail(nullptr, MM_ERR_INVALID_ARG, "unknown flag");
-    if ((b0 == nullptr) != (b1 == nullptr)) return fail(nullptr, MM_ERR_INVALID_ARG, "pass both density buffers or neither");
+    if (b0 == nullptr && b1 != nullptr) return fail(nullptr, MM_ERR_INVALID_ARG, "pass dens_buf0, both density buffers, or neither");
     if (b0 && (b0 == b1 || ((uintptr_t)b0 & 15) || ((uintptr_t)b1 & 15)))
         return fail(nullptr, MM_ERR_INVALID_ARG, "density buffers must be distinct and 16-byte aligned");
     const int64_t nc = (int64_t)g.nx * g.ny * g.ntheta;
@@ -550,6 +553,8 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->dens_cov_count = 0;
     // measured defaults: the coefficient-form kernel, 4 substeps per pass
     c->opt_kernel = 0; c->opt_fuse_t = 4; c->opt_fuse_mom = 1;
+    c->single = (b0 != nullptr && b1 == nullptr);
+    c->opt_inplace = c->single ? 1 : 0;
     c->checked_dt = NAN; c->launches = 0; c->kname[0] = 0;
     try { c->dens_cov.assign((size_t)nc, 0); } catch (...) { delete c; return fail(nullptr, MM_ERR_NOMEM, "host allocation failed"); }
 
@@ -700,6 +705,8 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
     // 1 generic, 2 warp-streamed (1-D TMA), 3 tile, 4 coefficient form (same grids/flags as 2)
     int kind = c->opt_kernel;
     if (kind == 0) kind = stream_supported(c) ? 4 : 1;
+    if (c->single && !(kind == 4 && stream_supported(c)))
+        return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context runs only the in-place coefficient-form / fused RK2 kernels (16x16 or 8x8 offset planes, no test flags)");
     if (kind == 2 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "streamed kernel does not support this grid/flags");
     if (kind == 4 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernel does not support this grid/flags");
     if (kind == 3 && !c->tile_ok) return fail(c, MM_ERR_INVALID_ARG, "tile kernel does not support this grid/flags");
@@ -726,13 +733,14 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         } else {
             t = remaining < c->opt_fuse_t ? remaining : c->opt_fuse_t;
             const bool mom = c->opt_fuse_mom && remaining == t;
+            const bool inpl = c->opt_inplace != 0;
             s = kind == 2   ? launch_stream(c, t, mom, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
-                : kind == 4 ? launch_coef(c, t, mom, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
+                : kind == 4 ? launch_coef(c, t, mom, dt, c->buf[c->cur], c->buf[inpl ? c->cur : c->cur ^ 1])
                             : launch_tile(c, t, mom, dt, c->cur, c->buf[c->cur ^ 1]);
             if (s == MM_OK && mom) c->mom_valid = true;
         }
         if (s != MM_OK) return s;
-        c->cur ^= 1;
+        if (!(kind == 4 && c->opt_inplace)) c->cur ^= 1;
         remaining -= t;
     }
     return MM_OK;
@@ -779,7 +787,7 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
         // fp64 (measured: in-place is slower there): ping-pong passes over all configurations,
         // finished ones copied through, moments in the last pass.
         const int32_t passes = (nmax + MM_MAX_FUSE_T - 1) / MM_MAX_FUSE_T;
-        const bool inplace = sizeof(real) == 4;
+        const bool inplace = sizeof(real) == 4 || c->opt_inplace;
         for (int32_t ps = 0; ps < passes; ++ps) {
             const int32_t done = ps * MM_MAX_FUSE_T;
             mm_status s;
@@ -804,6 +812,7 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
         if (c->opt_fuse_mom) c->mom_valid = true;
         return MM_OK;
     }
+    if (c->single) return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context runs only the in-place kernels");
     KParams<real> kp = make_kparams<real>(c, 1.0);   // per unit dt; the kernels scale by dt_c
     int64_t gblocks = (c->cells + 255) / 256;
     const int64_t gcap = (int64_t)c->sm_count * 64;
@@ -934,6 +943,9 @@ extern "C" mm_status mm_set_option(mm_ctx *c, mm_option opt, int64_t v)
         c->opt_fuse_t = (int)v; return MM_OK;
     case MM_OPT_FUSE_MOMENTS:
         c->opt_fuse_mom = v ? 1 : 0; return MM_OK;
+    case MM_OPT_INPLACE:
+        if (c->single && !v) return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context is always in place");
+        c->opt_inplace = v ? 1 : 0; return MM_OK;
     }
     return fail(c, MM_ERR_INVALID_ARG, "unknown option");
 }
@@ -945,6 +957,7 @@ extern "C" mm_status mm_get_option(const mm_ctx *c, mm_option opt, int64_t *v)
     case MM_OPT_KERNEL: *v = c->opt_kernel; return MM_OK;
     case MM_OPT_FUSE_T: *v = c->opt_fuse_t; return MM_OK;
     case MM_OPT_FUSE_MOMENTS: *v = c->opt_fuse_mom; return MM_OK;
+    case MM_OPT_INPLACE: *v = c->opt_inplace; return MM_OK;
     }
     return MM_ERR_INVALID_ARG;
 }

@@ -12,6 +12,7 @@ import pytest
 import mm_inputs as mi
 from mm_inputs import Grid, Params
 from util import check_parity, gpu_run, oracle_run, random_inputs, p1_density, TOL
+from oracle import mm_oracle as orc
 
 pytestmark = pytest.mark.gpu
 
@@ -258,3 +259,65 @@ def test_coef_dirty_masked_input_is_dropped():
     out, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [2], dt, kernel=4, fuse_t=2)
     ref, _ = oracle_run(g, p, U, V, Om, m0, [2], dt)
     assert p1_density(out, ref) < TOL["f64"]
+
+
+# ------------------------------------------------------------------ in-place passes / single-buffer contexts
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("mode", ["option", "single"])
+def test_inplace_passes_match_the_oracle(dtype, mode):
+    """MM_OPT_INPLACE and a context created with ONE density buffer: Euler (T = 3, ragged Ns), RK2 + Superbee and the
+    local step all update the buffer in place and still match the oracle; the second buffer is never touched."""
+    import torch
+    from paper_1908_04279_b200 import MM, binding as b
+    from util import NPDT, TOL, p2_moments
+    g = Grid(5, 7, 20, 7, 16, 16)
+    npdt = NPDT[dtype]
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    for flags, what in ((0, "euler"), (mi.FLAG_RK2_SUPERBEE, "rk2"), (0, "local")):
+        p = Params(flags=flags)
+        dt = _dt(g, p)
+        U, V, Om, m0 = random_inputs(g, p, dtype)
+        b0 = torch.empty(g.cells, dtype=tdt, device="cuda")
+        b1 = torch.full((g.cells,), 777.0, dtype=tdt, device="cuda") if mode == "option" else None
+        mm = MM(g, p, dtype, b0, b1)
+        if mode == "option":
+            mm.set_option(b.MM_OPT_INPLACE, 1)
+        assert mm.get_option(b.MM_OPT_INPLACE) == 1
+        mm.set_option(b.MM_OPT_FUSE_T, 3)
+        mm.set_density(np.ascontiguousarray(m0, npdt))
+        mm.set_filament_velocity(U, V, Om)
+        if what == "local":
+            mm.advance_local(6.5 * dt, 0.4)
+            ref, _ = orc.advance_local(g, p, U, V, Om, m0, 6.5 * dt, 0.4)
+        else:
+            mm.substep(7, dt)
+            ref = orc.run(g, p, U, V, Om, m0, 7, dt)
+        f, t = np.empty((g.nc, 2)), np.empty(g.nc)
+        mm.moments(f, t)
+        out = np.empty((g.nc, g.ns, g.nxi, g.neta), npdt)
+        mm.get_density(out)
+        name = mm.kernel_name
+        mm.destroy()
+        assert p1_density(out, ref) <= TOL[dtype], (what, name)
+        ef, et = p2_moments(f, t, orc.moments(g, p, ref))
+        assert ef <= TOL[dtype] and et <= TOL[dtype], (what, name)
+        assert np.array_equal(out.reshape(-1), b0.cpu().numpy()), "the result lives in the one buffer"
+        if b1 is not None:
+            assert bool((b1 == 777.0).all()), "the second buffer must not be touched"
+
+
+def test_single_buffer_context_refuses_two_buffer_kernels():
+    import torch
+    from paper_1908_04279_b200 import MM, MMError, binding as b
+    g = Grid(1, 2, 4, 5, 3, 7)            # odd offset plane: generic kernels only
+    p = Params()
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    mm = MM(g, p, "f64", torch.empty(g.cells, dtype=torch.float64, device="cuda"), None)
+    mm.set_density(m0); mm.set_filament_velocity(U, V, Om)
+    with pytest.raises(MMError):
+        mm.substep(1, _dt(g, p))
+    with pytest.raises(MMError):
+        mm.advance_local(0.01, 0.4)
+    with pytest.raises(MMError):
+        mm.set_option(b.MM_OPT_INPLACE, 0)
+    mm.destroy()
