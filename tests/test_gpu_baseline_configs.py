@@ -149,3 +149,62 @@ def _is_current(mm, b0, g, npdt):
     out = np.empty((1, g.ns, g.nxi, g.neta), npdt)
     mm.get_density_range(0, 1, out)
     return np.array_equal(out.reshape(-1), b0[:g.inner].cpu().numpy())
+
+
+def test_maximum_size_single_buffer():
+    """Edge case "maximum sizes": a SINGLE-BUFFER fp32 context four times configs[4] (Nx = 512, Ny = 128: 2^35 cells,
+    137 GB in one buffer -- it would not fit double-buffered), one fused pass of 4 substeps in place + fused moments,
+    sampled configurations (first, last, around flat offsets 2^31 ... 2^35 elements) against the oracle."""
+    import torch
+    from paper_1908_04279_b200 import MM, binding as b
+
+    w = mi.CONFIGS[4]
+    g = mi.Grid(512, 128, 32, 64, 16, 16)
+    p = w.params
+    free_b, _ = torch.cuda.mem_get_info()
+    if g.cells * 4 + (3 << 30) > free_b:
+        pytest.skip(f"needs {g.cells * 4 / 1e9:.0f} GB of device memory")
+    dev = torch.device("cuda:0")
+    pick = {0, 1, g.nc - 2, g.nc - 1}
+    for e in range(31, 36):
+        cc = (2 ** e) // g.inner
+        pick.update(x for x in (cc - 1, cc) if 0 <= x < g.nc)
+    rng = np.random.default_rng(99)
+    pick.update(int(x) for x in rng.integers(0, g.nc, 12))
+    sample = sorted(pick)
+    b0 = torch.empty(g.cells, dtype=torch.float32, device=dev)
+    mm = MM(g, p, "f32", b0, None)
+    assert mm.get_option(b.MM_OPT_INPLACE) == 1
+    st = mi.Stream(g, p.R, w.seed, w.omega_max)
+    U, V, Om = st.velocities(np.float32)
+    chunk = 4096
+    buf = np.empty((chunk, g.ns, g.nxi, g.neta), np.float32)
+    m0, sset = {}, set(sample)
+    for c0 in range(0, g.nc, chunk):
+        n = min(chunk, g.nc - c0)
+        st.density(n, np.float32, out=buf[:n])
+        mm.set_density_range(c0, n, buf[:n])
+        for c in sset.intersection(range(c0, c0 + n)):
+            m0[c] = buf[c - c0].copy()
+    st.close()
+    mm.set_filament_velocity(U, V, Om)
+    mm.substep(4, w.dt)
+    F = torch.empty((g.nc, 2), dtype=torch.float64, device=dev)
+    T = torch.empty(g.nc, dtype=torch.float64, device=dev)
+    mm.moments(F, T)
+    torch.cuda.synchronize()
+    assert mm.kernel_name.startswith("coef<f32"), mm.kernel_name
+    Fh, Th = F.cpu().numpy(), T.cpu().numpy()
+    assert np.isfinite(Fh).all() and np.isfinite(Th).all()
+    worst = 0.0
+    for c in sample:
+        ref = orc.run(g, p, U[c:c + 1], V[c:c + 1], Om[c:c + 1], m0[c][None], 4, w.dt, c_first=c)
+        out = np.empty((1, g.ns, g.nxi, g.neta), np.float32)
+        mm.get_density_range(c, 1, out)
+        e1 = p1_density(out, ref)
+        rm = orc.moments(g, p, ref, c_first=c)
+        ef, et = p2_moments(Fh[c:c + 1], Th[c:c + 1], rm)
+        worst = max(worst, e1, ef, et)
+        assert e1 <= TOL["f32"] and ef <= TOL["f32"] and et <= TOL["f32"], (c, e1, ef, et)
+    mm.destroy()
+    print(f"single-buffer {g.cells / 2**30:.0f} Gi cells ({g.cells * 4 / 1e9:.0f} GB): {len(sample)} configurations vs oracle, worst {worst:.2e}")
