@@ -185,6 +185,10 @@ def run_cuda(args):
     free_b, _ = torch.cuda.mem_get_info()
     idx = pick_workload(args.config, free_b)
     w = with_scheme(rank_workload(mi.CONFIGS[idx], rank), args.scheme)
+    if args.nx_mult > 1:   # a larger outer grid of the same structure (needs --single-buffer beyond 90 GB per buffer)
+        g0 = w.grid
+        w = mi.Workload(w.name + f"_nx{args.nx_mult}", mi.Grid(g0.nx * args.nx_mult, g0.ny, g0.ntheta, g0.ns, g0.nxi, g0.neta),
+                        w.dtype, w.n_sub, w.moments_every, w.omega_max, w.seed, w.params)
     g, es = w.grid, ES[w.dtype]
     tdt = torch.float64 if w.dtype == "f64" else torch.float32
     log(f"workload configs[{idx}] {w.name}: Nc={g.nc} cells={g.cells} dtype={w.dtype} n_sub={w.n_sub} "
@@ -192,7 +196,7 @@ def run_cuda(args):
 
     stream = torch.cuda.current_stream()
     b0 = torch.empty(g.cells, dtype=tdt, device=dev)
-    b1 = torch.empty(g.cells, dtype=tdt, device=dev)
+    b1 = None if args.single_buffer else torch.empty(g.cells, dtype=tdt, device=dev)
     mm = MM(g, w.params, w.dtype, b0, b1, stream=stream.cuda_stream)
     if args.fuse_t:
         mm.set_option(b.MM_OPT_FUSE_T, args.fuse_t)
@@ -350,7 +354,7 @@ def run_cuda(args):
            "config": {"workload": f"configs[{idx}] {w.name}", "grid": [g.nx, g.ny, g.ntheta, g.ns, g.nxi, g.neta],
                       "cells_per_gpu": g.cells, "n_sub_per_step": w.n_sub, "moments_every": w.moments_every,
                       "dt": w.dt, "seed": w.seed, "parallelism": f"configs x{world} (no collective)",
-                      "l2": "inputs larger than L2 (two density buffers of %.1f GB)" % (g.cells * es / 1e9)},
+                      "l2": "inputs larger than L2 (%s of %.1f GB)" % ("one density buffer, passes in place" if args.single_buffer else "two density buffers", g.cells * es / 1e9)},
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "impl": "cuda"}
     if spread_info:
         out["spread_force"] = spread_info
@@ -458,6 +462,9 @@ def main():
                     help="euler = forward Euler + upwind (north_star, default); rk2 = RK2 + Superbee in s (NEXT-1)")
     ap.add_argument("--local-dt", action="store_true",
                     help="NEXT-3: advance each macro interval with mm_advance_local (per-configuration local steps)")
+    ap.add_argument("--single-buffer", action="store_true",
+                    help="create the context with ONE density buffer: every pass in place (MM_OPT_INPLACE), half the memory")
+    ap.add_argument("--nx-mult", type=int, default=1, help="multiply the workload's Nx (a larger problem of the same structure)")
     ap.add_argument("--spread", action="store_true",
                     help="NEXT-4: also time mm_spread_force (motor-force spreading, Eq. 10) on the final density")
     ap.add_argument("--cfl", type=float, default=0.4, help="CFL number of --local-dt")
