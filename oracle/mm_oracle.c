@@ -100,10 +100,22 @@ static double superbee_slope(double a, double b) { return maxmod(minmod(2.0 * a,
  * (mbase = m^n both times; m = m^n with dt/2, then m = m* with dt).  `limited` switches the s flux
  * from first-order upwind to the Superbee-limited one.
  * m, mbase, mnew: [ns][nxi][neta], b fastest.  scratch: 3 flux arrays (sizes below). */
+/* Nearest node of the periodic (x, y) grid to the anchor (tail) of cell (c, j, a, b) -- SURVEY.md 8(f) NEXT-2,
+ * reading Q38/Q39: the tail is the head minus the stalk offset, r0 = x_c + s_j p_c - (xi_a, eta_b). */
+static size_t anchor_node(const mmo_grid *g, int ix, int iy, double ct, double st, double sj, double xi, double eta)
+{
+    double rx = ((double)ix / g->nx + sj * ct - xi) * g->nx, ry = ((double)iy / g->ny + sj * st - eta) * g->ny;
+    long nx_ = (long)floor(rx + 0.5) % g->nx, ny_ = (long)floor(ry + 0.5) % g->ny;
+    if (nx_ < 0) nx_ += g->nx;
+    if (ny_ < 0) ny_ += g->ny;
+    return (size_t)nx_ * g->ny + (size_t)ny_;
+}
+
 static void stage_config(const mmo_grid *g, const mmo_params *p, int itheta,
                          double U, double V, double Om, double dt,
                          const double *mbase, const double *m, double *mnew, int limited,
-                         double *Fs, double *Fxi, double *Feta)
+                         double *Fs, double *Fxi, double *Feta,
+                         const double *Mf, int ix, int iy)   /* Mf != NULL: source k_on M_f(r0) (Eq. 4 with Eq. 6) */
 {
     const int ns = g->ns, nxi = g->nxi, neta = g->neta;
     const int per_s = (p->flags & MMO_S_PERIODIC) != 0;
@@ -184,6 +196,10 @@ static void stage_config(const mmo_grid *g, const mmo_params *p, int itheta,
                 double kappa = p->k_off0 * exp(p->k_spring * r / p->f_detach) * E;     /* Bell law (Q7) */
                 int in = inside(g, p, a, b);
                 double src = in ? p->k_on * p->m_free : 0.0;                           /* Q11 */
+                if (Mf && in) {                                                        /* Q42: k_on M_f at the anchor's node */
+                    double sj = p->s_lo + (j + 0.5) * ds;
+                    src = p->k_on * Mf[anchor_node(g, ix, iy, ct, st, sj, xi, eta)];
+                }
                 double mc = M(j, a, b);
                 double div = (FS(j + 1, a, b) - FS(j, a, b)) / ds
                            + (FXI(j, a + 1, b) - FXI(j, a, b)) / dxi
@@ -208,9 +224,9 @@ static size_t scratch_doubles(const mmo_grid *g)
 /* Advance configurations [0, n_configs) by n_sub substeps of size dt, in place.
  * m: [n_configs][ns][nxi][neta]; U,V,Om: [n_configs]; itheta0: theta index of the first
  * configuration is (c_first % ntheta) where c_first is the global index of m's first config. */
-int mmo_run(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
-            const double *U, const double *V, const double *Om,
-            double *m, int32_t n_sub, double dt)
+static int run_impl(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
+                    const double *U, const double *V, const double *Om,
+                    double *m, int32_t n_sub, double dt, const double *Mf)
 {
     const size_t inner = (size_t)g->ns * g->nxi * g->neta;
     int fail = 0;
@@ -225,19 +241,83 @@ int mmo_run(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_c
         double *half = tmp + inner;
         double *cur = m + (size_t)c * inner;
         int itheta = (int)((c_first + c) % g->ntheta);
+        int iy = (int)(((c_first + c) / g->ntheta) % g->ny), ix = (int)((c_first + c) / ((int64_t)g->ntheta * g->ny));
         for (int n = 0; n < n_sub; ++n) {
             if (p->flags & MMO_RK2_SUPERBEE) {
                 /* Alg. 2 l.9: M_b at t + dt/2;  l.10: M_b at t + dt */
-                stage_config(g, p, itheta, U[c], V[c], Om[c], 0.5 * dt, cur, cur, half, 1, Fs, Fxi, Feta);
-                stage_config(g, p, itheta, U[c], V[c], Om[c], dt, cur, half, tmp, 1, Fs, Fxi, Feta);
+                stage_config(g, p, itheta, U[c], V[c], Om[c], 0.5 * dt, cur, cur, half, 1, Fs, Fxi, Feta, Mf, ix, iy);
+                stage_config(g, p, itheta, U[c], V[c], Om[c], dt, cur, half, tmp, 1, Fs, Fxi, Feta, Mf, ix, iy);
             } else {
-                stage_config(g, p, itheta, U[c], V[c], Om[c], dt, cur, cur, tmp, 0, Fs, Fxi, Feta);
+                stage_config(g, p, itheta, U[c], V[c], Om[c], dt, cur, cur, tmp, 0, Fs, Fxi, Feta, Mf, ix, iy);
             }
             memcpy(cur, tmp, sizeof(double) * inner);   /* "swap buffers" */
         }
         free(scr);
     }
     return fail ? -1 : 0;
+}
+
+int mmo_run(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
+            const double *U, const double *V, const double *Om,
+            double *m, int32_t n_sub, double dt)
+{
+    return run_impl(g, p, c_first, n_configs, U, V, Om, m, n_sub, dt, NULL);
+}
+
+/* ---- free-motor coupling -----------------------------------------------------------------
+ * Eq. 5: M_b,coarse = iiint M_b Psi ds dx dtheta (per r0);  Eq. 6: M_f = M - M_b,coarse;
+ * Alg. 2 l.14-20: compute M_b,coarse(r0) (reduction); if M_total(r0) < M_b,coarse(r0): scale all
+ * M_b of that r0 and set M_b,coarse = M_total; compute M_f(r0).  Readings Q38-Q42:
+ *  - the anchor of cell (c,j,a,b) is r0 = x_c + s_j p_c - (xi_a, eta_b); it is binned to the NEAREST node of the
+ *    periodic (x, y) grid, so that every cell belongs to exactly one r0 (the cap rescales "all M_b with that r0");
+ *  - M_b,coarse[n] = dtheta ds dxi deta sum_{cells -> n} Psi_c m   (dx at fixed r0 is dxi deta; h_x h_y cancels);
+ *  - M_total = params.m_free at every node; f[n] = min(1, M_total / M_b,coarse[n]) multiplies the cells of node n;
+ *  - M_f[n] = M_total - min(M_b,coarse[n], M_total) >= 0 then feeds the source k_on M_f(r0) 1_disc of Eq. 4.
+ * m: ALL configurations [nc][ns][nxi][neta], rescaled in place; Mbc, Mf: [nx][ny] (outputs, either may be NULL). */
+int mmo_free_motors(const mmo_grid *g, const mmo_params *p, double *m, const double *psi, double *Mbc, double *Mf)
+{
+    const int ns = g->ns, nxi = g->nxi, neta = g->neta;
+    const int64_t nc = (int64_t)g->nx * g->ny * g->ntheta;
+    const size_t nn = (size_t)g->nx * g->ny, inner = (size_t)ns * nxi * neta;
+    const double R = p->R;
+    const double ds = (p->s_hi - p->s_lo) / ns, dxi = 2.0 * R / nxi, deta = 2.0 * R / neta;
+    const double w = 2.0 * MMO_PI / (double)g->ntheta * ds * dxi * deta;
+    double *acc = (double *)calloc(nn, sizeof(double));
+    if (!acc) return -1;
+    for (int pass = 0; pass < 2; ++pass) {              /* pass 0: coarse sums; pass 1: cap rescale */
+        for (int64_t c = 0; c < nc; ++c) {
+            int itheta = (int)(c % g->ntheta);
+            int iy = (int)((c / g->ntheta) % g->ny), ix = (int)(c / ((int64_t)g->ntheta * g->ny));
+            double theta = 2.0 * MMO_PI * (double)itheta / (double)g->ntheta;
+            double ct = cos(theta), st = sin(theta);
+            for (int j = 0; j < ns; ++j) {
+                double sj = p->s_lo + (j + 0.5) * ds;
+                for (int a = 0; a < nxi; ++a)
+                    for (int b = 0; b < neta; ++b) {
+                        double xi = -R + (a + 0.5) * dxi, eta = -R + (b + 0.5) * deta;
+                        size_t n = anchor_node(g, ix, iy, ct, st, sj, xi, eta);
+                        double *v = &m[(size_t)c * inner + ((size_t)j * nxi + a) * neta + b];
+                        if (pass == 0) acc[n] += w * psi[c] * (*v);
+                        else if (acc[n] > p->m_free) *v *= p->m_free / acc[n];
+                    }
+            }
+        }
+    }
+    for (size_t n = 0; n < nn; ++n) {
+        double capped = acc[n] > p->m_free ? p->m_free : acc[n];
+        if (Mbc) Mbc[n] = capped;
+        if (Mf) Mf[n] = p->m_free - capped;
+    }
+    free(acc);
+    return 0;
+}
+
+/* mmo_run with the source k_on M_f(r0) of the given free-motor table (frozen over these substeps). */
+int mmo_run_coupled(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
+                    const double *U, const double *V, const double *Om,
+                    double *m, int32_t n_sub, double dt, const double *Mf)
+{
+    return run_impl(g, p, c_first, n_configs, U, V, Om, m, n_sub, dt, Mf);
 }
 
 /* ---- local adaptive time step per independent unit ------------------------------------

@@ -57,6 +57,10 @@ def _load():
         lib.mmo_advance_local.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, dbl, dbl, vp]
         lib.mmo_spread_force.restype = ctypes.c_int
         lib.mmo_spread_force.argtypes = [vp, vp, i64, i64, vp, vp, vp]
+        lib.mmo_free_motors.restype = ctypes.c_int
+        lib.mmo_free_motors.argtypes = [vp, vp, vp, vp, vp, vp]
+        lib.mmo_run_coupled.restype = ctypes.c_int
+        lib.mmo_run_coupled.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, dbl, vp]
         lib.mmo_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -145,6 +149,38 @@ def spread_force(grid, params, m, psi, c_first: int = 0, F2=None) -> np.ndarray:
     assert F2.dtype == np.float64 and F2.flags.c_contiguous and F2.shape == (grid.nx, grid.ny, 2)
     lib.mmo_spread_force(ctypes.byref(g), ctypes.byref(p), c_first, n, m.ctypes.data, psi.ctypes.data, F2.ctypes.data)
     return F2
+
+
+def free_motors(grid, params, m, psi):
+    """Free-motor coupling (Eq. 5-6, Alg. 2 l.14-20; readings Q38-Q42).  m: ALL configurations.  Returns
+    (m after the cap rescale [fp64 copy], M_b,coarse [nx][ny] after the cap, M_f [nx][ny])."""
+    lib = _load()
+    g, p = _grid(grid), _params(params)
+    out = np.array(m, dtype=np.float64, order="C", copy=True)
+    nc = grid.nx * grid.ny * grid.ntheta
+    assert out.size == nc * grid.ns * grid.nxi * grid.neta
+    psi = _f64(psi, nc)
+    Mbc, Mf = np.empty((grid.nx, grid.ny)), np.empty((grid.nx, grid.ny))
+    rc = lib.mmo_free_motors(ctypes.byref(g), ctypes.byref(p), out.ctypes.data, psi.ctypes.data, Mbc.ctypes.data, Mf.ctypes.data)
+    if rc != 0:
+        raise MemoryError("oracle scratch allocation failed")
+    return out.reshape(nc, grid.ns, grid.nxi, grid.neta), Mbc, Mf
+
+
+def run_coupled(grid, params, U, V, Om, m, n_sub: int, dt: float, Mf, c_first: int = 0) -> np.ndarray:
+    """`run` with the source k_on M_f(r0) of the free-motor table Mf [nx][ny] (reading Q42)."""
+    lib = _load()
+    g, p = _grid(grid), _params(params)
+    inner = grid.ns * grid.nxi * grid.neta
+    out = np.array(m, dtype=np.float64, order="C", copy=True)
+    n = out.size // inner
+    U, V, Om = _f64(U, n), _f64(V, n), _f64(Om, n)
+    Mf = _f64(Mf, grid.nx * grid.ny)
+    rc = lib.mmo_run_coupled(ctypes.byref(g), ctypes.byref(p), c_first, n, U.ctypes.data, V.ctypes.data, Om.ctypes.data,
+                             out.ctypes.data, n_sub, dt, Mf.ctypes.data)
+    if rc != 0:
+        raise MemoryError("oracle scratch allocation failed")
+    return out.reshape(n, grid.ns, grid.nxi, grid.neta)
 
 
 def moments(grid, params, m, c_first: int = 0):
