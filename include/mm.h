@@ -92,6 +92,9 @@ typedef enum {
                                 default 4 */
     MM_OPT_FUSE_MOMENTS = 2, /* 1 (default): the last pass of mm_substep also reduces the moments, so a
                                 following mm_moments is a copy; 0: mm_moments always runs its own pass */
+    MM_OPT_FREE_COUPLING = 4,/* 1: the source term of the substeps is k_on M_f(r0) from the table of the last
+                                mm_update_free_motors (which switches it on); 0: the constant k_on m_free again.
+                                MM_ERR_STATE when set to 1 before any mm_update_free_motors */
     MM_OPT_INPLACE = 3       /* 1: the coefficient-form, fused RK2 and local-step kernels update the current density
                                 buffer IN PLACE (plane j of the result depends on input planes <= j only, each already
                                 staged on the SM when plane j is stored, and one warp owns a configuration), the other
@@ -159,6 +162,18 @@ mm_status mm_local_steps(mm_ctx *ctx, int32_t *n_steps, double *lambda, int dst_
  *                   MM_ERR_STATE unless density and Psi have been set. */
 mm_status mm_set_psi(mm_ctx *ctx, const double *psi, int src_on_device);
 mm_status mm_spread_force(mm_ctx *ctx, double *F2, int dst_on_device);
+
+/* free-motor coupling (Eq. 5-6; Alg. 2 l.14-20).  Readings
+ * Q38-Q42 in DESIGN.md: the anchor of cell (c,j,a,b) is r0 = (ix/nx, iy/ny) + s_j p_c - (xi_a, eta_b), binned to the
+ * nearest node of the periodic (x, y) grid;
+ *     M_b,coarse[n] = dtheta ds dxi deta sum_{cells -> n} Psi_c m;      M_total = params.m_free at every node;
+ * where M_b,coarse[n] > M_total every cell of node n is scaled by M_total / M_b,coarse[n] (the density IS modified) and
+ * M_b,coarse[n] = M_total; M_f[n] = M_total - M_b,coarse[n] >= 0.  The call stores M_f and switches the source of the
+ * following substeps to k_on M_f(r0) 1_disc (MM_OPT_FREE_COUPLING), frozen until the next call.  With the coupled
+ * source mm_substep runs the generic kernels (two density buffers; MM_OPT_KERNEL 0 or 1) and mm_advance_local is
+ * refused.  Mb_coarse, M_free: [nx][ny] fp64 outputs, either may be NULL.  Needs mm_set_psi.  fp64 atomic adds: the
+ * summation order varies from call to call. */
+mm_status mm_update_free_motors(mm_ctx *ctx, double *Mb_coarse, double *M_free, int dst_on_device);
 
 /* Moments (S9) of the current density: force [Nc][2] = (Fx, Fy), torque [Nc]; always fp64
  * (macroscale data stays double precision).  Either pointer may be NULL to skip it. */

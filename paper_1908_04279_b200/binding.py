@@ -13,13 +13,13 @@ from . import build as _build
 MM_F32, MM_F64 = 0, 1
 MM_OK, MM_ERR_INVALID_ARG, MM_ERR_CUDA, MM_ERR_NOMEM, MM_ERR_STATE, MM_ERR_UNSTABLE = 0, -1, -2, -3, -4, -5
 MM_FLAG_S_PERIODIC, MM_FLAG_OFFSET_PERIODIC_NOMASK, MM_FLAG_CHECK_DT = 1, 2, 4
-MM_OPT_KERNEL, MM_OPT_FUSE_T, MM_OPT_FUSE_MOMENTS, MM_OPT_INPLACE = 0, 1, 2, 3
+MM_OPT_KERNEL, MM_OPT_FUSE_T, MM_OPT_FUSE_MOMENTS, MM_OPT_INPLACE, MM_OPT_FREE_COUPLING = 0, 1, 2, 3, 4
 MM_MAX_FUSE_T = 4
 
 EXPORTS = ["mm_create", "mm_set_density", "mm_get_density", "mm_set_density_range", "mm_get_density_range",
            "mm_set_filament_velocity", "mm_substep", "mm_moments", "mm_set_option", "mm_get_option", "mm_launch_count",
            "mm_kernel_name", "mm_destroy", "mm_status_string", "mm_last_error", "mm_advance_local", "mm_local_steps", "mm_set_psi",
-           "mm_spread_force"]
+           "mm_spread_force", "mm_update_free_motors"]
 
 
 class mm_grid(ctypes.Structure):
@@ -63,6 +63,7 @@ def lib():
         L.mm_local_steps.argtypes = [vp, vp, vp, ctypes.c_int]
         L.mm_set_psi.argtypes = [vp, vp, ctypes.c_int]
         L.mm_spread_force.argtypes = [vp, vp, ctypes.c_int]
+        L.mm_update_free_motors.argtypes = [vp, vp, vp, ctypes.c_int]
         L.mm_set_option.argtypes = [vp, ctypes.c_int, i64]
         L.mm_get_option.argtypes = [vp, ctypes.c_int, ctypes.POINTER(i64)]
         L.mm_launch_count.argtypes = [vp]
@@ -166,6 +167,11 @@ class MM:
         pf, dev = _ptr(F2)
         self._check(self._L.mm_spread_force(self._h, pf, dev))
         return F2
+
+    def update_free_motors(self, Mb_coarse=None, M_free=None):
+        (pb, d0), (pf, d1) = _ptr(Mb_coarse), _ptr(M_free)
+        self._check(self._L.mm_update_free_motors(self._h, pb, pf, d0 if Mb_coarse is not None else d1))
+        return Mb_coarse, M_free
 
     def moments(self, force, torque):
         (pf, d0), (pt, d1) = _ptr(force), _ptr(torque)

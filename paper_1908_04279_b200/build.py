@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libmm.so")
 SOURCES = [os.path.join(CSRC, "mm_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("mm_common.cuh", "mm_ptx.cuh", "mm_generic.cuh", "mm_stream.cuh", "mm_tile.cuh", "mm_coef.cuh", "mm_rk2.cuh", "mm_local.cuh", "mm_spread.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("mm_common.cuh", "mm_ptx.cuh", "mm_generic.cuh", "mm_stream.cuh", "mm_tile.cuh", "mm_coef.cuh", "mm_rk2.cuh", "mm_local.cuh", "mm_spread.cuh", "mm_free.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "mm.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]

@@ -18,6 +18,7 @@
 #include "mm_rk2.cuh"
 #include "mm_local.cuh"
 #include "mm_spread.cuh"
+#include "mm_free.cuh"
 
 using namespace mm;
 
@@ -50,6 +51,9 @@ struct mm_ctx {
     bool loc_valid;
     double *psi, *fline, *F2;       // NEXT-4: filament density weights [nc], plane forces [nc][ns][2], fluid-grid force
     bool psi_set;
+    double *Mf, *Mbc, *free_raw, *free_factor;   // NEXT-2: free / coarse bound motor tables [nx][ny], scratch
+    int *free_any;
+    bool coupled;                   // the substep source is k_on M_f(r0) instead of k_on m_free
     CUtensorMap tmap[2];            // tiled-TMA views of buf[0], buf[1] (tile kernel)
     bool tile_ok;                   // tensor maps built and grid/flags supported by the tile kernel
     std::string err;
@@ -84,6 +88,10 @@ static KParams<real> make_kparams(const mm_ctx *c, double dt)
     k.R = (real)p.R; k.dxi = (real)dxi; k.deta = (real)deta; k.ds = (real)ds; k.s_lo = (real)p.s_lo;
     k.dt = (real)dt; k.dt_ds = (real)(dt / ds); k.dt_dxi = (real)(dt / dxi); k.dt_deta = (real)(dt / deta);
     k.dt_src = (real)(dt * p.k_on * p.m_free);
+    k.dt_kon = (real)(dt * p.k_on);
+    k.Mf = (c->coupled && c->Mf) ? c->Mf : nullptr;
+    k.nx = g.nx; k.ny = g.ny;
+    k.geo_R = p.R; k.geo_dxi = dxi; k.geo_deta = deta; k.geo_ds = ds; k.geo_s_lo = p.s_lo;
     k.dt_endx = (real)(dt * (p.end_detach_mult - 1.0));
     k.mom_scale = -p.k_spring * ds * dxi * deta;
     k.U = (const real *)c->U; k.V = (const real *)c->V; k.Om = (const real *)c->Om;
@@ -549,6 +557,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->loc_lambda = nullptr; c->loc_n = c->loc_nmax = c->loc_list = c->loc_count = nullptr; c->loc_dt = nullptr;
     c->loc_valid = false;
     c->psi = c->fline = c->F2 = nullptr; c->psi_set = false;
+    c->Mf = c->Mbc = c->free_raw = c->free_factor = nullptr; c->free_any = nullptr; c->coupled = false;
     c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
     // measured defaults: the coefficient-form kernel, 4 substeps per pass
@@ -613,6 +622,7 @@ extern "C" mm_status mm_destroy(mm_ctx *c)
     cudaFree(c->loc_lambda); cudaFree(c->loc_n); cudaFree(c->loc_nmax); cudaFree(c->loc_dt);
     cudaFree(c->loc_list); cudaFree(c->loc_count);
     cudaFree(c->psi); cudaFree(c->fline); cudaFree(c->F2);
+    cudaFree(c->Mf); cudaFree(c->Mbc); cudaFree(c->free_raw); cudaFree(c->free_factor); cudaFree(c->free_any);
     delete c;
     return MM_OK;
 }
@@ -704,7 +714,9 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
     // kernel choice: 0 auto (coefficient form when the grid/flags are supported; else generic),
     // 1 generic, 2 warp-streamed (1-D TMA), 3 tile, 4 coefficient form (same grids/flags as 2)
     int kind = c->opt_kernel;
-    if (kind == 0) kind = stream_supported(c) ? 4 : 1;
+    if (kind == 0) kind = (stream_supported(c) && !c->coupled) ? 4 : 1;
+    if (c->coupled && kind != 1)
+        return fail(c, MM_ERR_INVALID_ARG, "the free-motor coupled source runs on the generic kernels (MM_OPT_KERNEL 0 or 1)");
     if (c->single && !(kind == 4 && stream_supported(c)))
         return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context runs only the in-place coefficient-form / fused RK2 kernels (16x16 or 8x8 offset planes, no test flags)");
     if (kind == 2 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "streamed kernel does not support this grid/flags");
@@ -715,7 +727,7 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         // kernel 0 (auto): the fused one-pass kernel where the grid is supported, else the generic stages; 1: generic
         if (c->opt_kernel != 0 && c->opt_kernel != 1)
             return fail(c, MM_ERR_INVALID_ARG, "RK2 + Superbee runs on kernel 0 (auto) or 1 (generic)");
-        const bool fused = c->opt_kernel == 0 && stream_supported(c);
+        const bool fused = c->opt_kernel == 0 && stream_supported(c) && !c->coupled;
         for (int n = 0; n < n_sub; ++n) {
             mm_status s = fused ? launch_rk2_fused_any(c, dt)
                                 : c->dtype == MM_F64 ? launch_rk2_generic<double>(c, dt) : launch_rk2_generic<float>(c, dt);
@@ -835,6 +847,7 @@ extern "C" mm_status mm_advance_local(mm_ctx *c, double dt, double cfl)
         return fail(c, MM_ERR_INVALID_ARG, "dt and cfl must be finite and > 0");
     if (c->p.flags & MM_FLAG_RK2_SUPERBEE)
         return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local drives the forward-Euler scheme only (no MM_FLAG_RK2_SUPERBEE yet)");
+    if (c->coupled) return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local does not take the free-motor coupled source yet");
     if (c->dens_cov_count != c->nc || !c->vel_set) return fail(c, MM_ERR_STATE, "set density and filament velocity first");
     if (!c->loc_n) {
         CUDA_TRY(c, cudaMalloc(&c->loc_lambda, (size_t)c->nc * sizeof(double)));
@@ -915,6 +928,56 @@ extern "C" mm_status mm_spread_force(mm_ctx *c, double *F2, int on_device)
     return MM_OK;
 }
 
+// ---- NEXT-2: free-motor coupling (mm_free.cuh) -------------------------------------------------------------------
+template <typename real>
+static mm_status free_impl(mm_ctx *c)
+{
+    const mm_grid &g = c->g;
+    const mm_params &p = c->p;
+    FreeGeom q;
+    q.R = p.R; q.dxi = 2.0 * p.R / g.nxi; q.deta = 2.0 * p.R / g.neta; q.ds = (p.s_hi - p.s_lo) / g.ns; q.s_lo = p.s_lo;
+    q.ns = g.ns; q.nxi = g.nxi; q.neta = g.neta; q.ntheta = g.ntheta; q.nx = g.nx; q.ny = g.ny;
+    const int nn = g.nx * g.ny;
+    const double w = 2.0 * 3.14159265358979323846264338327950288 / (double)g.ntheta * q.ds * q.dxi * q.deta;
+    CUDA_TRY(c, cudaMemsetAsync(c->free_raw, 0, (size_t)nn * sizeof(double), c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->free_any, 0, sizeof(int), c->stream));
+    int64_t blocks = (c->nc + 7) / 8;
+    const int64_t cap = (int64_t)c->sm_count * 8;
+    if (blocks > cap) blocks = cap;
+    real *dens = (real *)c->buf[c->cur];
+    free_cells_kernel<real, 0><<<(unsigned)blocks, 256, 0, c->stream>>>(q, c->nc, dens, c->psi, w, c->free_raw, nullptr, nullptr);
+    CUDA_TRY(c, cudaGetLastError());
+    free_cap_kernel<<<(nn + 255) / 256, 256, 0, c->stream>>>(nn, p.m_free, c->free_raw, c->free_factor, c->Mbc, c->Mf, c->free_any);
+    CUDA_TRY(c, cudaGetLastError());
+    free_cells_kernel<real, 1><<<(unsigned)blocks, 256, 0, c->stream>>>(q, c->nc, dens, nullptr, 0.0, nullptr, c->free_factor, c->free_any);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches += 3;
+    return MM_OK;
+}
+
+extern "C" mm_status mm_update_free_motors(mm_ctx *c, double *Mb_coarse, double *M_free, int on_device)
+{
+    if (!c) return MM_ERR_INVALID_ARG;
+    if (c->dens_cov_count != c->nc || !c->psi_set) return fail(c, MM_ERR_STATE, "set density and psi first");
+    const size_t nn = (size_t)c->g.nx * c->g.ny;
+    if (!c->Mf) {
+        CUDA_TRY(c, cudaMalloc(&c->Mf, nn * sizeof(double)));
+        CUDA_TRY(c, cudaMalloc(&c->Mbc, nn * sizeof(double)));
+        CUDA_TRY(c, cudaMalloc(&c->free_raw, nn * sizeof(double)));
+        CUDA_TRY(c, cudaMalloc(&c->free_factor, nn * sizeof(double)));
+        CUDA_TRY(c, cudaMalloc(&c->free_any, sizeof(int)));
+    }
+    mm_status s = c->dtype == MM_F64 ? free_impl<double>(c) : free_impl<float>(c);
+    if (s != MM_OK) return s;
+    c->coupled = true;
+    c->mom_valid = false;     // the cap may have rescaled the density
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (Mb_coarse) CUDA_TRY(c, cudaMemcpyAsync(Mb_coarse, c->Mbc, nn * sizeof(double), kind, c->stream));
+    if (M_free) CUDA_TRY(c, cudaMemcpyAsync(M_free, c->Mf, nn * sizeof(double), kind, c->stream));
+    if (!on_device) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MM_OK;
+}
+
 extern "C" mm_status mm_moments(mm_ctx *c, double *force, double *torque, int on_device)
 {
     if (!c) return MM_ERR_INVALID_ARG;
@@ -943,6 +1006,9 @@ extern "C" mm_status mm_set_option(mm_ctx *c, mm_option opt, int64_t v)
         c->opt_fuse_t = (int)v; return MM_OK;
     case MM_OPT_FUSE_MOMENTS:
         c->opt_fuse_mom = v ? 1 : 0; return MM_OK;
+    case MM_OPT_FREE_COUPLING:
+        if (v && !c->Mf) return fail(c, MM_ERR_STATE, "no free-motor table yet: call mm_update_free_motors first");
+        c->coupled = v != 0; return MM_OK;
     case MM_OPT_INPLACE:
         if (c->single && !v) return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context is always in place");
         c->opt_inplace = v ? 1 : 0; return MM_OK;
@@ -958,6 +1024,7 @@ extern "C" mm_status mm_get_option(const mm_ctx *c, mm_option opt, int64_t *v)
     case MM_OPT_FUSE_T: *v = c->opt_fuse_t; return MM_OK;
     case MM_OPT_FUSE_MOMENTS: *v = c->opt_fuse_mom; return MM_OK;
     case MM_OPT_INPLACE: *v = c->opt_inplace; return MM_OK;
+    case MM_OPT_FREE_COUPLING: *v = c->coupled ? 1 : 0; return MM_OK;
     }
     return MM_ERR_INVALID_ARG;
 }

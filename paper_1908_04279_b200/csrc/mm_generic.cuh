@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(256) substep_generic_kernel(const __grid_const
         const bool endc = (j < kp.n_end) || (j >= ns - kp.n_end);
         const real kap = kp.kappa[rem];
         real acc = m - kp.dt_ds * div_s - kp.dt_dxi * (Fxh - Fxl) - kp.dt_deta * (Feh - Fel);
-        acc += kp.dt_src - kp.dt * kap * m;
+        acc += source_increment(kp, c, j, a, b) - kp.dt * kap * m;
         if (endc) acc -= kp.dt_endx * kap * m;
         out[idx] = kp.inside[rem] ? acc : real(0);
     }

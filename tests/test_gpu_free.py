@@ -1,0 +1,83 @@
+"""GPU parity of the free-motor coupling (mm_update_free_motors + coupled source) against the
+oracle: coarse bound density, cap rescale, free density, and substeps driven by k_on M_f(r0)."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import mm_inputs as mi
+from mm_inputs import Grid, Params
+from oracle import mm_oracle as orc
+from util import NPDT, TOL, p1_density, random_inputs
+
+pytestmark = pytest.mark.gpu
+RNG = np.random.default_rng(2024)
+
+
+def gpu_coupled(g, p, dtype, U, V, Om, m0, psi, n_sub, dt):
+    from paper_1908_04279_b200 import MM, binding as b
+    mm = MM(g, p, dtype)
+    mm.set_density(np.ascontiguousarray(m0, NPDT[dtype]))
+    mm.set_filament_velocity(*(np.ascontiguousarray(x, NPDT[dtype]) for x in (U, V, Om)))
+    mm.set_psi(np.ascontiguousarray(psi, np.float64))
+    Mbc, Mf = np.empty((g.nx, g.ny)), np.empty((g.nx, g.ny))
+    mm.update_free_motors(Mbc, Mf)
+    assert mm.get_option(b.MM_OPT_FREE_COUPLING) == 1
+    capped = np.empty((g.nc, g.ns, g.nxi, g.neta), NPDT[dtype])
+    mm.get_density(capped)
+    mm.substep(n_sub, dt)
+    out = np.empty_like(capped)
+    mm.get_density(out)
+    name = mm.kernel_name
+    mm.destroy()
+    return Mbc, Mf, capped, out, name
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("flags", [0, mi.FLAG_RK2_SUPERBEE])
+@pytest.mark.parametrize("shape", [(6, 6, 8, 6, 16, 16), (5, 4, 4, 5, 6, 6), (8, 8, 4, 6, 8, 8)])
+def test_free_motor_coupling_parity(dtype, flags, shape):
+    g = Grid(*shape)
+    big = Params(flags=flags, m_free=1e9)
+    U, V, Om, m0 = random_inputs(g, big, dtype)
+    psi = RNG.random(g.nc) * 30.0
+    _, raw, _ = orc.free_motors(g, big, m0, psi)
+    p = dataclasses.replace(big, m_free=float(np.median(raw)))      # half of the nodes get capped
+    dt = mi.benchmark_dt(g, p, 1.0)
+    Mbc, Mf, capped, out, name = gpu_coupled(g, p, dtype, U, V, Om, m0, psi, 4, dt)
+    m_ref, Mbc_ref, Mf_ref = orc.free_motors(g, p, m0, psi)
+    tol = TOL[dtype]
+    assert np.max(np.abs(Mbc - Mbc_ref)) / p.m_free <= tol and np.max(np.abs(Mf - Mf_ref)) / p.m_free <= tol
+    assert (Mf >= 0).all() and (Mbc <= p.m_free).all()
+    assert p1_density(capped, m_ref) <= tol
+    # substeps with the coupled source, from the oracle's own capped state and table
+    ref = orc.run_coupled(g, p, U, V, Om, m_ref, 4, dt, Mf_ref)
+    assert p1_density(out, ref) <= tol, name
+    assert name.startswith("generic<") or name.startswith("rk2_generic<"), name
+
+
+def test_free_motor_option_and_errors():
+    from paper_1908_04279_b200 import MM, MMError, binding as b
+    g = Grid(4, 4, 4, 6, 8, 8)
+    p = Params()
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    mm = MM(g, p, "f64")
+    mm.set_density(m0); mm.set_filament_velocity(U, V, Om)
+    with pytest.raises(MMError):
+        mm.update_free_motors()                       # psi missing
+    with pytest.raises(MMError):
+        mm.set_option(b.MM_OPT_FREE_COUPLING, 1)     # no table yet
+    mm.set_psi(np.zeros(g.nc))                        # nothing bound counts: M_f = M_total everywhere
+    Mf = np.empty((4, 4))
+    mm.update_free_motors(None, Mf)
+    assert np.array_equal(Mf, np.full((4, 4), p.m_free))
+    dt = mi.benchmark_dt(g, p, 1.0)
+    mm.substep(3, dt)
+    a = np.empty_like(m0); mm.get_density(a)
+    assert p1_density(a, orc.run(g, p, U, V, Om, m0, 3, dt)) < 1e-12      # uniform table == constant source
+    with pytest.raises(MMError):
+        mm.advance_local(dt, 0.4)                     # not with the coupled source
+    mm.set_option(b.MM_OPT_FREE_COUPLING, 0)          # back to the fast path
+    mm.substep(1, dt)
+    assert mm.kernel_name.startswith("coef<")
+    mm.destroy()
