@@ -337,6 +337,32 @@ def run_cuda(args):
                        "point_forces_per_call": g.nc * g.ns, "atomic_adds_per_call": g.nc * g.ns * 32,
                        "grid": [g.nx, g.ny]}
 
+    # ---- optional: NEXT-2 free-motor coupling (macro cadence; outside the timed region; needs two buffers)
+    free_info = None
+    if args.free:
+        psi = torch.rand(g.nc, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(7))
+        mm.set_psi(psi)
+        Mf = torch.empty((g.nx, g.ny), dtype=torch.float64, device=dev)
+        mm.update_free_motors(None, Mf)
+        torch.cuda.synchronize()
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record(stream)
+        for _ in range(2):
+            mm.update_free_motors(None, Mf)
+        e1.record(stream)
+        mm.substep(w.moments_every, w.dt)        # warm-up of the coupled-source kernels
+        e1b = torch.cuda.Event(enable_timing=True)
+        e1b.record(stream)
+        mm.substep(2 * w.moments_every, w.dt)
+        e2.record(stream)
+        torch.cuda.synchronize()
+        cname = mm.kernel_name
+        free_info = {"update_ms_per_call": round(e0.elapsed_time(e1) / 2, 3), "atomic_adds_per_call": g.cells,
+                     "coupled_substep_kernel": cname,
+                     "coupled_substep_gcups": round(g.cells * 2 * w.moments_every / (e1b.elapsed_time(e2) * 1e-3) / 1e9, 2),
+                     "Mf_min": float(Mf.min().item()), "Mf_max": float(Mf.max().item())}
+        mm.set_option(b.MM_OPT_FREE_COUPLING, 0)
+
     # ---- end to end: pinned host (U,V,Omega) in, moments out to pinned host, every step
     for _ in range(2):
         step(Up, Vp, Op, Fp, Tp)
@@ -358,6 +384,8 @@ def run_cuda(args):
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "impl": "cuda"}
     if spread_info:
         out["spread_force"] = spread_info
+    if free_info:
+        out["free_motors"] = free_info
     if local_info:
         out["config"]["workload"] += "+local_dt"
         out["local_dt"] = local_info
@@ -465,6 +493,8 @@ def main():
     ap.add_argument("--single-buffer", action="store_true",
                     help="create the context with ONE density buffer: every pass in place (MM_OPT_INPLACE), half the memory")
     ap.add_argument("--nx-mult", type=int, default=1, help="multiply the workload's Nx (a larger problem of the same structure)")
+    ap.add_argument("--free", action="store_true",
+                    help="NEXT-2: also time mm_update_free_motors and two substeps with the coupled source k_on M_f(r0)")
     ap.add_argument("--spread", action="store_true",
                     help="NEXT-4: also time mm_spread_force (motor-force spreading, Eq. 10) on the final density")
     ap.add_argument("--cfl", type=float, default=0.4, help="CFL number of --local-dt")

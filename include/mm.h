@@ -170,8 +170,8 @@ mm_status mm_spread_force(mm_ctx *ctx, double *F2, int dst_on_device);
  * where M_b,coarse[n] > M_total every cell of node n is scaled by M_total / M_b,coarse[n] (the density IS modified) and
  * M_b,coarse[n] = M_total; M_f[n] = M_total - M_b,coarse[n] >= 0.  The call stores M_f and switches the source of the
  * following substeps to k_on M_f(r0) 1_disc (MM_OPT_FREE_COUPLING), frozen until the next call.  With the coupled
- * source mm_substep runs the generic kernels (two density buffers; MM_OPT_KERNEL 0 or 1) and mm_advance_local is
- * refused.  Mb_coarse, M_free: [nx][ny] fp64 outputs, either may be NULL.  Needs mm_set_psi.  fp64 atomic adds: the
+ * source mm_substep runs the coefficient-form kernels (forward Euler on 16x16 / 8x8 offset planes) or the generic
+ * kernels (any grid, RK2 + Superbee; two density buffers); mm_advance_local is refused.  Mb_coarse, M_free: [nx][ny] fp64 outputs, either may be NULL.  Needs mm_set_psi.  fp64 atomic adds: the
  * summation order varies from call to call. */
 mm_status mm_update_free_motors(mm_ctx *ctx, double *Mb_coarse, double *M_free, int dst_on_device);
 

@@ -214,8 +214,8 @@ static mm_status launch_stream(mm_ctx *c, int T, bool mom, double dt, const void
 #define MM_COEF_MINB_F64 2
 #endif
 
-template <typename real, int NXI, int NETA, int CB, int T, bool MOM>
-static mm_status launch_coef_inst(mm_ctx *c, double dt, const void *in, void *out)
+template <typename real, int NXI, int NETA, int CB, int T, bool MOM, bool MF>
+static mm_status launch_coef_inst_mf(mm_ctx *c, double dt, const void *in, void *out)
 {
     constexpr int P = sizeof(real) == 8 ? MM_COEF_P_F64 : MM_COEF_P_F32;
     constexpr int D = sizeof(real) == 8 ? MM_COEF_D_F64 : MM_COEF_D_F32, WARPS = MM_COEF_WARPS;
@@ -223,7 +223,7 @@ static mm_status launch_coef_inst(mm_ctx *c, double dt, const void *in, void *ou
     constexpr bool PM = sizeof(real) == 8;   // post-mask: fp64 only
     constexpr bool CS = sizeof(real) == 8;   // per-configuration constants in shared memory: fp64 only
     using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
-    auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB, PM, CS>;
+    auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB, PM, CS, false, MF>;
     static int blocks_per_sm = 0;
     if (blocks_per_sm == 0) {
         CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
@@ -240,9 +240,16 @@ static mm_status launch_coef_inst(mm_ctx *c, double dt, const void *in, void *ou
                                                                       c->mom_torque, nullptr, nullptr, 0, nullptr, nullptr);
     CUDA_TRY(c, cudaGetLastError());
     c->launches++;
-    snprintf(c->kname, sizeof c->kname, "coef<%s,%dx%d,CB=%d,T=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
+    snprintf(c->kname, sizeof c->kname, MF ? "coef_mf<%s,%dx%d,CB=%d,T=%d%s>" : "coef<%s,%dx%d,CB=%d,T=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
              CB, T, MOM ? ",mom" : "");
     return MM_OK;
+}
+
+template <typename real, int NXI, int NETA, int CB, int T, bool MOM>
+static mm_status launch_coef_inst(mm_ctx *c, double dt, const void *in, void *out)
+{
+    return c->coupled ? launch_coef_inst_mf<real, NXI, NETA, CB, T, MOM, true>(c, dt, in, out)
+                      : launch_coef_inst_mf<real, NXI, NETA, CB, T, MOM, false>(c, dt, in, out);
 }
 
 template <typename real, int NXI, int NETA, int CB>
@@ -714,9 +721,9 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
     // kernel choice: 0 auto (coefficient form when the grid/flags are supported; else generic),
     // 1 generic, 2 warp-streamed (1-D TMA), 3 tile, 4 coefficient form (same grids/flags as 2)
     int kind = c->opt_kernel;
-    if (kind == 0) kind = (stream_supported(c) && !c->coupled) ? 4 : 1;
-    if (c->coupled && kind != 1)
-        return fail(c, MM_ERR_INVALID_ARG, "the free-motor coupled source runs on the generic kernels (MM_OPT_KERNEL 0 or 1)");
+    if (kind == 0) kind = stream_supported(c) ? 4 : 1;
+    if (c->coupled && kind != 1 && kind != 4)
+        return fail(c, MM_ERR_INVALID_ARG, "the free-motor coupled source runs on the coefficient-form or generic kernels (MM_OPT_KERNEL 0, 1 or 4)");
     if (c->single && !(kind == 4 && stream_supported(c)))
         return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context runs only the in-place coefficient-form / fused RK2 kernels (16x16 or 8x8 offset planes, no test flags)");
     if (kind == 2 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "streamed kernel does not support this grid/flags");

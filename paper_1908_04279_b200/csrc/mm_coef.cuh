@@ -75,6 +75,11 @@ struct CoefCfg {
     static constexpr size_t SMEM_BYTES = TABLE_BYTES + WARPS * WARP_BYTES + (size_t)WARPS * D * sizeof(uint64_t);
 };
 
+// MF (free-motor coupling): the source of a cell is dt k_on M_f at the nearest node to its anchor
+// r0 = x_c + s_j p_c - (xi_a, eta_b) instead of the constant dt k_on m_free.  The node index separates -- its x part
+// depends on (j, a) only, its y part on (j, b) -- so a lane computes QA + CB node coordinates per plane, in fp64 with
+// every operation rounded separately exactly as the oracle does (ties), and gathers its 8 table entries (the table
+// is 128 KB at most and lives in L1/L2); the gathered sources are level-independent like the other coefficients.
 // LOC (mm_advance_local): every configuration takes its own local step dt_c and only the
 // levels it still owes this pass (n_steps[c] - done, clamped to 0..T); `kp` then carries the factors per unit dt and
 // they are scaled by dt_c once per configuration.  A LOC pass runs IN PLACE (in == out): plane j of the output
@@ -83,7 +88,7 @@ struct CoefCfg {
 // unfinished; NULL = all) and the finished ones cost no traffic.  With MOM the moments of a configuration are
 // written in the pass in which it finishes.
 template <typename real, int NXI, int NETA, int CB, int T, bool MOM, int P, int D, int WARPS, int MINB, bool PM, bool CS,
-          bool LOC = false>
+          bool LOC = false, bool MF = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
     substep_coef_kernel(const __grid_constant__ KParams<real> kp, const real *__restrict__ in, real *__restrict__ out,
                         double *__restrict__ force, double *__restrict__ torque,
@@ -142,6 +147,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     real dtc = real(1), dsrc = kp.dt_src;   // LOC: this configuration's local step and source increment
     int nlev = T;                           // LOC: levels this configuration takes in this pass
     bool last_pass = true;                  // LOC: the configuration finishes in this pass (moments are due)
+    double mf_tx = 0, mf_ty = 0, mf_ct = 0, mf_st = 0;   // MF: x_c in units of the domain, cos/sin(theta) in fp64
 
     const int ns = kp.ns;
     const int64_t inner = (int64_t)ns * PLANE;
@@ -186,6 +192,14 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             ct = kp.cos_t[kth];
             st = kp.sin_t[kth];
             const real U = kp.U[c], Vv = kp.V[c], Om = kp.Om[c];
+            if (MF) {
+                const double theta = 2.0 * 3.14159265358979323846264338327950288 * (double)kth / (double)kp.ntheta;
+                mf_ct = cos(theta);
+                mf_st = sin(theta);
+                const int iy = (int)((c / kp.ntheta) % kp.ny), ix = (int)(c / ((int64_t)kp.ntheta * kp.ny));
+                mf_tx = __ddiv_rn((double)ix, (double)kp.nx);
+                mf_ty = __ddiv_rn((double)iy, (double)kp.ny);
+            }
             if (LOC) {
                 dtc = dt_c[c];
                 const int owed = n_steps[c] - done;
@@ -259,6 +273,35 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             // re-zeroed at the next configuration.
             const bool live = j < ns;
             const real sj = kp.s_lo + (real(j) + real(0.5)) * kp.ds;
+            if constexpr (MF) {
+                const double sjd = __dadd_rn(kp.geo_s_lo, __dmul_rn(j + 0.5, kp.geo_ds));
+                const double hx_ = __dadd_rn(mf_tx, __dmul_rn(sjd, mf_ct)), hy_ = __dadd_rn(mf_ty, __dmul_rn(sjd, mf_st));
+                int nodx[QA], nody[CB];
+#pragma unroll
+                for (int q = 0; q < QA; ++q) {
+                    const double xid = __dadd_rn(-kp.geo_R, __dmul_rn(a0 + q + 0.5, kp.geo_dxi));
+                    // floor(r + 1/2) wrapped into [0, nx): the loops run 0-1 times (64-bit % would cost more than the plane)
+                    int n = __double2int_rd(__dadd_rn(__dmul_rn(__dsub_rn(hx_, xid), (double)kp.nx), 0.5));
+                    while (n < 0) n += kp.nx;
+                    while (n >= kp.nx) n -= kp.nx;
+                    nodx[q] = n * kp.ny;
+                }
+#pragma unroll
+                for (int cb = 0; cb < CB; ++cb) {
+                    const double etd = __dadd_rn(-kp.geo_R, __dmul_rn(b0 + cb + 0.5, kp.geo_deta));
+                    int n = __double2int_rd(__dadd_rn(__dmul_rn(__dsub_rn(hy_, etd), (double)kp.ny), 0.5));
+                    while (n < 0) n += kp.ny;
+                    while (n >= kp.ny) n -= kp.ny;
+                    nody[cb] = n;
+                }
+#pragma unroll
+                for (int q = 0; q < QA; ++q)
+#pragma unroll
+                    for (int cb = 0; cb < CB; ++cb) {
+                        const real sv = kp.dt_kon * (real)kp.Mf[nodx[q] + nody[cb]];
+                        srcm[q][cb] = PM ? sv : maskf[q][cb] * sv;
+                    }
+            }
             // ---- level-independent coefficients of this plane
             real c0j[QA][CB], cxm[QA][CB], cxp[QA][CB], cem[QA][CB], cep[QA][CB];
             {
@@ -426,7 +469,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
 #pragma unroll
                     for (int q = 0; q < QA; ++q)
 #pragma unroll
-                        for (int cb = 0; cb < CB; ++cb) nx[q][cb] = ofma(csm[q][cb], R[lv][q][cb], PM ? dsrc : srcm[q][cb]);
+                        for (int cb = 0; cb < CB; ++cb) nx[q][cb] = ofma(csm[q][cb], R[lv][q][cb], (PM && !MF) ? dsrc : srcm[q][cb]);
 #pragma unroll
                     for (int q = 0; q < QA; ++q)
 #pragma unroll
@@ -459,7 +502,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 for (int q = 0; q < QA; ++q)
 #pragma unroll
                     for (int cb = 0; cb < CB; ++cb) {
-                        real acc = fma(c0j[q][cb], x[q][cb], PM ? dsrc : srcm[q][cb]);
+                        real acc = fma(c0j[q][cb], x[q][cb], (PM && !MF) ? dsrc : srcm[q][cb]);
                         if (q > 0) acc = fma(cxm[q][cb], x[q - 1][cb], acc);
                         if (q + 1 < QA) acc = fma(cxp[q][cb], x[q + 1][cb], acc);
                         if (cb > 0) acc = fma(cem[q][cb], x[q][cb - 1], acc);

@@ -14,9 +14,10 @@ pytestmark = pytest.mark.gpu
 RNG = np.random.default_rng(2024)
 
 
-def gpu_coupled(g, p, dtype, U, V, Om, m0, psi, n_sub, dt):
+def gpu_coupled(g, p, dtype, U, V, Om, m0, psi, n_sub, dt, kernel=0):
     from paper_1908_04279_b200 import MM, binding as b
     mm = MM(g, p, dtype)
+    mm.set_option(b.MM_OPT_KERNEL, kernel)
     mm.set_density(np.ascontiguousarray(m0, NPDT[dtype]))
     mm.set_filament_velocity(*(np.ascontiguousarray(x, NPDT[dtype]) for x in (U, V, Om)))
     mm.set_psi(np.ascontiguousarray(psi, np.float64))
@@ -35,8 +36,9 @@ def gpu_coupled(g, p, dtype, U, V, Om, m0, psi, n_sub, dt):
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("flags", [0, mi.FLAG_RK2_SUPERBEE])
-@pytest.mark.parametrize("shape", [(6, 6, 8, 6, 16, 16), (5, 4, 4, 5, 6, 6), (8, 8, 4, 6, 8, 8)])
-def test_free_motor_coupling_parity(dtype, flags, shape):
+@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("shape", [(6, 6, 8, 7, 16, 16), (5, 4, 4, 5, 6, 6), (8, 8, 4, 6, 8, 8)])
+def test_free_motor_coupling_parity(dtype, flags, shape, kernel):
     g = Grid(*shape)
     big = Params(flags=flags, m_free=1e9)
     U, V, Om, m0 = random_inputs(g, big, dtype)
@@ -44,16 +46,17 @@ def test_free_motor_coupling_parity(dtype, flags, shape):
     _, raw, _ = orc.free_motors(g, big, m0, psi)
     p = dataclasses.replace(big, m_free=float(np.median(raw)))      # half of the nodes get capped
     dt = mi.benchmark_dt(g, p, 1.0)
-    Mbc, Mf, capped, out, name = gpu_coupled(g, p, dtype, U, V, Om, m0, psi, 4, dt)
+    Mbc, Mf, capped, out, name = gpu_coupled(g, p, dtype, U, V, Om, m0, psi, 7, dt, kernel)
     m_ref, Mbc_ref, Mf_ref = orc.free_motors(g, p, m0, psi)
     tol = TOL[dtype]
     assert np.max(np.abs(Mbc - Mbc_ref)) / p.m_free <= tol and np.max(np.abs(Mf - Mf_ref)) / p.m_free <= tol
     assert (Mf >= 0).all() and (Mbc <= p.m_free).all()
     assert p1_density(capped, m_ref) <= tol
     # substeps with the coupled source, from the oracle's own capped state and table
-    ref = orc.run_coupled(g, p, U, V, Om, m_ref, 4, dt, Mf_ref)
+    ref = orc.run_coupled(g, p, U, V, Om, m_ref, 7, dt, Mf_ref)
     assert p1_density(out, ref) <= tol, name
-    assert name.startswith("generic<") or name.startswith("rk2_generic<"), name
+    fast = kernel == 0 and flags == 0 and shape[4] in (8, 16)
+    assert name.startswith("coef_mf<" if fast else ("rk2_generic<" if flags else "generic<")), name
 
 
 def test_free_motor_option_and_errors():
@@ -75,6 +78,7 @@ def test_free_motor_option_and_errors():
     mm.substep(3, dt)
     a = np.empty_like(m0); mm.get_density(a)
     assert p1_density(a, orc.run(g, p, U, V, Om, m0, 3, dt)) < 1e-12      # uniform table == constant source
+    assert mm.kernel_name.startswith("coef_mf<")
     with pytest.raises(MMError):
         mm.advance_local(dt, 0.4)                     # not with the coupled source
     mm.set_option(b.MM_OPT_FREE_COUPLING, 0)          # back to the fast path
