@@ -29,7 +29,7 @@ def test_reference_arm_line():
 
 @pytest.mark.gpu
 def test_cuda_arm_line_and_option_legs():
-    d = run_bench("--config", "0", "--steps", "2", "--warmup", "3", "--cpu-seconds", "1", "--spread")
+    d = run_bench("--config", "0", "--steps", "2", "--warmup", "3", "--cpu-seconds", "1", "--spread", "--free")
     for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
               "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
         assert k in d, k
@@ -41,6 +41,7 @@ def test_cuda_arm_line_and_option_legs():
     assert r["kernel"].startswith("coef<") and "traffic" in r
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] > 0
     assert d["spread_force"]["ms_per_call"] > 0
+    assert d["free_motors"]["update_ms_per_call"] > 0 and d["free_motors"]["coupled_substep_kernel"].startswith("coef_mf<")
     d = run_bench("--config", "0", "--steps", "1", "--warmup", "1", "--no-cpu", "--no-t1", "--scheme", "rk2")
     assert d["roofline"]["kernel"].startswith("rk2_fused<") and d["config"]["workload"].endswith("+rk2_superbee")
     d = run_bench("--config", "0", "--steps", "1", "--warmup", "1", "--no-cpu", "--local-dt")
