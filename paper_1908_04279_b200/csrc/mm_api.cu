@@ -224,20 +224,25 @@ static mm_status launch_coef_inst_mf(mm_ctx *c, double dt, const void *in, void 
     constexpr bool CS = sizeof(real) == 8;   // per-configuration constants in shared memory: fp64 only
     using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
     auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB, PM, CS, false, MF>;
+    // MF: the warps' node tables (16-bit, ns * (NXI + NETA) entries each) sit behind the regular layout
+    const size_t smem = MF ? ((Cfg::SMEM_BYTES + 15) / 16) * 16 + (size_t)WARPS * c->g.ns * (NXI + NETA) * 2 : Cfg::SMEM_BYTES;
     static int blocks_per_sm = 0;
-    if (blocks_per_sm == 0) {
-        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
+    static size_t smem_set = 0;
+    if (blocks_per_sm == 0 || smem != smem_set) {
+        if (smem > 227 * 1024) return fail(c, MM_ERR_INVALID_ARG, "ns too large for the coupled coefficient-form kernel");
+        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int n = 0;
-        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, Cfg::SMEM_BYTES));
+        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, smem));
         if (n < 1) return fail(c, MM_ERR_CUDA, "coefficient-form kernel does not fit on an SM");
         blocks_per_sm = n;
+        smem_set = smem;
     }
     int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
     const int64_t need = (c->nc + WARPS - 1) / WARPS;
     if (grid > need) grid = need;
     KParams<real> kp = make_kparams<real>(c, dt);
-    kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(kp, (const real *)in, (real *)out, c->mom_force,
-                                                                      c->mom_torque, nullptr, nullptr, 0, nullptr, nullptr);
+    kern<<<(unsigned)grid, WARPS * 32, smem, c->stream>>>(kp, (const real *)in, (real *)out, c->mom_force, c->mom_torque,
+                                                           nullptr, nullptr, 0, nullptr, nullptr);
     CUDA_TRY(c, cudaGetLastError());
     c->launches++;
     snprintf(c->kname, sizeof c->kname, MF ? "coef_mf<%s,%dx%d,CB=%d,T=%d%s>" : "coef<%s,%dx%d,CB=%d,T=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
@@ -721,7 +726,9 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
     // kernel choice: 0 auto (coefficient form when the grid/flags are supported; else generic),
     // 1 generic, 2 warp-streamed (1-D TMA), 3 tile, 4 coefficient form (same grids/flags as 2)
     int kind = c->opt_kernel;
-    if (kind == 0) kind = stream_supported(c) ? 4 : 1;
+    if (kind == 0) kind = (stream_supported(c) && !(c->coupled && (c->g.nx > 32767 || c->g.ny > 32767))) ? 4 : 1;
+    if (c->coupled && kind == 4 && (c->g.nx > 32767 || c->g.ny > 32767))
+        return fail(c, MM_ERR_INVALID_ARG, "the coupled coefficient-form kernel needs nx, ny <= 32767");
     if (c->coupled && kind != 1 && kind != 4)
         return fail(c, MM_ERR_INVALID_ARG, "the free-motor coupled source runs on the coefficient-form or generic kernels (MM_OPT_KERNEL 0, 1 or 4)");
     if (c->single && !(kind == 4 && stream_supported(c)))

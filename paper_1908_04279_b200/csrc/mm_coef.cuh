@@ -51,6 +51,16 @@ __device__ __forceinline__ float ofma(float a, float b, float c)
     return d;
 }
 __device__ __forceinline__ double ofma(double a, double b, double c) { return fma(a, b, c); }
+// floor(r) wrapped into [0, n) without branches or integer division (branches inside the unrolled planes would cost
+// the shuffles their convergence guarantee): quotient estimate in fp64, exact remainder, one corrective step each way
+__device__ __forceinline__ int wrap_node(double r, int n)
+{
+    const double f = floor(r), q = floor(f * (1.0 / (double)n));
+    int m = __double2int_rn(f - q * (double)n);   // exact: |f| < 2^31, q n is an integer near f
+    m += m < 0 ? n : 0;
+    m -= m >= n ? n : 0;
+    return m;
+}
 __device__ __forceinline__ float rabs(float x) { return fabsf(x); }
 __device__ __forceinline__ double rabs(double x) { return fabs(x); }
 
@@ -77,9 +87,11 @@ struct CoefCfg {
 
 // MF (free-motor coupling): the source of a cell is dt k_on M_f at the nearest node to its anchor
 // r0 = x_c + s_j p_c - (xi_a, eta_b) instead of the constant dt k_on m_free.  The node index separates -- its x part
-// depends on (j, a) only, its y part on (j, b) -- so a lane computes QA + CB node coordinates per plane, in fp64 with
-// every operation rounded separately exactly as the oracle does (ties), and gathers its 8 table entries (the table
-// is 128 KB at most and lives in L1/L2); the gathered sources are level-independent like the other coefficients.
+// depends on (j, a) only, its y part on (j, b) -- so at the start of a configuration the warp fills two small
+// shared-memory tables, node_x[j][a] and node_y[j][b] (16-bit; Ns (Nxi + Neta) entries, 64 per lane), in fp64 with every
+// operation rounded separately exactly as the oracle does (ties); per plane a lane then reads its QA + CB entries and
+// gathers its 8 values of M_f (the table is 128 KB at most and lives in L1/L2).  The gathered sources are
+// level-independent like the other coefficients.  Needs nx, ny <= 32767 (host-checked).
 // LOC (mm_advance_local): every configuration takes its own local step dt_c and only the
 // levels it still owes this pass (n_steps[c] - done, clamped to 0..T); `kp` then carries the factors per unit dt and
 // they are scaled by dt_c once per configuration.  A LOC pass runs IN PLACE (in == out): plane j of the output
@@ -147,7 +159,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     real dtc = real(1), dsrc = kp.dt_src;   // LOC: this configuration's local step and source increment
     int nlev = T;                           // LOC: levels this configuration takes in this pass
     bool last_pass = true;                  // LOC: the configuration finishes in this pass (moments are due)
-    double mf_tx = 0, mf_ty = 0, mf_ct = 0, mf_st = 0;   // MF: x_c in units of the domain, cos/sin(theta) in fp64
+    // MF: this warp's node tables, behind the regular shared-memory layout (host adds WARPS * ns * (NXI + NETA) * 2 bytes)
+    unsigned short *nod = reinterpret_cast<unsigned short *>(smem_raw + ((Cfg::SMEM_BYTES + 15) / 16) * 16) +
+                          (size_t)warp * kp.ns * (NXI + NETA);
 
     const int ns = kp.ns;
     const int64_t inner = (int64_t)ns * PLANE;
@@ -194,11 +208,26 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             const real U = kp.U[c], Vv = kp.V[c], Om = kp.Om[c];
             if (MF) {
                 const double theta = 2.0 * 3.14159265358979323846264338327950288 * (double)kth / (double)kp.ntheta;
-                mf_ct = cos(theta);
-                mf_st = sin(theta);
+                const double mf_ct = cos(theta), mf_st = sin(theta);
                 const int iy = (int)((c / kp.ntheta) % kp.ny), ix = (int)(c / ((int64_t)kp.ntheta * kp.ny));
-                mf_tx = __ddiv_rn((double)ix, (double)kp.nx);
-                mf_ty = __ddiv_rn((double)iy, (double)kp.ny);
+                const double mf_tx = __ddiv_rn((double)ix, (double)kp.nx), mf_ty = __ddiv_rn((double)iy, (double)kp.ny);
+                __syncwarp();   // the previous configuration's planes are done with the tables
+                for (int e = lane; e < kp.ns * (NXI + NETA); e += 32) {
+                    const int jj = e / (NXI + NETA), r = e - jj * (NXI + NETA);
+                    const double sjd = __dadd_rn(kp.geo_s_lo, __dmul_rn(jj + 0.5, kp.geo_ds));
+                    int n;
+                    if (r < NXI) {
+                        const double xid = __dadd_rn(-kp.geo_R, __dmul_rn(r + 0.5, kp.geo_dxi));
+                        const double hx_ = __dadd_rn(mf_tx, __dmul_rn(sjd, mf_ct));
+                        n = wrap_node(__dadd_rn(__dmul_rn(__dsub_rn(hx_, xid), (double)kp.nx), 0.5), kp.nx);
+                    } else {
+                        const double etd = __dadd_rn(-kp.geo_R, __dmul_rn(r - NXI + 0.5, kp.geo_deta));
+                        const double hy_ = __dadd_rn(mf_ty, __dmul_rn(sjd, mf_st));
+                        n = wrap_node(__dadd_rn(__dmul_rn(__dsub_rn(hy_, etd), (double)kp.ny), 0.5), kp.ny);
+                    }
+                    nod[e] = (unsigned short)n;
+                }
+                __syncwarp();
             }
             if (LOC) {
                 dtc = dt_c[c];
@@ -274,26 +303,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             const bool live = j < ns;
             const real sj = kp.s_lo + (real(j) + real(0.5)) * kp.ds;
             if constexpr (MF) {
-                const double sjd = __dadd_rn(kp.geo_s_lo, __dmul_rn(j + 0.5, kp.geo_ds));
-                const double hx_ = __dadd_rn(mf_tx, __dmul_rn(sjd, mf_ct)), hy_ = __dadd_rn(mf_ty, __dmul_rn(sjd, mf_st));
+                const unsigned short *nj = nod + (live ? j : 0) * (NXI + NETA);
                 int nodx[QA], nody[CB];
 #pragma unroll
-                for (int q = 0; q < QA; ++q) {
-                    const double xid = __dadd_rn(-kp.geo_R, __dmul_rn(a0 + q + 0.5, kp.geo_dxi));
-                    // floor(r + 1/2) wrapped into [0, nx): the loops run 0-1 times (64-bit % would cost more than the plane)
-                    int n = __double2int_rd(__dadd_rn(__dmul_rn(__dsub_rn(hx_, xid), (double)kp.nx), 0.5));
-                    while (n < 0) n += kp.nx;
-                    while (n >= kp.nx) n -= kp.nx;
-                    nodx[q] = n * kp.ny;
-                }
+                for (int q = 0; q < QA; ++q) nodx[q] = (int)nj[a0 + q] * kp.ny;
 #pragma unroll
-                for (int cb = 0; cb < CB; ++cb) {
-                    const double etd = __dadd_rn(-kp.geo_R, __dmul_rn(b0 + cb + 0.5, kp.geo_deta));
-                    int n = __double2int_rd(__dadd_rn(__dmul_rn(__dsub_rn(hy_, etd), (double)kp.ny), 0.5));
-                    while (n < 0) n += kp.ny;
-                    while (n >= kp.ny) n -= kp.ny;
-                    nody[cb] = n;
-                }
+                for (int cb = 0; cb < CB; ++cb) nody[cb] = (int)nj[NXI + b0 + cb];
 #pragma unroll
                 for (int q = 0; q < QA; ++q)
 #pragma unroll
