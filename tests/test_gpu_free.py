@@ -85,3 +85,47 @@ def test_free_motor_option_and_errors():
     mm.substep(1, dt)
     assert mm.kernel_name.startswith("coef<")
     mm.destroy()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_full_microscale_step_against_the_oracle(dtype):
+    """Alg. 2 on this path, two macro steps in a row: free-motor update (coarse density, cap, M_f), substeps with the
+    coupled source, moments, force spreading -- every output of every stage against the oracle run the same way."""
+    from paper_1908_04279_b200 import MM
+    from util import p2_moments
+    g = Grid(8, 6, 8, 9, 16, 16)
+    big = Params(m_free=1e9)
+    U, V, Om, m0 = random_inputs(g, big, dtype)
+    psi = RNG.random(g.nc) * 25.0
+    _, raw, _ = orc.free_motors(g, big, m0, psi)
+    p = dataclasses.replace(big, m_free=float(np.quantile(raw, 0.7)))
+    dt = mi.benchmark_dt(g, p, 1.0)
+    tol = TOL[dtype]
+    mm = MM(g, p, dtype)
+    mm.set_density(np.ascontiguousarray(m0, NPDT[dtype]))
+    mm.set_psi(psi)
+    ref = np.asarray(m0, np.float64)
+    for step in range(2):
+        Us, Vs, Os = ((1.0 - 0.3 * step) * x for x in (U, V, Om))     # new macroscale velocities every step
+        mm.set_filament_velocity(*(np.ascontiguousarray(x, NPDT[dtype]) for x in (Us, Vs, Os)))
+        Mbc, Mf = np.empty((g.nx, g.ny)), np.empty((g.nx, g.ny))
+        mm.update_free_motors(Mbc, Mf)
+        mm.substep(6, dt)
+        f, t = np.empty((g.nc, 2)), np.empty(g.nc)
+        mm.moments(f, t)
+        F2 = np.empty((g.nx, g.ny, 2))
+        mm.spread_force(F2)
+        out = np.empty((g.nc, g.ns, g.nxi, g.neta), NPDT[dtype])
+        mm.get_density(out)
+        # oracle, same sequence (fp32: from the velocities as stored)
+        Uo, Vo, Oo = (np.asarray(np.asarray(x, NPDT[dtype]), np.float64) for x in (Us, Vs, Os))
+        ref, Mbc_o, Mf_o = orc.free_motors(g, p, ref, psi)
+        ref = orc.run_coupled(g, p, Uo, Vo, Oo, ref, 6, dt, Mf_o)
+        assert np.max(np.abs(Mbc - Mbc_o)) / p.m_free <= tol and np.max(np.abs(Mf - Mf_o)) / p.m_free <= tol, step
+        assert p1_density(out, ref) <= tol, step
+        ef, et = p2_moments(f, t, orc.moments(g, p, ref))
+        assert ef <= tol and et <= tol, step
+        F2_o = orc.spread_force(g, p, ref, psi)
+        assert np.max(np.abs(F2 - F2_o)) / np.max(np.abs(F2_o)) <= tol, step
+    assert mm.kernel_name.startswith("coef_mf<")
+    mm.destroy()
