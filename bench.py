@@ -216,9 +216,16 @@ def run_cuda(args):
 
     sub_events = []   # (start, stop, n_sub) around every mm_substep call of the timed region
 
+    if args.full:   # the whole microscale step of Alg. 2 on this path: NEXT-2 + A0-A4 + NEXT-4
+        psi_full = torch.rand(g.nc, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(7))
+        mm.set_psi(psi_full)
+        F2_full = torch.empty((g.nx, g.ny, 2), dtype=torch.float64, device=dev)
+
     def step(U, V, Om, F, T, record=False):
         mm.set_filament_velocity(U, V, Om)                                  # A0
         for k in range(n_mom):
+            if args.full:
+                mm.update_free_motors(None, None)                           # NEXT-2: M_b,coarse, cap, M_f
             if record:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
@@ -230,6 +237,8 @@ def run_cuda(args):
                 e1.record(stream)
                 sub_events.append((e0, e1, w.moments_every))
             mm.moments(F[k], T[k])                                          # A4
+            if args.full:
+                mm.spread_force(F2_full)                                    # NEXT-4: Eq. 10
 
     def barrier():
         if world > 1:
@@ -386,6 +395,10 @@ def run_cuda(args):
         out["spread_force"] = spread_info
     if free_info:
         out["free_motors"] = free_info
+    if args.full:
+        out["config"]["workload"] += "+full_step"
+        out["full_step"] = {"per_macro_interval": "mm_update_free_motors, mm_substep (coupled source), mm_moments, mm_spread_force",
+                            "note": "value still counts cell-updates of the substeps only; the roofline object refers to the substep kernel"}
     if local_info:
         out["config"]["workload"] += "+local_dt"
         out["local_dt"] = local_info
@@ -493,6 +506,8 @@ def main():
     ap.add_argument("--single-buffer", action="store_true",
                     help="create the context with ONE density buffer: every pass in place (MM_OPT_INPLACE), half the memory")
     ap.add_argument("--nx-mult", type=int, default=1, help="multiply the workload's Nx (a larger problem of the same structure)")
+    ap.add_argument("--full", action="store_true",
+                    help="time the whole microscale step: free-motor update + coupled substeps + moments + force spreading")
     ap.add_argument("--free", action="store_true",
                     help="NEXT-2: also time mm_update_free_motors and two substeps with the coupled source k_on M_f(r0)")
     ap.add_argument("--spread", action="store_true",
