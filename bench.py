@@ -286,7 +286,7 @@ def run_cuda(args):
     fuse_t = 1 if args.scheme == "rk2" else (args.fuse_t or mm.get_option(b.MM_OPT_FUSE_T))
     launches_per_call = -(-w.moments_every // fuse_t)
     if args.local_dt:
-        launches_per_call = -(-local_info["n_c_max"] // b.MM_MAX_FUSE_T)
+        launches_per_call = -(-local_info["n_c_max"] // b.MM_LOCAL_FUSE_T)
     n_launch = launches_per_call * len(sub_events)
     peak, peak_src = measured_peaks()
     alg_bytes = 2.0 * es * g.cells * sub_n                 # 2*sizeof(real) B per cell-update (T=1 count)

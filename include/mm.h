@@ -88,8 +88,9 @@ typedef enum {
                                 flags); 2 force the warp-streamed 1-D-TMA kernels; 3 force the tiled-TMA kernels;
                                 4 force the coefficient-form kernels (the default where supported)
                                 (2, 3, 4: MM_ERR_INVALID_ARG from mm_substep if the grid/flags are unsupported) */
-    MM_OPT_FUSE_T = 1,       /* max substeps fused per HBM pass (temporal fusion), 1..MM_MAX_FUSE_T;
-                                default 4 */
+    MM_OPT_FUSE_T = 1,       /* max substeps fused per HBM pass (temporal fusion), 1..MM_MAX_FUSE_T; mm_substep uses as
+                                few passes as this allows, of balanced depth (10 substeps at depth 6 = 5 + 5);
+                                default 6 (fp32) / 4 (fp64) */
     MM_OPT_FUSE_MOMENTS = 2, /* 1 (default): the last pass of mm_substep also reduces the moments, so a
                                 following mm_moments is a copy; 0: mm_moments always runs its own pass */
     MM_OPT_FREE_COUPLING = 4,/* 1: the source term of the substeps is k_on M_f(r0) from the table of the last
@@ -101,7 +102,8 @@ typedef enum {
                                 buffer is not touched; same results, same speed, half the memory.  Default 0; always 1
                                 for a context created with ONE density buffer (mm_create, dens_buf1 = NULL) */
 } mm_option;
-#define MM_MAX_FUSE_T 4
+#define MM_MAX_FUSE_T 6   /* coefficient-form kernels; the streamed / tiled variants fuse at most 4 */
+#define MM_LOCAL_FUSE_T 4 /* levels per pass of mm_advance_local */
 
 /* Create a context.
  *  grid, params : copied.  Invalid (MM_ERR_INVALID_ARG): any dim < 1, R <= 0, f_stall <= 0,

@@ -269,16 +269,18 @@ static mm_status launch_coef_shape(mm_ctx *c, int T, bool mom, double dt, const 
         MM_CASE(2)
         MM_CASE(3)
         MM_CASE(4)
+        MM_CASE(5)
+        MM_CASE(6)
     }
 #undef MM_CASE
     return fail(c, MM_ERR_INVALID_ARG, "unsupported fuse depth");
 }
 
-// NEXT-3: one pass of the local-step variant (T = MM_MAX_FUSE_T levels at most per configuration)
+// NEXT-3: one pass of the local-step variant (T = MM_LOCAL_FUSE_T levels at most per configuration)
 template <typename real, int NXI, int NETA, int CB, bool MOM>
 static mm_status launch_coef_local_inst(mm_ctx *c, const void *in, void *out, int32_t done, bool use_list)
 {
-    constexpr int T = MM_MAX_FUSE_T;
+    constexpr int T = MM_LOCAL_FUSE_T;
     // 2 planes x 3 slots for both dtypes: the kernel holds T+1 straight-line instances of the chunk body (one per
     // level count), so the chunk is kept short to stay inside the instruction cache
     constexpr int P = 2, D = 3, WARPS = MM_COEF_WARPS;
@@ -572,8 +574,9 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->Mf = c->Mbc = c->free_raw = c->free_factor = nullptr; c->free_any = nullptr; c->coupled = false;
     c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
-    // measured defaults: the coefficient-form kernel, 4 substeps per pass
-    c->opt_kernel = 0; c->opt_fuse_t = 4; c->opt_fuse_mom = 1;
+    // measured defaults: the coefficient-form kernel, at most 6 (fp32) / 4 (fp64)
+    // substeps per pass
+    c->opt_kernel = 0; c->opt_fuse_t = dtype == MM_F64 ? 4 : 6; c->opt_fuse_mom = 1;
     c->single = (b0 != nullptr && b1 == nullptr);
     c->opt_inplace = c->single ? 1 : 0;
     c->checked_dt = NAN; c->launches = 0; c->kname[0] = 0;
@@ -757,7 +760,11 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
             s = c->dtype == MM_F64 ? launch_generic<double>(c, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
                                    : launch_generic<float>(c, dt, c->buf[c->cur], c->buf[c->cur ^ 1]);
         } else {
-            t = remaining < c->opt_fuse_t ? remaining : c->opt_fuse_t;
+            // balanced passes: as few as the fuse depth allows, of equal depth (10 substeps at depth 6 = 5 + 5)
+            int tmax = c->opt_fuse_t;
+            if (kind != 4 && tmax > 4) tmax = 4;   // the streamed / tiled variants are instantiated up to 4
+            const int passes_left = (remaining + tmax - 1) / tmax;
+            t = (remaining + passes_left - 1) / passes_left;
             const bool mom = c->opt_fuse_mom && remaining == t;
             const bool inpl = c->opt_inplace != 0;
             s = kind == 2   ? launch_stream(c, t, mom, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
@@ -812,14 +819,14 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
         // configurations (compact list built on the device); a configuration writes its moments when it finishes.
         // fp64 (measured: in-place is slower there): ping-pong passes over all configurations,
         // finished ones copied through, moments in the last pass.
-        const int32_t passes = (nmax + MM_MAX_FUSE_T - 1) / MM_MAX_FUSE_T;
+        const int32_t passes = (nmax + MM_LOCAL_FUSE_T - 1) / MM_LOCAL_FUSE_T;
         const bool inplace = sizeof(real) == 4 || c->opt_inplace;
         for (int32_t ps = 0; ps < passes; ++ps) {
-            const int32_t done = ps * MM_MAX_FUSE_T;
+            const int32_t done = ps * MM_LOCAL_FUSE_T;
             mm_status s;
             if (inplace) {
                 // moments are only compiled into the passes in which some configuration can finish
-                const bool mom = c->opt_fuse_mom != 0 && nmin <= done + MM_MAX_FUSE_T;
+                const bool mom = c->opt_fuse_mom != 0 && nmin <= done + MM_LOCAL_FUSE_T;
                 if (ps > 0) {
                     CUDA_TRY(c, cudaMemsetAsync(c->loc_count, 0, sizeof(int32_t), c->stream));
                     int64_t lb = (c->nc + 255) / 256;

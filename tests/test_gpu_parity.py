@@ -193,13 +193,13 @@ def test_tile_dirty_masked_input_is_dropped():
 
 # ------------------------------------------------------------------ coefficient-form kernels (mm_coef.cuh)
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("T", [1, 2, 3, 4])
+@pytest.mark.parametrize("T", [1, 2, 3, 4, 5, 6])
 @pytest.mark.parametrize("nxi", [16, 8])
 def test_coef_kernel_parity(dtype, T, nxi):
     # Ns=7: ragged last chunk (P=2); 700 configurations: several per warp
     g = Grid(5, 7, 20, 7, nxi, nxi)
     p = Params()
-    e, info = check_parity(g, p, dtype, [5, 3], _dt(g, p), kernel=4, fuse_t=T)
+    e, info = check_parity(g, p, dtype, [11, 7] if T > 4 else [5, 3], _dt(g, p), kernel=4, fuse_t=T)
     assert info["kernel"].startswith("coef<"), info
 
 
