@@ -222,7 +222,7 @@ static mm_status launch_coef_inst_mf(mm_ctx *c, double dt, const void *in, void 
     constexpr int MINB = sizeof(real) == 8 ? MM_COEF_MINB_F64 : MM_COEF_MINB_F32;
     constexpr bool PM = sizeof(real) == 8;   // post-mask: fp64 only
     constexpr bool CS = sizeof(real) == 8;   // per-configuration constants in shared memory: fp64 only
-    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
+    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS, coef_rs(T)>;
     auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB, PM, CS, false, MF>;
     // MF: the warps' node tables (16-bit, ns * (NXI + NETA) entries each) sit behind the regular layout
     const size_t smem = MF ? ((Cfg::SMEM_BYTES + 15) / 16) * 16 + (size_t)WARPS * c->g.ns * (NXI + NETA) * 2 : Cfg::SMEM_BYTES;
@@ -271,6 +271,14 @@ static mm_status launch_coef_shape(mm_ctx *c, int T, bool mom, double dt, const 
         MM_CASE(4)
         MM_CASE(5)
         MM_CASE(6)
+    }
+    if constexpr (sizeof(real) == 4 && NXI == 16) {   // deeper fusion where it pays: fp32, the BASELINE offset plane
+        switch (T) {
+            MM_CASE(7)
+            MM_CASE(8)
+            MM_CASE(9)
+            MM_CASE(10)
+        }
     }
 #undef MM_CASE
     return fail(c, MM_ERR_INVALID_ARG, "unsupported fuse depth");
@@ -574,9 +582,9 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->Mf = c->Mbc = c->free_raw = c->free_factor = nullptr; c->free_any = nullptr; c->coupled = false;
     c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
-    // measured defaults: the coefficient-form kernel, at most 6 (fp32) / 4 (fp64)
-    // substeps per pass
-    c->opt_kernel = 0; c->opt_fuse_t = dtype == MM_F64 ? 4 : 6; c->opt_fuse_mom = 1;
+    // measured defaults: the coefficient-form kernel, at most 10 (fp32; 6 off the 16x16
+    // offset plane) / 4 (fp64) substeps per pass
+    c->opt_kernel = 0; c->opt_fuse_t = dtype == MM_F64 ? 4 : 10; c->opt_fuse_mom = 1;
     c->single = (b0 != nullptr && b1 == nullptr);
     c->opt_inplace = c->single ? 1 : 0;
     c->checked_dt = NAN; c->launches = 0; c->kname[0] = 0;
@@ -763,6 +771,7 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
             // balanced passes: as few as the fuse depth allows, of equal depth (10 substeps at depth 6 = 5 + 5)
             int tmax = c->opt_fuse_t;
             if (kind != 4 && tmax > 4) tmax = 4;   // the streamed / tiled variants are instantiated up to 4
+            if (kind == 4 && tmax > 6 && !(c->dtype == MM_F32 && c->g.nxi == 16)) tmax = 6;   // depth 7-10: fp32 16x16 only
             const int passes_left = (remaining + tmax - 1) / tmax;
             t = (remaining + passes_left - 1) / passes_left;
             const bool mom = c->opt_fuse_mom && remaining == t;

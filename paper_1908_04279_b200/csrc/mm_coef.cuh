@@ -64,7 +64,12 @@ __device__ __forceinline__ int wrap_node(double r, int n)
 __device__ __forceinline__ float rabs(float x) { return fabsf(x); }
 __device__ __forceinline__ double rabs(double x) { return fabs(x); }
 
-template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, bool CS>
+#ifndef MM_COEF_RREG
+#define MM_COEF_RREG 6   // fuse levels whose upwind plane stays in registers; deeper levels keep it in shared memory
+#endif
+__host__ __device__ constexpr int coef_rs(int T) { return T > MM_COEF_RREG ? T - MM_COEF_RREG : 0; }
+
+template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, bool CS, int RS = 0>
 struct CoefCfg {
     static constexpr int LB = NETA / CB;       // lanes per patch row
     static constexpr int G = 32 / LB;          // patch rows per plane
@@ -81,7 +86,10 @@ struct CoefCfg {
     static constexpr int NK = (QA + 1) * CB + QA * (CB + 1) + QA * CB;   // constants per lane
     static constexpr int NKV = (NK + VW - 1) / VW;                       // ... in vectors
     static constexpr size_t CST_BYTES = CS ? (size_t)NKV * 32 * VW * sizeof(real) : 0;
-    static constexpr size_t WARP_BYTES = RING_BYTES + CST_BYTES;
+    // RS: levels beyond the register budget keep their upwind plane (plane j-1 at that level) in a warp-private block,
+    // [level][row][vector][lane] -- lane-private slots, 128-bit and conflict-free, no synchronisation needed
+    static constexpr size_t RSM_BYTES = (size_t)RS * PLANE * sizeof(real);
+    static constexpr size_t WARP_BYTES = RING_BYTES + CST_BYTES + RSM_BYTES;
     static constexpr size_t SMEM_BYTES = TABLE_BYTES + WARPS * WARP_BYTES + (size_t)WARPS * D * sizeof(uint64_t);
 };
 
@@ -108,7 +116,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                         int32_t done = 0, const int32_t *__restrict__ list = nullptr,
                         const int32_t *__restrict__ list_count = nullptr)
 {
-    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
+    constexpr int RS = coef_rs(T), TR = T - RS;   // levels with the upwind plane in shared memory / in registers
+    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS, RS>;
     constexpr int LB = Cfg::LB, G = Cfg::G, QA = Cfg::QA, PLANE = Cfg::PLANE, NK = Cfg::NK, NKV = Cfg::NKV;
     constexpr int VW = Cfg::VW;
     constexpr bool XS = MM_COEF_XSTATIONARY != 0;   // operand-reuse-friendly order of the level update
@@ -122,6 +131,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     real *ring = reinterpret_cast<real *>(smem_raw + Cfg::TABLE_BYTES + (size_t)warp * Cfg::WARP_BYTES);
     real *cst = ring + Cfg::RING_BYTES / sizeof(real) + lane * VW;   // this lane's column of the constants block
+    real *rsm = ring + (Cfg::RING_BYTES + Cfg::CST_BYTES) / sizeof(real) + lane * VW;   // ... of the upwind-plane block
     uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + Cfg::TABLE_BYTES + (size_t)WARPS * Cfg::WARP_BYTES) +
                      warp * D;
 
@@ -193,7 +203,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     real kc[NKV * VW];
     real csm[QA][CB];       // mask dt W/ds                                                            (S5, s flux)
     real hbx = 0, hbe = 0, ct = 0, st = 0;
-    real R[T][QA][CB];      // plane j-1 at levels n .. n+T-1
+    real R[TR][QA][CB];     // plane j-1 at levels n .. n+TR-1 (levels TR .. T-1: in shared memory, rsm)
+    auto rsm_at = [&](int lv, int q, int v4) { return rsm + (((lv - TR) * QA + q) * (CB / VW) + v4) * 32 * VW; };
     real FX = 0, FY = 0, TQ = 0;
 
     int64_t k = 0, c = 0;
@@ -280,9 +291,20 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
 #pragma unroll
             for (int lv = 0; lv < T; ++lv)
 #pragma unroll
-                for (int q = 0; q < QA; ++q)
+                for (int q = 0; q < QA; ++q) {
+                    if (lv < TR) {
 #pragma unroll
-                    for (int cb = 0; cb < CB; ++cb) R[lv][q][cb] = real(0);   // zero inflow at s_lo (S5)
+                        for (int cb = 0; cb < CB; ++cb) R[lv < TR ? lv : 0][q][cb] = real(0);   // zero inflow at s_lo (S5)
+                    } else {
+#pragma unroll
+                        for (int v4 = 0; v4 < CB / VW; ++v4) {
+                            V128 z;
+#pragma unroll
+                            for (int e = 0; e < VW; ++e) z.v[e] = real(0);
+                            *reinterpret_cast<V128 *>(rsm_at(lv, q, v4)) = z;
+                        }
+                    }
+                }
             FX = FY = TQ = real(0);
         }
 
@@ -439,6 +461,21 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 }
 #pragma unroll
             for (int lv = 0; lv < NL; ++lv) {
+                real Rl[QA][CB];   // plane j-1 at this level
+#pragma unroll
+                for (int q = 0; q < QA; ++q) {
+                    if (lv < TR) {
+#pragma unroll
+                        for (int cb = 0; cb < CB; ++cb) Rl[q][cb] = R[lv < TR ? lv : 0][q][cb];
+                    } else {
+#pragma unroll
+                        for (int v4 = 0; v4 < CB / VW; ++v4) {
+                            const V128 t = *reinterpret_cast<const V128 *>(rsm_at(lv, q, v4));
+#pragma unroll
+                            for (int e = 0; e < VW; ++e) Rl[q][v4 * VW + e] = t.v[e];
+                        }
+                    }
+                }
                 real up[CB], dn[CB], lf[QA], rt[QA];
 #pragma unroll
                 for (int cb = 0; cb < CB; ++cb) {
@@ -472,7 +509,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                             acc.y = fmaf(cem[q][e1], x[q][e0], acc.y);
                             acc.x = fmaf(cep[q][e0], x[q][e1], acc.x);
                             acc.y = fmaf(cep[q][e1], e1 + 1 < CB ? x[q][e1 + 1 < CB ? e1 + 1 : 0] : rt[q], acc.y);
-                            acc = __ffma2_rn(make_float2(csm[q][e0], csm[q][e1]), make_float2(R[lv][q][e0], R[lv][q][e1]), acc);
+                            acc = __ffma2_rn(make_float2(csm[q][e0], csm[q][e1]), make_float2(Rl[q][e0], Rl[q][e1]), acc);
                             nx[q][e0] = acc.x;
                             nx[q][e1] = acc.y;
                         }
@@ -484,7 +521,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
 #pragma unroll
                     for (int q = 0; q < QA; ++q)
 #pragma unroll
-                        for (int cb = 0; cb < CB; ++cb) nx[q][cb] = ofma(csm[q][cb], R[lv][q][cb], (PM && !MF) ? dsrc : srcm[q][cb]);
+                        for (int cb = 0; cb < CB; ++cb) nx[q][cb] = ofma(csm[q][cb], Rl[q][cb], (PM && !MF) ? dsrc : srcm[q][cb]);
 #pragma unroll
                     for (int q = 0; q < QA; ++q)
 #pragma unroll
@@ -526,18 +563,28 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                         if (q + 1 == QA) acc = fma(cxp[q][cb], up[cb], acc);
                         if (cb == 0) acc = fma(cem[q][cb], lf[q], acc);
                         if (cb + 1 == CB) acc = fma(cep[q][cb], rt[q], acc);
-                        acc = fma(csm[q][cb], R[lv][q][cb], acc);   // last: the result may reuse R's register
+                        acc = fma(csm[q][cb], Rl[q][cb], acc);   // last: the result may reuse R's register
                         nx[q][cb] = PM ? and_mask(acc, maskw[q][cb]) : acc;
                     }
                 }
                 }
 #pragma unroll
-                for (int q = 0; q < QA; ++q)
+                for (int q = 0; q < QA; ++q) {
+                    if (lv < TR) {
 #pragma unroll
-                    for (int cb = 0; cb < CB; ++cb) {
-                        R[lv][q][cb] = x[q][cb];
-                        x[q][cb] = nx[q][cb];
+                        for (int cb = 0; cb < CB; ++cb) R[lv < TR ? lv : 0][q][cb] = x[q][cb];
+                    } else {
+#pragma unroll
+                        for (int v4 = 0; v4 < CB / VW; ++v4) {
+                            V128 t;
+#pragma unroll
+                            for (int e = 0; e < VW; ++e) t.v[e] = x[q][v4 * VW + e];
+                            *reinterpret_cast<V128 *>(rsm_at(lv, q, v4)) = t;
+                        }
                     }
+#pragma unroll
+                    for (int cb = 0; cb < CB; ++cb) x[q][cb] = nx[q][cb];
+                }
             }
             // ---- store level T of plane j; S9 partial sums
             if (live) {

@@ -89,7 +89,7 @@ def test_state_and_argument_errors_on_gpu():
     with pytest.raises(b.MMError):
         mm.set_density_range(1, 2, np.zeros(2 * g.inner))
     with pytest.raises(b.MMError):
-        mm.set_option(b.MM_OPT_FUSE_T, 9)
+        mm.set_option(b.MM_OPT_FUSE_T, b.MM_MAX_FUSE_T + 1)
     mm.set_option(b.MM_OPT_KERNEL, 2)
     with pytest.raises(b.MMError) as e:          # 3x3 offsets: streamed kernel unsupported -> loud error
         mm.substep(1, 0.01)

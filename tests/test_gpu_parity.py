@@ -203,6 +203,18 @@ def test_coef_kernel_parity(dtype, T, nxi):
     assert info["kernel"].startswith("coef<"), info
 
 
+@pytest.mark.parametrize("T", [7, 8, 9, 10])
+def test_coef_deep_fusion_fp32(T):
+    """Depth 7-10 (fp32, 16x16 only): the upwind planes of the levels beyond 6 live in shared memory."""
+    g = Grid(5, 7, 20, 7, 16, 16)
+    p = Params()
+    e, info = check_parity(g, p, "f32", [2 * T + 3, T], _dt(g, p), kernel=4, fuse_t=T)
+    assert info["kernel"].startswith("coef<f32"), info
+    # other dtypes / planes clamp the depth to 6 and still match
+    check_parity(Grid(3, 3, 8, 7, 8, 8), p, "f32", [13], _dt(Grid(3, 3, 8, 7, 8, 8), p), kernel=4, fuse_t=T)
+    check_parity(g, p, "f64", [13], _dt(g, p), kernel=4, fuse_t=T)
+
+
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_coef_many_configs_per_warp(dtype):
     g = Grid(16, 16, 16, 6, 8, 8)   # 4096 configs of 384 cells
