@@ -90,7 +90,7 @@ typedef enum {
                                 (2, 3, 4: MM_ERR_INVALID_ARG from mm_substep if the grid/flags are unsupported) */
     MM_OPT_FUSE_T = 1,       /* max substeps fused per HBM pass (temporal fusion), 1..MM_MAX_FUSE_T; mm_substep uses as
                                 few passes as this allows, of balanced depth (10 substeps at depth 6 = 5 + 5);
-                                default 10 (fp32) / 4 (fp64) */
+                                default 10 (fp32) / 5 (fp64) */
     MM_OPT_FUSE_MOMENTS = 2, /* 1 (default): the last pass of mm_substep also reduces the moments, so a
                                 following mm_moments is a copy; 0: mm_moments always runs its own pass */
     MM_OPT_FREE_COUPLING = 4,/* 1: the source term of the substeps is k_on M_f(r0) from the table of the last

@@ -222,7 +222,7 @@ static mm_status launch_coef_inst_mf(mm_ctx *c, double dt, const void *in, void 
     constexpr int MINB = sizeof(real) == 8 ? MM_COEF_MINB_F64 : MM_COEF_MINB_F32;
     constexpr bool PM = sizeof(real) == 8;   // post-mask: fp64 only
     constexpr bool CS = sizeof(real) == 8;   // per-configuration constants in shared memory: fp64 only
-    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS, coef_rs(T)>;
+    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS, coef_rs<real>(T)>;
     auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB, PM, CS, false, MF>;
     // MF: the warps' node tables (16-bit, ns * (NXI + NETA) entries each) sit behind the regular layout
     const size_t smem = MF ? ((Cfg::SMEM_BYTES + 15) / 16) * 16 + (size_t)WARPS * c->g.ns * (NXI + NETA) * 2 : Cfg::SMEM_BYTES;
@@ -294,7 +294,7 @@ static mm_status launch_coef_local_inst(mm_ctx *c, const void *in, void *out, in
     constexpr int P = 2, D = 3, WARPS = MM_COEF_WARPS;
     constexpr int MINB = sizeof(real) == 8 ? MM_COEF_MINB_F64 : MM_COEF_MINB_F32;
     constexpr bool PM = sizeof(real) == 8, CS = sizeof(real) == 8;
-    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
+    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS, coef_rs<real>(T)>;
     auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB, PM, CS, true>;
     static int blocks_per_sm = 0;
     if (blocks_per_sm == 0) {
@@ -583,8 +583,8 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
     // measured defaults: the coefficient-form kernel, at most 10 (fp32; 6 off the 16x16
-    // offset plane) / 4 (fp64) substeps per pass
-    c->opt_kernel = 0; c->opt_fuse_t = dtype == MM_F64 ? 4 : 10; c->opt_fuse_mom = 1;
+    // offset plane) / 5 (fp64) substeps per pass
+    c->opt_kernel = 0; c->opt_fuse_t = dtype == MM_F64 ? 5 : 10; c->opt_fuse_mom = 1;
     c->single = (b0 != nullptr && b1 == nullptr);
     c->opt_inplace = c->single ? 1 : 0;
     c->checked_dt = NAN; c->launches = 0; c->kname[0] = 0;

@@ -67,7 +67,14 @@ __device__ __forceinline__ double rabs(double x) { return fabs(x); }
 #ifndef MM_COEF_RREG
 #define MM_COEF_RREG 6   // fuse levels whose upwind plane stays in registers; deeper levels keep it in shared memory
 #endif
-__host__ __device__ constexpr int coef_rs(int T) { return T > MM_COEF_RREG ? T - MM_COEF_RREG : 0; }
+#ifndef MM_COEF_RREG_F64
+#define MM_COEF_RREG_F64 1   // fp64: only the first level's upwind plane in registers (measured, profiles/r01h_README.md)
+#endif
+template <typename real>
+__host__ __device__ constexpr int coef_rs(int T)
+{
+    return T > (sizeof(real) == 8 ? MM_COEF_RREG_F64 : MM_COEF_RREG) ? T - (sizeof(real) == 8 ? MM_COEF_RREG_F64 : MM_COEF_RREG) : 0;
+}
 
 template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, bool CS, int RS = 0>
 struct CoefCfg {
@@ -116,7 +123,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                         int32_t done = 0, const int32_t *__restrict__ list = nullptr,
                         const int32_t *__restrict__ list_count = nullptr)
 {
-    constexpr int RS = coef_rs(T), TR = T - RS;   // levels with the upwind plane in shared memory / in registers
+    constexpr int RS = coef_rs<real>(T), TR = T - RS;   // levels with the upwind plane in shared memory / in registers
     using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS, RS>;
     constexpr int LB = Cfg::LB, G = Cfg::G, QA = Cfg::QA, PLANE = Cfg::PLANE, NK = Cfg::NK, NKV = Cfg::NKV;
     constexpr int VW = Cfg::VW;
