@@ -28,6 +28,16 @@ __device__ __forceinline__ int anchor_node(const FreeGeom &q, int ix, int iy, do
     return (int)(nx_ * q.ny + ny_);
 }
 
+// floor(r) wrapped into [0, n) without integer division (same construction as wrap_node in mm_coef.cuh)
+__device__ __forceinline__ int wrap_floor(double r, int n)
+{
+    const double f = floor(r), qd = floor(f * (1.0 / (double)n));
+    int m = __double2int_rn(f - qd * (double)n);
+    m += m < 0 ? n : 0;
+    m -= m >= n ? n : 0;
+    return m;
+}
+
 // MODE 0: raw[n] += w Psi_c m over all cells (fp64 atomic adds, macro cadence).  MODE 1: m *= f[n] (cap rescale), skipped
 // entirely when no node was capped.  One warp per configuration, lanes stride over the cells of each plane.
 template <typename real, int MODE>
@@ -46,12 +56,34 @@ __global__ void __launch_bounds__(256) free_cells_kernel(const FreeGeom q, int64
         const double ct = cos(theta), st = sin(theta);
         const double wp = MODE == 0 ? w * psi[c] : 0.0;
         real *mc = dens + c * (int64_t)plane * q.ns;
+        const bool small = q.nxi <= 16 && q.neta <= 16;   // node index separates: 32 node coordinates per plane, not 2 per cell
         for (int j = 0; j < q.ns; ++j) {
             const double sj = __dadd_rn(q.s_lo, __dmul_rn(j + 0.5, q.ds));
-            for (int i = lane; i < plane; i += 32) {
-                const int a = i / q.neta, b = i - a * q.neta;
-                const double xi = __dadd_rn(-q.R, __dmul_rn(a + 0.5, q.dxi)), eta = __dadd_rn(-q.R, __dmul_rn(b + 0.5, q.deta));
-                const int n = anchor_node(q, ix, iy, ct, st, sj, xi, eta);
+            int my_node = 0;   // lanes 0..15: x node of row a = lane (times ny); lanes 16..31: y node of column b = lane - 16
+            if (small) {
+                const int k = lane & 15;
+                if (lane < 16) {
+                    const double xi = __dadd_rn(-q.R, __dmul_rn(k + 0.5, q.dxi));
+                    const double rx = __dmul_rn(__dsub_rn(__dadd_rn(__ddiv_rn((double)ix, (double)q.nx), __dmul_rn(sj, ct)), xi), (double)q.nx);
+                    my_node = wrap_floor(__dadd_rn(rx, 0.5), q.nx) * q.ny;
+                } else {
+                    const double eta = __dadd_rn(-q.R, __dmul_rn(k + 0.5, q.deta));
+                    const double ry = __dmul_rn(__dsub_rn(__dadd_rn(__ddiv_rn((double)iy, (double)q.ny), __dmul_rn(sj, st)), eta), (double)q.ny);
+                    my_node = wrap_floor(__dadd_rn(ry, 0.5), q.ny);
+                }
+            }
+            for (int i0 = 0; i0 < plane; i0 += 32) {
+                const int i = i0 + lane;
+                const bool in_plane = i < plane;
+                const int a = in_plane ? i / q.neta : 0, b = in_plane ? i - a * q.neta : 0;
+                int n;
+                if (small) {
+                    n = __shfl_sync(0xffffffffu, my_node, a) + __shfl_sync(0xffffffffu, my_node, 16 + b);
+                } else {
+                    const double xi = __dadd_rn(-q.R, __dmul_rn(a + 0.5, q.dxi)), eta = __dadd_rn(-q.R, __dmul_rn(b + 0.5, q.deta));
+                    n = anchor_node(q, ix, iy, ct, st, sj, xi, eta);
+                }
+                if (!in_plane) continue;
                 real *v = mc + (int64_t)j * plane + i;
                 if (MODE == 0) {
                     const double val = (double)*v;
