@@ -300,7 +300,11 @@ def run_cuda(args):
                 "avg_launch_ms": round(sub_ms / n_launch, 4),
                 "pass_gbs": round(pass_bytes / (sub_ms * 1e-3) / 1e9, 1),
                 "pass_frac": round(pass_bytes / (sub_ms * 1e-3) / 1e9 / peak, 4),
-                "kernel_share_of_step": round(sub_ms / ms, 4)}
+                "kernel_share_of_step": round(sub_ms / ms, 4),
+                "note": "achieved = algorithmic bytes (2*sizeof(real) per cell-update, the one-substep-per-pass count of "
+                        "SURVEY 8(d)) / kernel time; a launch fuses fuse_T substeps into ONE read + ONE write of the density, "
+                        "so frac > 1 is temporal fusion, not a faster memory: pass_gbs/pass_frac = DRAM rate of the pass "
+                        "actually moved (= traffic / time), t1_* = the same kernel unfused"}
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_file):
         try:
