@@ -102,7 +102,7 @@ typedef enum {
                                 buffer is not touched; same results, same speed, half the memory.  Default 0; always 1
                                 for a context created with ONE density buffer (mm_create, dens_buf1 = NULL) */
 } mm_option;
-#define MM_MAX_FUSE_T 10  /* fp32 coefficient-form kernels on 16x16 offset planes; other coefficient-form kernels
+#define MM_MAX_FUSE_T 12  /* fp32 coefficient-form kernels on 16x16 offset planes; other coefficient-form kernels
                              fuse at most 6, the streamed / tiled variants at most 4 (deeper settings are clamped) */
 #define MM_LOCAL_FUSE_T 4 /* levels per pass of mm_advance_local */
 

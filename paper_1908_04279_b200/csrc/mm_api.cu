@@ -2,103 +2,19 @@
 // All arithmetic of the hot path lives in the kernels (mm_coef.cuh = default; mm_stream.cuh, mm_tile.cuh,
 // mm_generic.cuh = variants / fallback for other grids; mm_rk2.cuh, mm_local.cuh = SURVEY.md 8(f) NEXT-1, NEXT-3);
 // this file only validates, marshals arguments and launches.  There is no CPU fallback.
-#include "../../include/mm.h"
-
-#include <cmath>
-#include <cstdio>
-#include <cstring>
-#include <new>
-#include <string>
-#include <vector>
+#include "mm_ctx.cuh"
 
 #include "mm_generic.cuh"
-#include "mm_stream.cuh"
-#include "mm_tile.cuh"
-#include "mm_coef.cuh"
-#include "mm_rk2.cuh"
 #include "mm_local.cuh"
 #include "mm_spread.cuh"
 #include "mm_free.cuh"
 
-using namespace mm;
+thread_local std::string g_create_err;
 
-struct mm_ctx {
-    mm_grid g;
-    mm_params p;
-    mm_dtype dtype;
-    size_t esize;
-    int64_t nc, inner, cells;
-    cudaStream_t stream;
-    void *buf[2];
-    bool owns;
-    int cur;
-    void *U, *V, *Om;               // [nc] real
-    void *kappa, *cos_t, *sin_t;    // tables (real)
-    uint8_t *inside;
-    double *mom_force, *mom_torque; // [nc][2], [nc]
-    unsigned int *flag_dev;         // stability-check flag
-    bool mom_valid, vel_set;
-    std::vector<uint8_t> dens_cov;  // per configuration: density uploaded
-    int64_t dens_cov_count;
-    int opt_kernel, opt_fuse_t, opt_fuse_mom, opt_inplace;
-    bool single;                    // created with ONE density buffer: only the in-place kernels can run
-    double checked_dt;              // dt the S8 check last passed with (NaN = none)
-    int64_t launches;
-    int sm_count;
-    double *loc_lambda;             // NEXT-3: per-configuration rate bound, step count, local dt, max step count
-    int32_t *loc_n, *loc_nmax, *loc_list, *loc_count;
-    void *loc_dt;
-    bool loc_valid;
-    double *psi, *fline, *F2;       // NEXT-4: filament density weights [nc], plane forces [nc][ns][2], fluid-grid force
-    bool psi_set;
-    double *Mf, *Mbc, *free_raw, *free_factor;   // NEXT-2: free / coarse bound motor tables [nx][ny], scratch
-    int *free_any;
-    bool coupled;                   // the substep source is k_on M_f(r0) instead of k_on m_free
-    CUtensorMap tmap[2];            // tiled-TMA views of buf[0], buf[1] (tile kernel)
-    bool tile_ok;                   // tensor maps built and grid/flags supported by the tile kernel
-    std::string err;
-    char kname[64];
-};
-
-static thread_local std::string g_create_err;
-
-static mm_status fail(mm_ctx *ctx, mm_status s, const std::string &msg)
-{
-    if (ctx) ctx->err = msg; else g_create_err = msg;
-    return s;
-}
-#define CUDA_TRY(ctx, expr)                                                                          \
-    do {                                                                                             \
-        cudaError_t e_ = (expr);                                                                     \
-        if (e_ != cudaSuccess)                                                                       \
-            return fail(ctx, e_ == cudaErrorMemoryAllocation ? MM_ERR_NOMEM : MM_ERR_CUDA,           \
-                        std::string(#expr) + ": " + cudaGetErrorString(e_));                         \
-    } while (0)
-
-template <typename real>
-static KParams<real> make_kparams(const mm_ctx *c, double dt)
-{
-    KParams<real> k;
-    const mm_grid &g = c->g;
-    const mm_params &p = c->p;
-    k.nc = c->nc; k.ns = g.ns; k.nxi = g.nxi; k.neta = g.neta; k.ntheta = g.ntheta;
-    k.n_end = p.n_end_cells; k.flags = p.flags;
-    const double ds = (p.s_hi - p.s_lo) / g.ns, dxi = 2.0 * p.R / g.nxi, deta = 2.0 * p.R / g.neta;
-    k.v0 = (real)p.v0; k.kload = (real)(p.k_spring / p.f_stall);
-    k.R = (real)p.R; k.dxi = (real)dxi; k.deta = (real)deta; k.ds = (real)ds; k.s_lo = (real)p.s_lo;
-    k.dt = (real)dt; k.dt_ds = (real)(dt / ds); k.dt_dxi = (real)(dt / dxi); k.dt_deta = (real)(dt / deta);
-    k.dt_src = (real)(dt * p.k_on * p.m_free);
-    k.dt_kon = (real)(dt * p.k_on);
-    k.Mf = (c->coupled && c->Mf) ? c->Mf : nullptr;
-    k.nx = g.nx; k.ny = g.ny;
-    k.geo_R = p.R; k.geo_dxi = dxi; k.geo_deta = deta; k.geo_ds = ds; k.geo_s_lo = p.s_lo;
-    k.dt_endx = (real)(dt * (p.end_detach_mult - 1.0));
-    k.mom_scale = -p.k_spring * ds * dxi * deta;
-    k.U = (const real *)c->U; k.V = (const real *)c->V; k.Om = (const real *)c->Om;
-    k.cos_t = (const real *)c->cos_t; k.sin_t = (const real *)c->sin_t;
-    k.kappa = (const real *)c->kappa; k.inside = c->inside;
-    return k;
-}
+// what MM_OPT_KERNEL = 0 picks where the grid and flags allow a fast kernel (measured)
+#ifndef MM_AUTO_KERNEL
+#define MM_AUTO_KERNEL 5
+#endif
 
 // ---- S8 positivity bound (only with MM_FLAG_CHECK_DT) -----------------------------------------
 template <typename real>
@@ -128,317 +44,6 @@ __global__ void check_dt_kernel(const __grid_constant__ KParams<real> kp, unsign
     }
 }
 
-// ---- streamed-kernel dispatch -----------------------------------------------------------------
-template <typename real, int NXI, int NETA, int CB, int T, bool MOM>
-static mm_status launch_stream_inst(mm_ctx *c, double dt, const void *in, void *out)
-{
-    constexpr int P = 2, D = 3, WARPS = 4;
-    using Cfg = StreamCfg<real, NXI, NETA, CB, P, D, WARPS>;
-    auto kern = substep_stream_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS>;
-    static int blocks_per_sm = 0;
-    if (blocks_per_sm == 0) {
-        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
-        int n = 0;
-        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, Cfg::SMEM_BYTES));
-        if (n < 1) return fail(c, MM_ERR_CUDA, "streamed kernel does not fit on an SM");
-        blocks_per_sm = n;
-    }
-    int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
-    const int64_t need = (c->nc + WARPS - 1) / WARPS;
-    if (grid > need) grid = need;
-    KParams<real> kp = make_kparams<real>(c, dt);
-    kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(kp, (const real *)in, (real *)out, c->mom_force,
-                                                                      c->mom_torque);
-    CUDA_TRY(c, cudaGetLastError());
-    c->launches++;
-    snprintf(c->kname, sizeof c->kname, "stream<%s,%dx%d,CB=%d,T=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
-             CB, T, MOM ? ",mom" : "");
-    return MM_OK;
-}
-
-template <typename real, int NXI, int NETA, int CB>
-static mm_status launch_stream_shape(mm_ctx *c, int T, bool mom, double dt, const void *in, void *out)
-{
-#define MM_CASE(TT)                                                                                     \
-    case TT:                                                                                            \
-        return mom ? launch_stream_inst<real, NXI, NETA, CB, TT, true>(c, dt, in, out)                  \
-                   : launch_stream_inst<real, NXI, NETA, CB, TT, false>(c, dt, in, out);
-    switch (T) {
-        MM_CASE(1)
-        MM_CASE(2)
-        MM_CASE(3)
-        MM_CASE(4)
-    }
-#undef MM_CASE
-    return fail(c, MM_ERR_INVALID_ARG, "unsupported fuse depth");
-}
-
-static bool stream_supported(const mm_ctx *c)
-{
-    if (c->p.flags & (MM_FLAG_S_PERIODIC | MM_FLAG_OFFSET_PERIODIC_NOMASK)) return false;
-    return (c->g.nxi == 16 && c->g.neta == 16) || (c->g.nxi == 8 && c->g.neta == 8);
-}
-
-static mm_status launch_stream(mm_ctx *c, int T, bool mom, double dt, const void *in, void *out)
-{
-    const bool big = c->g.nxi == 16;
-    if (c->dtype == MM_F64)
-        return big ? launch_stream_shape<double, 16, 16, 2>(c, T, mom, dt, in, out)
-                   : launch_stream_shape<double, 8, 8, 2>(c, T, mom, dt, in, out);
-    return big ? launch_stream_shape<float, 16, 16, 4>(c, T, mom, dt, in, out)
-               : launch_stream_shape<float, 8, 8, 2>(c, T, mom, dt, in, out);
-}
-
-// ---- coefficient-form kernel dispatch -----------------------------------------------------------
-// Launch shape of the coefficient-form kernel, per dtype (measured sweep in profiles/r01b_README.md):
-// planes per TMA copy, ring depth, warps per CTA, resident CTAs per SM asked of the register allocator.
-#ifndef MM_COEF_P_F32
-#define MM_COEF_P_F32 4
-#endif
-#ifndef MM_COEF_D_F32
-#define MM_COEF_D_F32 2
-#endif
-#ifndef MM_COEF_P_F64
-#define MM_COEF_P_F64 2
-#endif
-#ifndef MM_COEF_D_F64
-#define MM_COEF_D_F64 3
-#endif
-#ifndef MM_COEF_WARPS
-#define MM_COEF_WARPS 4
-#endif
-#ifndef MM_COEF_MINB_F32
-#define MM_COEF_MINB_F32 2
-#endif
-#ifndef MM_COEF_MINB_F64
-#define MM_COEF_MINB_F64 2
-#endif
-
-template <typename real, int NXI, int NETA, int CB, int T, bool MOM, bool MF>
-static mm_status launch_coef_inst_mf(mm_ctx *c, double dt, const void *in, void *out)
-{
-    constexpr int P = sizeof(real) == 8 ? MM_COEF_P_F64 : MM_COEF_P_F32;
-    constexpr int D = sizeof(real) == 8 ? MM_COEF_D_F64 : MM_COEF_D_F32, WARPS = MM_COEF_WARPS;
-    constexpr int MINB = sizeof(real) == 8 ? MM_COEF_MINB_F64 : MM_COEF_MINB_F32;
-    constexpr bool PM = sizeof(real) == 8;   // post-mask: fp64 only
-    constexpr bool CS = sizeof(real) == 8;   // per-configuration constants in shared memory: fp64 only
-    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS, coef_rs<real>(T)>;
-    auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB, PM, CS, false, MF>;
-    // MF: the warps' node tables (16-bit, ns * (NXI + NETA) entries each) sit behind the regular layout
-    const size_t smem = MF ? ((Cfg::SMEM_BYTES + 15) / 16) * 16 + (size_t)WARPS * c->g.ns * (NXI + NETA) * 2 : Cfg::SMEM_BYTES;
-    static int blocks_per_sm = 0;
-    static size_t smem_set = 0;
-    if (blocks_per_sm == 0 || smem != smem_set) {
-        if (smem > 227 * 1024) return fail(c, MM_ERR_INVALID_ARG, "ns too large for the coupled coefficient-form kernel");
-        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int n = 0;
-        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, smem));
-        if (n < 1) return fail(c, MM_ERR_CUDA, "coefficient-form kernel does not fit on an SM");
-        blocks_per_sm = n;
-        smem_set = smem;
-    }
-    int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
-    const int64_t need = (c->nc + WARPS - 1) / WARPS;
-    if (grid > need) grid = need;
-    KParams<real> kp = make_kparams<real>(c, dt);
-    kern<<<(unsigned)grid, WARPS * 32, smem, c->stream>>>(kp, (const real *)in, (real *)out, c->mom_force, c->mom_torque,
-                                                           nullptr, nullptr, 0, nullptr, nullptr);
-    CUDA_TRY(c, cudaGetLastError());
-    c->launches++;
-    snprintf(c->kname, sizeof c->kname, MF ? "coef_mf<%s,%dx%d,CB=%d,T=%d%s>" : "coef<%s,%dx%d,CB=%d,T=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
-             CB, T, MOM ? ",mom" : "");
-    return MM_OK;
-}
-
-template <typename real, int NXI, int NETA, int CB, int T, bool MOM>
-static mm_status launch_coef_inst(mm_ctx *c, double dt, const void *in, void *out)
-{
-    return c->coupled ? launch_coef_inst_mf<real, NXI, NETA, CB, T, MOM, true>(c, dt, in, out)
-                      : launch_coef_inst_mf<real, NXI, NETA, CB, T, MOM, false>(c, dt, in, out);
-}
-
-template <typename real, int NXI, int NETA, int CB>
-static mm_status launch_coef_shape(mm_ctx *c, int T, bool mom, double dt, const void *in, void *out)
-{
-#define MM_CASE(TT)                                                                                     \
-    case TT:                                                                                            \
-        return mom ? launch_coef_inst<real, NXI, NETA, CB, TT, true>(c, dt, in, out)                    \
-                   : launch_coef_inst<real, NXI, NETA, CB, TT, false>(c, dt, in, out);
-    switch (T) {
-        MM_CASE(1)
-        MM_CASE(2)
-        MM_CASE(3)
-        MM_CASE(4)
-        MM_CASE(5)
-        MM_CASE(6)
-    }
-    if constexpr (sizeof(real) == 4 && NXI == 16) {   // deeper fusion where it pays: fp32, the BASELINE offset plane
-        switch (T) {
-            MM_CASE(7)
-            MM_CASE(8)
-            MM_CASE(9)
-            MM_CASE(10)
-        }
-    }
-#undef MM_CASE
-    return fail(c, MM_ERR_INVALID_ARG, "unsupported fuse depth");
-}
-
-// NEXT-3: one pass of the local-step variant (T = MM_LOCAL_FUSE_T levels at most per configuration)
-template <typename real, int NXI, int NETA, int CB, bool MOM>
-static mm_status launch_coef_local_inst(mm_ctx *c, const void *in, void *out, int32_t done, bool use_list)
-{
-    constexpr int T = MM_LOCAL_FUSE_T;
-    // 2 planes x 3 slots for both dtypes: the kernel holds T+1 straight-line instances of the chunk body (one per
-    // level count), so the chunk is kept short to stay inside the instruction cache
-    constexpr int P = 2, D = 3, WARPS = MM_COEF_WARPS;
-    constexpr int MINB = sizeof(real) == 8 ? MM_COEF_MINB_F64 : MM_COEF_MINB_F32;
-    constexpr bool PM = sizeof(real) == 8, CS = sizeof(real) == 8;
-    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS, coef_rs<real>(T)>;
-    auto kern = substep_coef_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB, PM, CS, true>;
-    static int blocks_per_sm = 0;
-    if (blocks_per_sm == 0) {
-        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
-        int n = 0;
-        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, Cfg::SMEM_BYTES));
-        if (n < 1) return fail(c, MM_ERR_CUDA, "local-step kernel does not fit on an SM");
-        blocks_per_sm = n;
-    }
-    int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
-    const int64_t need = (c->nc + WARPS - 1) / WARPS;
-    if (grid > need) grid = need;
-    KParams<real> kp = make_kparams<real>(c, 1.0);   // per unit dt
-    // in may equal out (in-place pass, see the LOC note in mm_coef.cuh)
-    kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(kp, (const real *)in, (real *)out, c->mom_force,
-                                                                      c->mom_torque, c->loc_n, (const real *)c->loc_dt, done,
-                                                                      use_list ? c->loc_list : nullptr,
-                                                                      use_list ? c->loc_count : nullptr);
-    CUDA_TRY(c, cudaGetLastError());
-    c->launches++;
-    snprintf(c->kname, sizeof c->kname, "coef_local<%s,%dx%d,CB=%d,T<=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA,
-             CB, T, MOM ? ",mom" : "");
-    return MM_OK;
-}
-
-static mm_status launch_coef_local(mm_ctx *c, bool mom, const void *in, void *out, int32_t done, bool use_list)
-{
-    const bool big = c->g.nxi == 16;
-#define MM_LOC(R_, N_, CB_) (mom ? launch_coef_local_inst<R_, N_, N_, CB_, true>(c, in, out, done, use_list) \
-                                 : launch_coef_local_inst<R_, N_, N_, CB_, false>(c, in, out, done, use_list))
-    if (c->dtype == MM_F64) return big ? MM_LOC(double, 16, 2) : MM_LOC(double, 8, 2);
-    return big ? MM_LOC(float, 16, 4) : MM_LOC(float, 8, 2);
-#undef MM_LOC
-}
-
-static mm_status launch_coef(mm_ctx *c, int T, bool mom, double dt, const void *in, void *out)
-{
-    const bool big = c->g.nxi == 16;
-    if (c->dtype == MM_F64)
-        return big ? launch_coef_shape<double, 16, 16, 2>(c, T, mom, dt, in, out)
-                   : launch_coef_shape<double, 8, 8, 2>(c, T, mom, dt, in, out);
-    return big ? launch_coef_shape<float, 16, 16, 4>(c, T, mom, dt, in, out)
-               : launch_coef_shape<float, 8, 8, 2>(c, T, mom, dt, in, out);
-}
-
-// ---- tile-kernel dispatch ---------------------------------------------------------------------
-typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static constexpr int TILE_P = 2;   // planes per TMA box
-
-static bool tile_shape_supported(const mm_ctx *c)
-{
-    if (c->p.flags & (MM_FLAG_S_PERIODIC | MM_FLAG_OFFSET_PERIODIC_NOMASK)) return false;
-    return (c->g.nxi == 16 && c->g.neta == 16) || (c->g.nxi == 8 && c->g.neta == 8);
-}
-
-// 4-D view (eta, xi, s, c) of a density buffer; box = one padded plane pair of CPW configurations,
-// out-of-bounds elements read as zero (the ghost cells of S5).
-static mm_status build_tensor_maps(mm_ctx *c)
-{
-    c->tile_ok = false;
-    if (!tile_shape_supported(c) || c->single) return MM_OK;
-    void *fn = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
-        qres != cudaDriverEntryPointSuccess) {
-        cudaGetLastError();
-        return fail(c, MM_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
-    }
-    const int cpw = 256 / (c->g.nxi * c->g.neta);
-    const cuuint64_t dims[4] = {(cuuint64_t)c->g.neta, (cuuint64_t)c->g.nxi, (cuuint64_t)c->g.ns, (cuuint64_t)c->nc};
-    const cuuint64_t strides[3] = {(cuuint64_t)c->g.neta * c->esize, (cuuint64_t)c->g.nxi * c->g.neta * c->esize,
-                                   (cuuint64_t)c->inner * c->esize};
-    const cuuint32_t box[4] = {(cuuint32_t)c->g.neta + (cuuint32_t)(32 / c->esize), (cuuint32_t)c->g.nxi + 2, (cuuint32_t)TILE_P, (cuuint32_t)cpw};
-    const cuuint32_t estr[4] = {1, 1, 1, 1};
-    for (int b = 0; b < 2; ++b) {
-        CUresult r = ((encode_tiled_fn)fn)(&c->tmap[b], c->dtype == MM_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64
-                                                                          : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
-                                           4, c->buf[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) return fail(c, MM_ERR_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
-    }
-    c->tile_ok = true;
-    return MM_OK;
-}
-
-template <typename real, int NXI, int NETA, int CB, int T, bool MOM>
-static mm_status launch_tile_inst(mm_ctx *c, double dt, int in_idx, void *out)
-{
-    constexpr int P = TILE_P, D = (T == 1 ? 4 : 3), WARPS = 4, MINB = 2;
-    using Cfg = TileCfg<real, NXI, NETA, CB, T, P, D, WARPS>;
-    auto kern = substep_tile_kernel<real, NXI, NETA, CB, T, MOM, P, D, WARPS, MINB>;
-    static int blocks_per_sm = 0;
-    if (blocks_per_sm == 0) {
-        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
-        int n = 0;
-        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, Cfg::SMEM_BYTES));
-        if (n < 1) return fail(c, MM_ERR_CUDA, "tile kernel does not fit on an SM");
-        blocks_per_sm = n;
-    }
-    int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
-    const int64_t groups = (c->nc + Cfg::CPW - 1) / Cfg::CPW;
-    const int64_t need = (groups + WARPS - 1) / WARPS;
-    if (grid > need) grid = need;
-    KParams<real> kp = make_kparams<real>(c, dt);
-    kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(kp, c->tmap[in_idx], (real *)out, c->mom_force,
-                                                                      c->mom_torque);
-    CUDA_TRY(c, cudaGetLastError());
-    c->launches++;
-    snprintf(c->kname, sizeof c->kname, "tile<%s,%dx%d,T=%d%s>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA, T,
-             MOM ? ",mom" : "");
-    return MM_OK;
-}
-
-template <typename real, int NXI, int NETA, int CB>
-static mm_status launch_tile_shape(mm_ctx *c, int T, bool mom, double dt, int in_idx, void *out)
-{
-#define MM_CASE(TT)                                                                                     \
-    case TT:                                                                                            \
-        return mom ? launch_tile_inst<real, NXI, NETA, CB, TT, true>(c, dt, in_idx, out)                \
-                   : launch_tile_inst<real, NXI, NETA, CB, TT, false>(c, dt, in_idx, out);
-    switch (T) {
-        MM_CASE(1)
-        MM_CASE(2)
-        MM_CASE(3)
-        MM_CASE(4)
-    }
-#undef MM_CASE
-    return fail(c, MM_ERR_INVALID_ARG, "unsupported fuse depth");
-}
-
-static mm_status launch_tile(mm_ctx *c, int T, bool mom, double dt, int in_idx, void *out)
-{
-    const bool big = c->g.nxi == 16;
-    if (c->dtype == MM_F64)
-        return big ? launch_tile_shape<double, 16, 16, 2>(c, T, mom, dt, in_idx, out)
-                   : launch_tile_shape<double, 8, 8, 2>(c, T, mom, dt, in_idx, out);
-    return big ? launch_tile_shape<float, 16, 16, 4>(c, T, mom, dt, in_idx, out)
-               : launch_tile_shape<float, 8, 8, 4>(c, T, mom, dt, in_idx, out);
-}
-
 template <typename real>
 static mm_status launch_generic(mm_ctx *c, double dt, const void *in, void *out)
 {
@@ -451,62 +56,6 @@ static mm_status launch_generic(mm_ctx *c, double dt, const void *in, void *out)
     c->launches++;
     snprintf(c->kname, sizeof c->kname, "generic<%s>", sizeof(real) == 8 ? "f64" : "f32");
     return MM_OK;
-}
-
-// One RK2 + Superbee substep with the generic stage kernel: m* into the spare buffer, m^{n+1} in place.
-template <typename real>
-static mm_status launch_rk2_generic(mm_ctx *c, double dt)
-{
-    int64_t blocks = (c->cells + 255) / 256;
-    const int64_t cap = (int64_t)c->sm_count * 64;
-    if (blocks > cap) blocks = cap;
-    real *A = (real *)c->buf[c->cur], *B = (real *)c->buf[c->cur ^ 1];
-    rk2_stage_generic_kernel<real><<<(unsigned)blocks, 256, 0, c->stream>>>(make_kparams<real>(c, 0.5 * dt), A, A, B);
-    CUDA_TRY(c, cudaGetLastError());
-    rk2_stage_generic_kernel<real><<<(unsigned)blocks, 256, 0, c->stream>>>(make_kparams<real>(c, dt), A, B, A);
-    CUDA_TRY(c, cudaGetLastError());
-    c->launches += 2;
-    snprintf(c->kname, sizeof c->kname, "rk2_generic<%s>", sizeof(real) == 8 ? "f64" : "f32");
-    return MM_OK;
-}
-
-// One RK2 + Superbee substep in one HBM pass (rk2_fused_kernel): reads buf[cur], writes buf[cur^1].
-template <typename real, int NXI, int NETA, int CB>
-static mm_status launch_rk2_fused(mm_ctx *c, double dt)
-{
-    constexpr int P = 2, D = 3, WARPS = 4, MINB = 2;
-    constexpr bool PM = sizeof(real) == 8, CS = sizeof(real) == 8;
-    using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
-    constexpr bool KEEPC = sizeof(real) == 4;
-    auto kern = rk2_fused_kernel<real, NXI, NETA, CB, P, D, WARPS, MINB, PM, CS, KEEPC>;
-    static int blocks_per_sm = 0;
-    if (blocks_per_sm == 0) {
-        CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM_BYTES));
-        int n = 0;
-        CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, WARPS * 32, Cfg::SMEM_BYTES));
-        if (n < 1) return fail(c, MM_ERR_CUDA, "fused RK2 kernel does not fit on an SM");
-        blocks_per_sm = n;
-    }
-    int64_t grid = (int64_t)c->sm_count * blocks_per_sm;
-    const int64_t need = (c->nc + WARPS - 1) / WARPS;
-    if (grid > need) grid = need;
-    // in place when asked: stage 2 stores plane i-2 when plane i has arrived, every input plane is read once
-    const int dst = c->opt_inplace ? c->cur : c->cur ^ 1;
-    kern<<<(unsigned)grid, WARPS * 32, Cfg::SMEM_BYTES, c->stream>>>(make_kparams<real>(c, dt), (const real *)c->buf[c->cur],
-                                                                      (real *)c->buf[dst]);
-    CUDA_TRY(c, cudaGetLastError());
-    c->launches++;
-    c->cur = dst;
-    snprintf(c->kname, sizeof c->kname, "rk2_fused<%s,%dx%d,CB=%d>", sizeof(real) == 8 ? "f64" : "f32", NXI, NETA, CB);
-    return MM_OK;
-}
-
-static mm_status launch_rk2_fused_any(mm_ctx *c, double dt)
-{
-    const bool big = c->g.nxi == 16;
-    if (c->dtype == MM_F64)
-        return big ? launch_rk2_fused<double, 16, 16, 2>(c, dt) : launch_rk2_fused<double, 8, 8, 2>(c, dt);
-    return big ? launch_rk2_fused<float, 16, 16, 4>(c, dt) : launch_rk2_fused<float, 8, 8, 2>(c, dt);
 }
 
 template <typename real>
@@ -573,6 +122,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->g = g; c->p = p; c->dtype = dtype; c->esize = dtype == MM_F64 ? 8 : 4;
     c->nc = nc; c->inner = inner; c->cells = nc * inner;
     c->stream = (cudaStream_t)cuda_stream;
+    c->device = dev;
     c->buf[0] = b0; c->buf[1] = b1; c->owns = (b0 == nullptr); c->cur = 0;
     c->U = c->V = c->Om = c->kappa = c->cos_t = c->sin_t = nullptr;
     c->inside = nullptr; c->mom_force = c->mom_torque = nullptr; c->flag_dev = nullptr;
@@ -734,18 +284,20 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         if (flag) return fail(c, MM_ERR_UNSTABLE, "dt violates the positivity bound S8");
         c->checked_dt = dt;
     }
-    // kernel choice: 0 auto (coefficient form when the grid/flags are supported; else generic),
-    // 1 generic, 2 warp-streamed (1-D TMA), 3 tile, 4 coefficient form (same grids/flags as 2)
+    // kernel choice: 0 auto (the upwind-sparse tensor-memory kernel when the grid/flags are supported; else generic),
+    // 1 generic, 2 warp-streamed (1-D TMA), 3 tile, 4 coefficient form, 5 upwind-sparse / tensor memory (same
+    // grids/flags as 2)
     int kind = c->opt_kernel;
-    if (kind == 0) kind = (stream_supported(c) && !(c->coupled && (c->g.nx > 32767 || c->g.ny > 32767))) ? 4 : 1;
-    if (c->coupled && kind == 4 && (c->g.nx > 32767 || c->g.ny > 32767))
-        return fail(c, MM_ERR_INVALID_ARG, "the coupled coefficient-form kernel needs nx, ny <= 32767");
-    if (c->coupled && kind != 1 && kind != 4)
-        return fail(c, MM_ERR_INVALID_ARG, "the free-motor coupled source runs on the coefficient-form or generic kernels (MM_OPT_KERNEL 0, 1 or 4)");
-    if (c->single && !(kind == 4 && stream_supported(c)))
+    if (kind == 0) kind = (stream_supported(c) && !(c->coupled && (c->g.nx > 32767 || c->g.ny > 32767))) ? MM_AUTO_KERNEL : 1;
+    const bool fast = kind == 4 || kind == 5;   // the two coefficient-form families: coupled source, in-place passes
+    if (c->coupled && fast && (c->g.nx > 32767 || c->g.ny > 32767))
+        return fail(c, MM_ERR_INVALID_ARG, "the coupled coefficient-form kernels need nx, ny <= 32767");
+    if (c->coupled && kind != 1 && !fast)
+        return fail(c, MM_ERR_INVALID_ARG, "the free-motor coupled source runs on the coefficient-form or generic kernels (MM_OPT_KERNEL 0, 1, 4 or 5)");
+    if (c->single && !(fast && stream_supported(c)))
         return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context runs only the in-place coefficient-form / fused RK2 kernels (16x16 or 8x8 offset planes, no test flags)");
     if (kind == 2 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "streamed kernel does not support this grid/flags");
-    if (kind == 4 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernel does not support this grid/flags");
+    if (fast && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernels do not support this grid/flags");
     if (kind == 3 && !c->tile_ok) return fail(c, MM_ERR_INVALID_ARG, "tile kernel does not support this grid/flags");
     c->mom_valid = false;
     if (c->p.flags & MM_FLAG_RK2_SUPERBEE) {
@@ -753,9 +305,12 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         if (c->opt_kernel != 0 && c->opt_kernel != 1)
             return fail(c, MM_ERR_INVALID_ARG, "RK2 + Superbee runs on kernel 0 (auto) or 1 (generic)");
         const bool fused = c->opt_kernel == 0 && stream_supported(c) && !c->coupled;
+        // the generic stages write m* into the spare buffer: a single-buffer context has none
+        if (c->single && !fused)
+            return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context runs RK2 + Superbee only on the fused in-place kernel (no coupled source, 16x16 or 8x8 offset planes)");
         for (int n = 0; n < n_sub; ++n) {
             mm_status s = fused ? launch_rk2_fused_any(c, dt)
-                                : c->dtype == MM_F64 ? launch_rk2_generic<double>(c, dt) : launch_rk2_generic<float>(c, dt);
+                                : launch_rk2_generic(c, dt);
             if (s != MM_OK) return s;
         }
         return MM_OK;
@@ -770,19 +325,22 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         } else {
             // balanced passes: as few as the fuse depth allows, of equal depth (10 substeps at depth 6 = 5 + 5)
             int tmax = c->opt_fuse_t;
-            if (kind != 4 && tmax > 4) tmax = 4;   // the streamed / tiled variants are instantiated up to 4
+            if (!fast && tmax > 4) tmax = 4;   // the streamed / tiled variants are instantiated up to 4
+            if (kind == 4 && tmax > 10) tmax = 10;
             if (kind == 4 && tmax > 6 && !(c->dtype == MM_F32 && c->g.nxi == 16)) tmax = 6;   // depth 7-10: fp32 16x16 only
+            if (kind == 5 && tmax > tm_max_levels(c)) tmax = tm_max_levels(c);               // tensor-memory budget
             const int passes_left = (remaining + tmax - 1) / tmax;
             t = (remaining + passes_left - 1) / passes_left;
             const bool mom = c->opt_fuse_mom && remaining == t;
             const bool inpl = c->opt_inplace != 0;
             s = kind == 2   ? launch_stream(c, t, mom, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
                 : kind == 4 ? launch_coef(c, t, mom, dt, c->buf[c->cur], c->buf[inpl ? c->cur : c->cur ^ 1])
+                : kind == 5 ? launch_tm(c, t, mom, dt, c->buf[c->cur], c->buf[inpl ? c->cur : c->cur ^ 1], false, 0, false)
                             : launch_tile(c, t, mom, dt, c->cur, c->buf[c->cur ^ 1]);
             if (s == MM_OK && mom) c->mom_valid = true;
         }
         if (s != MM_OK) return s;
-        if (!(kind == 4 && c->opt_inplace)) c->cur ^= 1;
+        if (!(fast && c->opt_inplace)) c->cur ^= 1;
         remaining -= t;
     }
     return MM_OK;
@@ -819,23 +377,31 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
     c->loc_valid = true;
     c->mom_valid = false;
     // kernel choice: 0 auto = the coefficient-form local-step kernel where the grid is supported, else (or 1) generic
-    if (c->opt_kernel != 0 && c->opt_kernel != 1 && c->opt_kernel != 4)
-        return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local runs on kernel 0 (auto), 1 (generic) or 4 (coefficient form)");
-    if (c->opt_kernel == 4 && !stream_supported(c))
-        return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernel does not support this grid/flags");
+    if (c->opt_kernel != 0 && c->opt_kernel != 1 && c->opt_kernel != 4 && c->opt_kernel != 5)
+        return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local runs on kernel 0 (auto), 1 (generic), 4 (coefficient form) or 5 (upwind-sparse)");
+    if ((c->opt_kernel == 4 || c->opt_kernel == 5) && !stream_supported(c))
+        return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernels do not support this grid/flags");
     if (c->opt_kernel != 1 && stream_supported(c)) {
+        // kernel 5 (and auto): the tensor-memory kernel takes the level count of a configuration at run time, so a pass
+        // fuses up to MM_OPT_FUSE_T local steps; kernel 4: the coefficient-form instances, MM_LOCAL_FUSE_T per pass
+        const bool tm = c->opt_kernel == 5 || (c->opt_kernel == 0 && MM_AUTO_KERNEL == 5);
+        int FT = MM_LOCAL_FUSE_T;
+        if (tm) { FT = c->opt_fuse_t; if (FT > tm_max_levels(c)) FT = tm_max_levels(c); }
+        auto launch_pass = [&](bool mom, const void *in, void *out, int32_t done, bool use_list) {
+            return tm ? launch_tm(c, FT, mom, 1.0, in, out, true, done, use_list) : launch_coef_local(c, mom, in, out, done, use_list);
+        };
         // fp32: passes run IN PLACE on the current buffer and, from the second pass on, visit only the unfinished
         // configurations (compact list built on the device); a configuration writes its moments when it finishes.
         // fp64 (measured: in-place is slower there): ping-pong passes over all configurations,
         // finished ones copied through, moments in the last pass.
-        const int32_t passes = (nmax + MM_LOCAL_FUSE_T - 1) / MM_LOCAL_FUSE_T;
+        const int32_t passes = (nmax + FT - 1) / FT;
         const bool inplace = sizeof(real) == 4 || c->opt_inplace;
         for (int32_t ps = 0; ps < passes; ++ps) {
-            const int32_t done = ps * MM_LOCAL_FUSE_T;
+            const int32_t done = ps * FT;
             mm_status s;
             if (inplace) {
                 // moments are only compiled into the passes in which some configuration can finish
-                const bool mom = c->opt_fuse_mom != 0 && nmin <= done + MM_LOCAL_FUSE_T;
+                const bool mom = c->opt_fuse_mom != 0 && nmin <= done + FT;
                 if (ps > 0) {
                     CUDA_TRY(c, cudaMemsetAsync(c->loc_count, 0, sizeof(int32_t), c->stream));
                     int64_t lb = (c->nc + 255) / 256;
@@ -844,9 +410,9 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
                     CUDA_TRY(c, cudaGetLastError());
                     c->launches++;
                 }
-                s = launch_coef_local(c, mom, c->buf[c->cur], c->buf[c->cur], done, ps > 0);
+                s = launch_pass(mom, c->buf[c->cur], c->buf[c->cur], done, ps > 0);
             } else {
-                s = launch_coef_local(c, c->opt_fuse_mom != 0 && ps == passes - 1, c->buf[c->cur], c->buf[c->cur ^ 1], done, false);
+                s = launch_pass(c->opt_fuse_mom != 0 && ps == passes - 1, c->buf[c->cur], c->buf[c->cur ^ 1], done, false);
                 if (s == MM_OK) c->cur ^= 1;
             }
             if (s != MM_OK) return s;
@@ -879,13 +445,19 @@ extern "C" mm_status mm_advance_local(mm_ctx *c, double dt, double cfl)
         return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local drives the forward-Euler scheme only (no MM_FLAG_RK2_SUPERBEE yet)");
     if (c->coupled) return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local does not take the free-motor coupled source yet");
     if (c->dens_cov_count != c->nc || !c->vel_set) return fail(c, MM_ERR_STATE, "set density and filament velocity first");
-    if (!c->loc_n) {
-        CUDA_TRY(c, cudaMalloc(&c->loc_lambda, (size_t)c->nc * sizeof(double)));
-        CUDA_TRY(c, cudaMalloc(&c->loc_n, (size_t)c->nc * sizeof(int32_t)));
-        CUDA_TRY(c, cudaMalloc(&c->loc_dt, (size_t)c->nc * c->esize));
-        CUDA_TRY(c, cudaMalloc(&c->loc_nmax, 2 * sizeof(int32_t)));
-        CUDA_TRY(c, cudaMalloc(&c->loc_list, (size_t)c->nc * sizeof(int32_t)));
-        CUDA_TRY(c, cudaMalloc(&c->loc_count, sizeof(int32_t)));
+    if (c->nc > INT32_MAX) return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local keeps 32-bit configuration lists: nx*ny*ntheta must be < 2^31");
+    if (!c->loc_count) {   // the group counts as allocated when its LAST member is (a failed call leaves no half group behind)
+        void *g[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+        const size_t bytes[6] = {(size_t)c->nc * sizeof(double), (size_t)c->nc * sizeof(int32_t), (size_t)c->nc * c->esize,
+                                 2 * sizeof(int32_t), (size_t)c->nc * sizeof(int32_t), sizeof(int32_t)};
+        for (int i = 0; i < 6; ++i)
+            if (cudaMalloc(&g[i], bytes[i]) != cudaSuccess) {
+                cudaGetLastError();
+                for (int k = 0; k < i; ++k) cudaFree(g[k]);
+                return fail(c, MM_ERR_NOMEM, "device allocation failed (local-step buffers)");
+            }
+        c->loc_lambda = (double *)g[0]; c->loc_n = (int32_t *)g[1]; c->loc_dt = g[2];
+        c->loc_nmax = (int32_t *)g[3]; c->loc_list = (int32_t *)g[4]; c->loc_count = (int32_t *)g[5];
     }
     return c->dtype == MM_F64 ? advance_local_impl<double>(c, dt, cfl) : advance_local_impl<float>(c, dt, cfl);
 }
@@ -946,9 +518,15 @@ extern "C" mm_status mm_spread_force(mm_ctx *c, double *F2, int on_device)
     if (!c) return MM_ERR_INVALID_ARG;
     if (!F2) return fail(c, MM_ERR_INVALID_ARG, "NULL destination");
     if (c->dens_cov_count != c->nc || !c->psi_set) return fail(c, MM_ERR_STATE, "set density and psi first");
-    if (!c->fline) {
-        CUDA_TRY(c, cudaMalloc(&c->fline, (size_t)c->nc * c->g.ns * 2 * sizeof(double)));
-        CUDA_TRY(c, cudaMalloc(&c->F2, (size_t)c->g.nx * c->g.ny * 2 * sizeof(double)));
+    if (!c->F2) {   // allocated as a pair, committed together
+        void *a = nullptr, *b = nullptr;
+        if (cudaMalloc(&a, (size_t)c->nc * c->g.ns * 2 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&b, (size_t)c->g.nx * c->g.ny * 2 * sizeof(double)) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(a);
+            return fail(c, MM_ERR_NOMEM, "device allocation failed (spreading buffers)");
+        }
+        c->fline = (double *)a; c->F2 = (double *)b;
     }
     mm_status s = c->dtype == MM_F64 ? spread_impl<double>(c) : spread_impl<float>(c);
     if (s != MM_OK) return s;
@@ -990,12 +568,17 @@ extern "C" mm_status mm_update_free_motors(mm_ctx *c, double *Mb_coarse, double 
     if (!c) return MM_ERR_INVALID_ARG;
     if (c->dens_cov_count != c->nc || !c->psi_set) return fail(c, MM_ERR_STATE, "set density and psi first");
     const size_t nn = (size_t)c->g.nx * c->g.ny;
-    if (!c->Mf) {
-        CUDA_TRY(c, cudaMalloc(&c->Mf, nn * sizeof(double)));
-        CUDA_TRY(c, cudaMalloc(&c->Mbc, nn * sizeof(double)));
-        CUDA_TRY(c, cudaMalloc(&c->free_raw, nn * sizeof(double)));
-        CUDA_TRY(c, cudaMalloc(&c->free_factor, nn * sizeof(double)));
-        CUDA_TRY(c, cudaMalloc(&c->free_any, sizeof(int)));
+    if (!c->free_any) {   // allocated as a group, committed together
+        void *g[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+        const size_t bytes[5] = {nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), sizeof(int)};
+        for (int i = 0; i < 5; ++i)
+            if (cudaMalloc(&g[i], bytes[i]) != cudaSuccess) {
+                cudaGetLastError();
+                for (int k = 0; k < i; ++k) cudaFree(g[k]);
+                return fail(c, MM_ERR_NOMEM, "device allocation failed (free-motor tables)");
+            }
+        c->Mf = (double *)g[0]; c->Mbc = (double *)g[1]; c->free_raw = (double *)g[2]; c->free_factor = (double *)g[3];
+        c->free_any = (int *)g[4];
     }
     mm_status s = c->dtype == MM_F64 ? free_impl<double>(c) : free_impl<float>(c);
     if (s != MM_OK) return s;
@@ -1029,7 +612,7 @@ extern "C" mm_status mm_set_option(mm_ctx *c, mm_option opt, int64_t v)
     if (!c) return MM_ERR_INVALID_ARG;
     switch (opt) {
     case MM_OPT_KERNEL:
-        if (v < 0 || v > 4) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_KERNEL in 0..4");
+        if (v < 0 || v > 5) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_KERNEL in 0..5");
         c->opt_kernel = (int)v; return MM_OK;
     case MM_OPT_FUSE_T:
         if (v < 1 || v > MM_MAX_FUSE_T) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_FUSE_T in 1..MM_MAX_FUSE_T");

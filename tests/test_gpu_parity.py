@@ -273,6 +273,127 @@ def test_coef_dirty_masked_input_is_dropped():
     assert p1_density(out, ref) < TOL["f64"]
 
 
+# ------------------------------------------------------------------ upwind-sparse tensor-memory kernel (mm_tm.cuh)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("T", [1, 2, 3, 4, 5, 6, 7, 9, 10, 12])
+@pytest.mark.parametrize("nxi", [16, 8])
+def test_tm_kernel_parity(dtype, T, nxi):
+    # Ns=7: ragged last chunk; 700 configurations: several per warp; odd and even depths (the level loop is rolled by two)
+    g = Grid(5, 7, 20, 7, nxi, nxi)
+    p = Params()
+    e, info = check_parity(g, p, dtype, [2 * T + 3, T] if T > 4 else [5, 3], _dt(g, p), kernel=5, fuse_t=T)
+    assert info["kernel"].startswith("tm<"), info
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_tm_every_upwind_variant(dtype):
+    """The 9 straight-line variants of the level loop: per configuration (U, V) is chosen so that the xi (eta) face
+    velocities are all positive, all negative or of mixed sign over the whole plane; Omega = 0 keeps the choice the
+    same on every plane, Omega != 0 lets it change from plane to plane."""
+    g = Grid(6, 6, 8, 9, 16, 16)
+    p = Params()
+    dt = 0.12 * _dt(g, p)
+    U, V, Om, m0 = random_inputs(g, p, dtype)
+    sel = np.arange(g.nc)
+    big = np.array([-2.5, 0.0, 2.5])
+    U = np.where((sel % 3) == 1, U, big[sel % 3]).astype(U.dtype)
+    V = np.where(((sel // 3) % 3) == 1, V, big[(sel // 3) % 3]).astype(V.dtype)
+    Om = np.where((sel // 9) % 2 == 0, 0.0, Om).astype(Om.dtype)
+    out, moms, info = gpu_run(g, p, dtype, U, V, Om, m0, [6, 5], dt, kernel=5, fuse_t=6)
+    ref, om = oracle_run(g, p, U, V, Om, m0, [6, 5], dt)
+    assert info["kernel"].startswith("tm<"), info
+    assert p1_density(out, ref) <= TOL[dtype]
+    from util import p2_moments
+    for (f, t), r in zip(moms, om):
+        ef, et = p2_moments(f, t, r)
+        assert ef <= TOL[dtype] and et <= TOL[dtype]
+    # and the skipping is exact: the coefficient-form kernel, which multiplies by the zeros, agrees to rounding
+    out4, _, _ = gpu_run(g, p, dtype, U, V, Om, m0, [6, 5], dt, kernel=4, fuse_t=6)
+    assert p1_density(out, out4) <= (1e-13 if dtype == "f64" else 5e-5)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_tm_many_configs_per_warp(dtype):
+    g = Grid(16, 16, 16, 6, 8, 8)   # 4096 configs of 384 cells
+    p = Params()
+    check_parity(g, p, dtype, [4], _dt(g, p), kernel=5, fuse_t=2)
+    g = Grid(16, 16, 24, 5, 16, 16)   # 6144 configurations: more than the 2368 resident warps of the fp32 launch
+    check_parity(g, p, dtype, [7], _dt(g, p), kernel=5, fuse_t=7)
+
+
+def test_tm_equals_generic_and_fusion_invariance():
+    g = Grid(3, 3, 8, 10, 16, 16)
+    p = Params()
+    dt = _dt(g, p)
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    ref, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [7], dt, kernel=1)
+    for T in (1, 2, 3, 4, 7):
+        out, _, info = gpu_run(g, p, "f64", U, V, Om, m0, [7], dt, kernel=5, fuse_t=T)
+        assert p1_density(out, ref) < 1e-13, (T, info)
+    a, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [3, 4], dt, kernel=5, fuse_t=2)
+    b, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [7], dt, kernel=5, fuse_t=2)
+    assert p1_density(a, b) < 1e-13
+
+
+def test_tm_moments_fused_equals_standalone():
+    g = Grid(2, 3, 8, 12, 16, 16)
+    p = Params()
+    dt = _dt(g, p)
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    _, mf, _ = gpu_run(g, p, "f64", U, V, Om, m0, [4, 4], dt, kernel=5, fuse_t=2, fuse_mom=1)
+    _, ms, _ = gpu_run(g, p, "f64", U, V, Om, m0, [4, 4], dt, kernel=5, fuse_t=2, fuse_mom=0)
+    for (f1, t1), (f2, t2) in zip(mf, ms):
+        assert np.allclose(f1, f2, rtol=0, atol=1e-14) and np.allclose(t1, t2, rtol=0, atol=1e-14)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_tm_stall_clamp_wide_ends_and_omega2(dtype):
+    g = Grid(2, 2, 8, 9, 16, 16)
+    p = Params(k_spring=200.0, n_end_cells=2, end_detach_mult=3.0)
+    check_parity(g, p, dtype, [6], 0.25 * _dt(g, p, 2.0), omega_max=2.0, kernel=5, fuse_t=3)
+
+
+def test_tm_zero_rates_and_zero_speed():
+    g = Grid(1, 2, 8, 8, 16, 16)
+    p = Params(k_on=0.0, v0=0.0, k_spring=0.0)
+    check_parity(g, p, "f64", [5], _dt(g, Params()), kernel=5, fuse_t=2)
+
+
+def test_tm_dirty_masked_input_is_dropped():
+    g = Grid(1, 2, 4, 6, 16, 16)
+    p = Params()
+    dt = _dt(g, p)
+    U, V, Om, m0 = random_inputs(g, p, "f64")
+    m0 = m0.copy(); m0[:, :, ~mi.inside_mask(16, 16)] = 3.0
+    out, _, _ = gpu_run(g, p, "f64", U, V, Om, m0, [2], dt, kernel=5, fuse_t=2)
+    ref, _ = oracle_run(g, p, U, V, Om, m0, [2], dt)
+    assert p1_density(out, ref) < TOL["f64"]
+
+
+def test_two_contexts_back_to_back_share_no_launch_state():
+    """Launch shapes are cached per context (no process-wide statics): contexts of different dtype and offset plane,
+    alive at the same time and used alternately, each run their own kernels."""
+    from paper_1908_04279_b200 import MM
+    ga, gb = Grid(2, 2, 8, 6, 16, 16), Grid(3, 2, 8, 5, 8, 8)
+    p = Params()
+    runs = []
+    for g, dtype in ((ga, "f32"), (gb, "f64")):
+        U, V, Om, m0 = random_inputs(g, p, dtype)
+        mm = MM(g, p, dtype)
+        mm.set_density(m0); mm.set_filament_velocity(U, V, Om)
+        runs.append((g, dtype, mm, U, V, Om, m0))
+    for rep in range(2):
+        for g, dtype, mm, *_ in runs:
+            mm.substep(3, _dt(g, p))
+    for g, dtype, mm, U, V, Om, m0 in runs:
+        from util import NPDT
+        out = np.empty((g.nc, g.ns, g.nxi, g.neta), NPDT[dtype])
+        mm.get_density(out)
+        mm.destroy()
+        ref, _ = oracle_run(g, p, U, V, Om, m0, [6], _dt(g, p))
+        assert p1_density(out, ref) <= TOL[dtype]
+
+
 # ------------------------------------------------------------------ in-place passes / single-buffer contexts
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("mode", ["option", "single"])

@@ -107,3 +107,80 @@ def test_n5_translation():
     assert np.max(np.abs(Mbc2 - np.roll(Mbc, (2, 1), axis=(0, 1)))) < 1e-15
     assert (Mbc < 0.07).any() and (Mbc == 0.07).any()          # some nodes capped, some not
     assert np.max(np.abs(out2.reshape(m5.shape) - np.roll(out.reshape(m5.shape), (2, 1), axis=(0, 1)))) < 1e-13
+
+
+def _anchor_nodes_exact(g, R):
+    """Node of every cell's anchor r0 = x_c + s_j p_c - (xi_a, eta_b) (readings Q38/Q39) in EXACT rational arithmetic,
+    for ntheta = 4 (cos, sin in {0, +-1}): written from the definition, not from the oracle's floating-point
+    expression.  Returns int arrays (node_x, node_y) of shape [nx][ny][4][ns][nxi][neta]; asserts that no anchor is a tie."""
+    from fractions import Fraction as Fr
+    assert g.ntheta == 4
+    cs = [(1, 0), (0, 1), (-1, 0), (0, -1)]
+    R = Fr(R).limit_denominator(1000)
+    nodx = np.empty((g.nx, g.ny, 4, g.ns, g.nxi, g.neta), np.int64)
+    nody = np.empty_like(nodx)
+    for ix in range(g.nx):
+        for iy in range(g.ny):
+            for k, (c, s) in enumerate(cs):
+                for j in range(g.ns):
+                    sj = Fr(-1, 2) + Fr(2 * j + 1, 2 * g.ns)
+                    for a in range(g.nxi):
+                        xi = -R + Fr(2 * a + 1, 2) * (2 * R / g.nxi)
+                        rx = (Fr(ix, g.nx) + sj * c - xi) * g.nx + Fr(1, 2)
+                        assert rx.denominator != 1 or True
+                        assert (rx - Fr(1, 2)).denominator != 2, "tie"
+                        for b in range(g.neta):
+                            eta = -R + Fr(2 * b + 1, 2) * (2 * R / g.neta)
+                            ry = (Fr(iy, g.ny) + sj * s - eta) * g.ny + Fr(1, 2)
+                            assert (ry - Fr(1, 2)).denominator != 2, "tie"
+                            nodx[ix, iy, k, j, a, b] = (rx.numerator // rx.denominator) % g.nx
+                            nody[ix, iy, k, j, a, b] = (ry.numerator // ry.denominator) % g.ny
+    return nodx, nody
+
+
+def test_n6_one_hot_table_feeds_exactly_the_cells_anchored_on_that_node():
+    """Eq. 4's source k_on M_f(r0) 1_{D_rc} with Eq. 6: with M_f = delta(node n*), m0 = 0, no
+    transport and no detachment, ONE Euler substep puts dt k_on into exactly the cells whose anchor is n* and leaves
+    every other cell 0.  Pins WHICH node `mmo_run_coupled` reads for a cell: by hand on N1's geometry (plane j = 2 of
+    configuration (3, 5, theta = 0) on the 8x8 grid, R = 0.2: cells (a,b) = (0,0), (0,1), (1,0), (1,1) are anchored on
+    (5,6), (5,4), (3,6), (3,4)), then for every node of a NON-SQUARE grid against exact rational arithmetic, and on a
+    slice of configurations (c_first != 0)."""
+    dt = 0.125
+    # (1) by hand, N1's geometry
+    g = Grid(8, 8, 4, 4, 2, 2)
+    p = Params(R=0.2, v0=0.0, k_off0=0.0, k_on=5.0)
+    z = np.zeros(g.nc)
+    m0 = np.zeros((g.nc, g.ns, 2, 2))
+    c = (3 * g.ny + 5) * g.ntheta
+    for (a, b), (nx_, ny_) in {(0, 0): (5, 6), (0, 1): (5, 4), (1, 0): (3, 6), (1, 1): (3, 4)}.items():
+        Mf = np.zeros((8, 8)); Mf[nx_, ny_] = 1.0
+        out = orc.run_coupled(g, p, z, z, z, m0, 1, dt, Mf)
+        assert out[c, 2, a, b] == dt * 5.0, (a, b)
+        others = [(aa, bb) for aa in range(2) for bb in range(2) if (aa, bb) != (a, b)]
+        assert all(out[c, 2, aa, bb] == 0.0 for aa, bb in others)
+        # theta = 0: the head of plane j sits 8 s_j = -3, -1, 1, 3 nodes from x_c, so node (5,6) is also reached from
+        # other planes / configurations, but in total by ns * (cells per plane) * ntheta cells, every one with dt k_on
+        assert np.count_nonzero(out) == g.ns * 4 * g.ntheta and set(np.unique(out)) == {0.0, dt * 5.0}
+    # (2) every node of a non-square grid (an ix/iy swap cannot survive), exact rational expectation; 4x4 offsets,
+    # corners masked: the source is k_on M_f 1_disc
+    g = Grid(8, 4, 4, 4, 4, 4)
+    p = Params(R=0.2, v0=0.0, k_off0=0.0, k_on=5.0)
+    nodx, nody = _anchor_nodes_exact(g, 0.2)
+    nodx = nodx.reshape(g.nc, g.ns, g.nxi, g.neta); nody = nody.reshape(g.nc, g.ns, g.nxi, g.neta)
+    inside = mi.inside_mask(g.nxi, g.neta).astype(bool)
+    assert not inside[0, 0] and inside[1, 1]
+    z = np.zeros(g.nc)
+    m0 = np.zeros((g.nc, g.ns, g.nxi, g.neta))
+    Mf = RNG.random((g.nx, g.ny)) + 0.5                          # all nodes at once: distinct values identify the node
+    out = orc.run_coupled(g, p, z, z, z, m0, 1, dt, Mf)
+    expect = np.where(inside[None, None], dt * (5.0 * Mf[nodx, nody]), 0.0)
+    assert np.array_equal(out, expect)
+    for n_star in ((5, 2), (0, 3), (7, 0)):
+        one = np.zeros((g.nx, g.ny)); one[n_star] = 1.0
+        out = orc.run_coupled(g, p, z, z, z, m0, 1, dt, one)
+        hit = (nodx == n_star[0]) & (nody == n_star[1]) & inside[None, None]
+        assert hit.any() and np.array_equal(out, np.where(hit, dt * 5.0, 0.0))
+    # (3) a slice of configurations: the node follows the GLOBAL configuration index
+    c0, n = 37, 29
+    out = orc.run_coupled(g, p, z[:n], z[:n], z[:n], m0[c0:c0 + n], 1, dt, Mf, c_first=c0)
+    assert np.array_equal(out, expect[c0:c0 + n])
