@@ -132,9 +132,9 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->Mf = c->Mbc = c->free_raw = c->free_factor = nullptr; c->free_any = nullptr; c->coupled = false;
     c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
-    // measured defaults: the coefficient-form kernel, at most 10 (fp32; 6 off the 16x16
-    // offset plane) / 5 (fp64) substeps per pass
-    c->opt_kernel = 0; c->opt_fuse_t = dtype == MM_F64 ? 5 : 10; c->opt_fuse_mom = 1;
+    // measured defaults: the upwind-sparse tensor-memory kernel, at most MM_MAX_FUSE_T
+    // substeps per pass (with MM_AUTO_KERNEL = 4: the coefficient-form kernel at depth 10 / 5)
+    c->opt_kernel = 0; c->opt_fuse_t = MM_AUTO_KERNEL == 5 ? MM_MAX_FUSE_T : (dtype == MM_F64 ? 5 : 10); c->opt_fuse_mom = 1;
     c->single = (b0 != nullptr && b1 == nullptr);
     c->opt_inplace = c->single ? 1 : 0;
     c->checked_dt = NAN; c->launches = 0; c->kname[0] = 0;

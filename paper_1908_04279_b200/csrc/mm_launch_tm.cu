@@ -38,14 +38,14 @@ struct TmShape {
     using Cfg = TmCfg<real, NXI, NETA, CB, P, D, WARPS, MINB>;
 };
 
-template <typename real, int NXI, int NETA, int CB, bool MF>
-static mm_status launch_tm_inst(mm_ctx *c, int nlev, bool mom, double dt, const void *in, void *out, bool local, int32_t done,
-                                bool use_list)
+template <typename real, int NXI, int NETA, int CB, bool MF, bool LOC>
+static mm_status launch_tm_inst(mm_ctx *c, int nlev, bool mom, double dt, const void *in, void *out, int32_t done, bool use_list)
 {
+    constexpr bool local = LOC;
     using S = TmShape<real, NXI, NETA, CB>;
     using Cfg = typename S::Cfg;
     constexpr int WARPS = S::WARPS;
-    auto kern = substep_tm_kernel<real, NXI, NETA, CB, S::P, S::D, WARPS, S::MINB, MF>;
+    auto kern = substep_tm_kernel<real, NXI, NETA, CB, S::P, S::D, WARPS, S::MINB, MF, LOC>;
     if (nlev < 1 || nlev > Cfg::TMAX) return fail(c, MM_ERR_INVALID_ARG, "fuse depth beyond the tensor-memory budget of the kernel");
     // MF: the warps' node tables (16-bit, ns * (NXI + NETA) entries each) sit behind the regular layout
     const size_t smem = MF ? ((Cfg::SMEM_BYTES + 15) / 16) * 16 + (size_t)WARPS * c->g.ns * (NXI + NETA) * 2 : Cfg::SMEM_BYTES;
@@ -89,8 +89,11 @@ template <typename real, int NXI, int NETA, int CB>
 static mm_status launch_tm_shape(mm_ctx *c, int nlev, bool mom, double dt, const void *in, void *out, bool local, int32_t done,
                                  bool use_list)
 {
-    return c->coupled ? launch_tm_inst<real, NXI, NETA, CB, true>(c, nlev, mom, dt, in, out, local, done, use_list)
-                      : launch_tm_inst<real, NXI, NETA, CB, false>(c, nlev, mom, dt, in, out, local, done, use_list);
+    if (local)
+        return c->coupled ? launch_tm_inst<real, NXI, NETA, CB, true, true>(c, nlev, mom, dt, in, out, done, use_list)
+                          : launch_tm_inst<real, NXI, NETA, CB, false, true>(c, nlev, mom, dt, in, out, done, use_list);
+    return c->coupled ? launch_tm_inst<real, NXI, NETA, CB, true, false>(c, nlev, mom, dt, in, out, done, use_list)
+                      : launch_tm_inst<real, NXI, NETA, CB, false, false>(c, nlev, mom, dt, in, out, done, use_list);
 }
 
 mm_status launch_tm(mm_ctx *c, int nlev, bool mom, double dt, const void *in, void *out, bool local, int32_t done, bool use_list)

@@ -194,7 +194,8 @@ __device__ __forceinline__ void tm_level(const TmCoef<real, QA, CB> &k, const re
 }
 
 // All `nlev` levels of one plane, in place in x.  The loop is rolled by two: the plane values alternate between x and
-// y, so no register copies are needed (an odd count ends with one copy per plane).
+// y, so no register copies are needed (an odd count ends with one copy per plane).  Rolled by four it runs at less than
+// half the speed: 9 variants x 7 level bodies no longer fit the instruction cache (profiles/r02a_README.md).
 template <int SK, typename real, int QA, int CB, int LB, int CPL>
 __device__ __forceinline__ void tm_plane(const TmCoef<real, QA, CB> &k, real (&x)[QA][CB], uint32_t tbase, int nlev)
 {
@@ -214,10 +215,10 @@ __device__ __forceinline__ void tm_plane(const TmCoef<real, QA, CB> &k, real (&x
     }
 }
 
-// nlev: substeps this pass fuses (<= TmCfg::TMAX); mom: also reduce the S9 moments.  Local-step mode (n_steps != NULL):
+// nlev: substeps this pass fuses (<= TmCfg::TMAX); mom: also reduce the S9 moments.  Local-step mode (LOC):
 // configuration c takes clamp(n_steps[c] - done, 0, nlev) steps of its own size dt_c[c]; `kp` then carries the factors
 // per unit dt; `list` as in mm_coef.cuh.
-template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, int MINB, bool MF>
+template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, int MINB, bool MF, bool LOC>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
     substep_tm_kernel(const __grid_constant__ KParams<real> kp, const real *__restrict__ in, real *__restrict__ out,
                       double *__restrict__ force, double *__restrict__ torque, int nlev_pass, int mom,
@@ -258,7 +259,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     const int g = lane / LB, lb = lane - g * LB;
     const int a0 = g * QA, b0 = lb * CB;
     const bool is_g0 = (g == 0), is_gtop = (g == G - 1), is_l0 = (lb == 0), is_lr = (lb == LB - 1);
-    const bool loc = n_steps != nullptr;
+    constexpr bool loc = LOC;   // compile time: in the global mode the level count stays a kernel argument (uniform)
     real maskf[QA][CB], xiq[QA], etab[CB];
 #pragma unroll
     for (int q = 0; q < QA; ++q) {
