@@ -11,7 +11,10 @@ between steps, as the paper prescribes; step k+1 continues f
 Prints ONE JSON line (rank 0).  `value` = motor-cell updates/s (G/s), whole job, inputs resident in HBM;
 `e2e` = same metric through the same C-ABI calls with pinned HOST buffers for (U,V,Omega) and the moments,
 i.e. the host<->device copies of every macro step inside the timed region.  `roofline` is for the dominant
-kernel (the fused advect+react(+moments) substep kernel), timed live with CUDA events on the library's stream.
+kernel (the fused advect+react(+moments) substep kernel), timed live with CUDA events on the library's stream: it is
+bound by FMA issue ("alu"; peak = mm_measure_fma_peak in the same run); `roofline_hbm` is its HBM side (real DRAM rate of
+the fused pass, the algorithmic rate, the unfused T = 1 point, each also against the nominal 8 TB/s).  `per_config`
+holds short runs of the other single-GPU workloads of BASELINE.json (default run only).
 `--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -159,14 +162,244 @@ def upload_inputs(mm, w, chunk_configs=2048, log=None):
     st.close()
     if log:
         log(f"inputs: {g.cells/1e9:.2f} G cells generated+uploaded in {time.time()-t0:.1f} s")
-    return U, V, Om
 
 
 # --------------------------------------------------------------------------------------------- CUDA arm
+FMA_PER_CELL_UPDATE = 6     # S7 in coefficient form: self + s-upwind + four offset neighbours
+NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s"
+
+
+def kernel_evidence(idx, kname):
+    """DRAM bytes per launch and executed instructions per cell-update of this kernel family on this workload, from the
+    committed `ncu --set full` captures (profiles/traffic.json); None where no capture of THIS kernel exists."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            tr = json.load(f).get(f"configs[{idx}]", {}).get(kname.split("<")[0])
+    except Exception:
+        tr = None
+    return tr or {}
+
+
+def measure(mm, w, idx, args, steps, warmup, dev, stream, world, log, full_protocol):
+    """Time `steps` macro steps of workload w on the context mm (density already uploaded).  Returns the pieces of the
+    JSON line: value, e2e, rooflines, launches, clocks."""
+    import torch
+    from paper_1908_04279_b200 import binding as b, shard
+
+    g, es = w.grid, ES[w.dtype]
+    Uh, Vh, Oh = mi.Stream(g, w.params.R, w.seed, w.omega_max).velocities(np.float64 if w.dtype == "f64" else np.float32)
+    n_mom = w.n_sub // w.moments_every
+    Ud, Vd, Od = (torch.from_numpy(x).to(dev) for x in (Uh, Vh, Oh))          # device-resident inputs for `value`
+    Fd = torch.empty((n_mom, g.nc, 2), dtype=torch.float64, device=dev)
+    Td = torch.empty((n_mom, g.nc), dtype=torch.float64, device=dev)
+    Up, Vp, Op = (torch.from_numpy(x).pin_memory() for x in (Uh, Vh, Oh))      # pinned host buffers for `e2e`
+    Fp = torch.empty((n_mom, g.nc, 2), dtype=torch.float64).pin_memory()
+    Tp = torch.empty((n_mom, g.nc), dtype=torch.float64).pin_memory()
+    sub_events = []   # (start, stop, n_sub) around every mm_substep call of the timed region
+
+    if args.full and full_protocol:   # the whole microscale step of Alg. 2 on this path: NEXT-2 + A0-A4 + NEXT-4
+        psi_full = torch.rand(g.nc, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(7))
+        mm.set_psi(psi_full)
+        F2_full = torch.empty((g.nx, g.ny, 2), dtype=torch.float64, device=dev)
+    full = args.full and full_protocol
+    local_dt = args.local_dt and full_protocol
+
+    def step(U, V, Om, F, T, record=False):
+        mm.set_filament_velocity(U, V, Om)                                  # A0
+        for k in range(n_mom):
+            if full:
+                mm.update_free_motors(None, None)                           # NEXT-2: M_b,coarse, cap, M_f
+            if record:
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                lc0 = mm.launch_count
+            if local_dt:   # NEXT-3: same macro interval, every configuration with its own local steps
+                mm.advance_local(w.moments_every * w.dt, args.cfl)
+            else:
+                mm.substep(w.moments_every, w.dt)                           # A1-A3 (+A4 fused into the last pass)
+            if record:
+                e1.record(stream)
+                sub_events.append((e0, e1, w.moments_every, mm.launch_count - lc0))
+            mm.moments(F[k], T[k])                                          # A4
+            if full:
+                mm.spread_force(F2_full)                                    # NEXT-4: Eq. 10
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(nsteps, U, V, Om, F, T, record=False):
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = mm.launch_count
+        e0.record(stream)
+        for _ in range(nsteps):
+            step(U, V, Om, F, T, record)
+        e1.record(stream)
+        barrier()
+        return shard.max_over_ranks(e0.elapsed_time(e1), dev), mm.launch_count - l0
+
+    # ---- warm-up, then the timed region (inputs resident in HBM)
+    for _ in range(max(warmup, 0)):
+        step(Ud, Vd, Od, Fd, Td)
+    sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else dev.index)
+    sampler.start()
+    ms, launches = timed(steps, Ud, Vd, Od, Fd, Td, record=True)
+    clocks = sampler.stop()
+    kname = mm.kernel_name
+    units_rank_step = g.cells * w.n_sub          # cell-updates one rank performs per step
+    local_info = None
+    if local_dt:
+        n_c = torch.empty(g.nc, dtype=torch.int32, device=dev)
+        mm.local_steps(n_c, None)
+        n_sum, n_max = int(n_c.sum().item()), int(n_c.max().item())
+        units_rank_step = g.inner * n_sum * n_mom
+        local_info = {"macro_dt": w.moments_every * w.dt, "cfl": args.cfl, "n_c_mean": round(n_sum / g.nc, 3),
+                      "n_c_max": n_max, "n_c_min": int(n_c.min().item()),
+                      "global_step_equivalent": round(g.cells * w.n_sub * world * steps / (ms * 1e-3) / 1e9, 2),
+                      "note": "value counts the cell-updates actually performed (sum of n_c); global_step_equivalent "
+                              "= rate at which the same physical time would need the global-dt substeps"}
+    updates_per_step = units_rank_step * world
+    value = shard.whole_job_rate(units_rank_step, steps, world, ms) / 1e9
+
+    # ---- dominant kernel: average launch duration over the timed region (CUDA events on the library's stream)
+    sub_ms = sum(a.elapsed_time(c) for a, c, _, _ in sub_events)
+    sub_n = sum(n for _, _, n, _ in sub_events)
+    fuse_opt = mm.get_option(b.MM_OPT_FUSE_T)
+    m = __import__("re").search(r"T(?:<=|=)(\d+)", kname)
+    fuse_t = 1 if args.scheme == "rk2" else (int(m.group(1)) if m else fuse_opt)   # depth of the launches actually made
+    # launches of the pass kernel: counted by the library (local-step mode adds one rate + list kernel per pass: the
+    # full-density passes are ceil(n_c_max / depth) per call)
+    n_launch = sum(l for _, _, _, l in sub_events)
+    if local_dt:
+        n_launch = -(-local_info["n_c_max"] // max(fuse_t, 1)) * len(sub_events)
+    cell_updates = float(g.cells) * sub_n if not local_dt else float(units_rank_step) / n_mom * len(sub_events)
+    sub_s = sub_ms * 1e-3
+    ev = kernel_evidence(idx, kname)
+    # (1) the roof the fused kernel sits under: FMA issue (no tensor cores: 7-point stencil + reduction)
+    fma_peak = b.measure_fma_peak(w.dtype, stream.cuda_stream)             # TFLOP/s, register-only probe, this run
+    nominal_fma = 148 * (64 if w.dtype == "f64" else 128) * 2 * 1.965e9 / 1e12
+    alu_tflops = 2.0 * FMA_PER_CELL_UPDATE * cell_updates / sub_s / 1e12
+    roofline = {"bound": "alu", "kernel": kname, "achieved": round(alu_tflops, 3), "peak": round(fma_peak, 3),
+                "unit": "TFLOP/s", "frac": round(alu_tflops / fma_peak, 4), "traffic": ev.get("dram_bytes_per_launch"),
+                "peak_source": f"measured in this run: mm_measure_fma_peak({w.dtype}), register-only FMA probe on all SMs",
+                "peak_nominal": round(nominal_fma, 2),
+                "peak_nominal_derivation": "148 SMs x %d FMA lanes x 2 flops x 1.965 GHz" % (64 if w.dtype == "f64" else 128),
+                "flops_per_cell_update": 2 * FMA_PER_CELL_UPDATE,
+                "executed_inst_per_cell_update": ev.get("inst_per_cell_update"),
+                "traffic_source": ev.get("source"), "fuse_T": fuse_t, "launches": n_launch,
+                "avg_launch_ms": round(sub_ms / max(n_launch, 1), 4), "kernel_share_of_step": round(sub_ms / ms, 4),
+                "note": "achieved = the method's 6 FMAs per cell-update (12 flops) x cell-updates of the timed mm_substep calls / "
+                        "their CUDA-event time; the fused kernel moves one read + one write of the density per fuse_T substeps "
+                        "and is bound by FMA issue, not HBM (roofline_hbm); a three-register FFMA issues every other cycle "
+                        "(DESIGN.md section 8), so 0.5 is the practical ceiling of frac for fp32"}
+    # (2) the HBM side: real DRAM rate of the fused pass, the algorithmic (T = 1 byte count) rate, the unfused kernel
+    peak, peak_src = measured_peaks()
+    alg_gbs = 2.0 * es * cell_updates / sub_s / 1e9                      # SURVEY.md 8(d): 2*sizeof(real) B per cell-update
+    pass_gbs = 2.0 * es * g.cells * n_launch / sub_s / 1e9               # one fused pass: read once + write once
+    hbm = {"bound": "hbm", "kernel": kname, "achieved": round(pass_gbs, 1), "peak": peak, "unit": "GB/s",
+           "frac": round(pass_gbs / peak, 4), "traffic": ev.get("dram_bytes_per_launch"), "peak_source": peak_src,
+           "frac_nominal_8tbs": round(pass_gbs / NOMINAL_HBM_GBS, 4),
+           "effective_gbs": round(alg_gbs, 1), "effective_frac": round(alg_gbs / peak, 4),
+           "effective_frac_nominal_8tbs": round(alg_gbs / NOMINAL_HBM_GBS, 4), "bytes_per_cell_update": 2 * es,
+           "note": "achieved/frac = bytes the fused passes really move (one read + one write of the density per launch) / time; "
+                   "effective_* = the algorithmic byte count of SURVEY 8(d) (2*sizeof(real) per cell-update, one substep per "
+                   "pass) / time: above 1 because a launch fuses fuse_T substeps, not because memory is faster; t1_* = the "
+                   "same kernel unfused, where both coincide -- north_star's >= 70 % of ~8 TB/s is stated on that point"}
+
+    # ---- the same kernel unfused (T=1) for the T=1 roofline point (outside the timed region)
+    if not args.no_t1 and fuse_t != 1 and not local_dt:
+        mm.set_option(b.MM_OPT_FUSE_T, 1)
+        mm.substep(3, w.dt)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        mm.substep(6, w.dt)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        t1 = 2.0 * es * g.cells * 6 / (e0.elapsed_time(e1) * 1e-3) / 1e9
+        hbm.update({"t1_gbs": round(t1, 1), "t1_frac": round(t1 / peak, 4), "t1_frac_nominal_8tbs": round(t1 / NOMINAL_HBM_GBS, 4),
+                    "t1_kernel": mm.kernel_name})
+        mm.set_option(b.MM_OPT_FUSE_T, fuse_opt)
+
+    extras = {}
+    # ---- optional: NEXT-4 motor-force spreading of the current density (macro cadence; outside the timed region)
+    if args.spread and full_protocol:
+        psi = torch.rand(g.nc, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(7))
+        F2 = torch.empty((g.nx, g.ny, 2), dtype=torch.float64, device=dev)
+        mm.set_psi(psi)
+        mm.spread_force(F2)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(3):
+            mm.spread_force(F2)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        sms = e0.elapsed_time(e1) / 3
+        extras["spread_force"] = {"ms_per_call": round(sms, 3), "density_read_gbs": round(g.cells * es / (sms * 1e-3) / 1e9, 1),
+                                  "density_read_frac": round(g.cells * es / (sms * 1e-3) / 1e9 / peak, 4),
+                                  "point_forces_per_call": g.nc * g.ns, "grid": [g.nx, g.ny]}
+
+    # ---- optional: NEXT-2 free-motor coupling (macro cadence; outside the timed region; needs two buffers)
+    if args.free and full_protocol:
+        psi = torch.rand(g.nc, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(7))
+        mm.set_psi(psi)
+        Mf = torch.empty((g.nx, g.ny), dtype=torch.float64, device=dev)
+        mm.update_free_motors(None, Mf)
+        torch.cuda.synchronize()
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record(stream)
+        for _ in range(2):
+            mm.update_free_motors(None, Mf)
+        e1.record(stream)
+        mm.substep(w.moments_every, w.dt)        # warm-up of the coupled-source kernels
+        e1b = torch.cuda.Event(enable_timing=True)
+        e1b.record(stream)
+        mm.substep(2 * w.moments_every, w.dt)
+        e2.record(stream)
+        torch.cuda.synchronize()
+        ums = e0.elapsed_time(e1) / 2
+        extras["free_motors"] = {"update_ms_per_call": round(ums, 3),
+                                 "density_read_gbs": round(g.cells * es / (ums * 1e-3) / 1e9, 1),
+                                 "density_read_frac": round(g.cells * es / (ums * 1e-3) / 1e9 / peak, 4),
+                                 "coupled_substep_kernel": mm.kernel_name,
+                                 "coupled_substep_gcups": round(g.cells * 2 * w.moments_every / (e1b.elapsed_time(e2) * 1e-3) / 1e9, 2),
+                                 "Mf_min": float(Mf.min().item()), "Mf_max": float(Mf.max().item())}
+        mm.set_option(b.MM_OPT_FREE_COUPLING, 0)
+
+    # ---- end to end: pinned host (U,V,Omega) in, moments out to pinned host, every step
+    for _ in range(2 if full_protocol else 1):
+        step(Up, Vp, Op, Fp, Tp)
+    ms_e2e, _ = timed(steps, Up, Vp, Op, Fp, Tp)
+    e2e = {"value": round(updates_per_step * steps / (ms_e2e * 1e-3) / 1e9, 2), "unit": UNIT,
+           "h2d_bytes_per_step": int(3 * g.nc * es), "d2h_bytes_per_step": int(n_mom * 3 * g.nc * 8),
+           "ms_per_step": round(ms_e2e / steps, 3),
+           "note": "density is resident state (PAPER.md:133,143); per-step host traffic is (U,V,Omega) in, moments out"}
+    return {"value": value, "ms": ms, "launches": launches, "clocks": clocks, "kname": kname, "e2e": e2e,
+            "roofline": roofline, "roofline_hbm": hbm, "local_info": local_info, "extras": extras}
+
+
+def make_context(w, args, dev, stream, log):
+    import torch
+    from paper_1908_04279_b200 import MM, binding as b
+    tdt = torch.float64 if w.dtype == "f64" else torch.float32
+    b0 = torch.empty(w.grid.cells, dtype=tdt, device=dev)
+    b1 = None if args.single_buffer else torch.empty(w.grid.cells, dtype=tdt, device=dev)
+    mm = MM(w.grid, w.params, w.dtype, b0, b1, stream=stream.cuda_stream)
+    if args.fuse_t:
+        mm.set_option(b.MM_OPT_FUSE_T, args.fuse_t)
+    if args.kernel is not None:
+        mm.set_option(b.MM_OPT_KERNEL, args.kernel)
+    upload_inputs(mm, w, log=log)
+    return mm, (b0, b1)
+
+
 def run_cuda(args):
     import torch
     import torch.distributed as dist
-    from paper_1908_04279_b200 import MM, binding as b, shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -190,222 +423,57 @@ def run_cuda(args):
         w = mi.Workload(w.name + f"_nx{args.nx_mult}", mi.Grid(g0.nx * args.nx_mult, g0.ny, g0.ntheta, g0.ns, g0.nxi, g0.neta),
                         w.dtype, w.n_sub, w.moments_every, w.omega_max, w.seed, w.params)
     g, es = w.grid, ES[w.dtype]
-    tdt = torch.float64 if w.dtype == "f64" else torch.float32
     log(f"workload configs[{idx}] {w.name}: Nc={g.nc} cells={g.cells} dtype={w.dtype} n_sub={w.n_sub} "
         f"moments every {w.moments_every}; dt={w.dt:.6e}")
 
     stream = torch.cuda.current_stream()
-    b0 = torch.empty(g.cells, dtype=tdt, device=dev)
-    b1 = None if args.single_buffer else torch.empty(g.cells, dtype=tdt, device=dev)
-    mm = MM(g, w.params, w.dtype, b0, b1, stream=stream.cuda_stream)
-    if args.fuse_t:
-        mm.set_option(b.MM_OPT_FUSE_T, args.fuse_t)
-    if args.kernel is not None:
-        mm.set_option(b.MM_OPT_KERNEL, args.kernel)
-    Uh, Vh, Oh = upload_inputs(mm, w, log=log)
-
-    n_mom = w.n_sub // w.moments_every
-    # device-resident inputs/outputs for `value`
-    Ud, Vd, Od = (torch.from_numpy(x).to(dev) for x in (Uh, Vh, Oh))
-    Fd = torch.empty((n_mom, g.nc, 2), dtype=torch.float64, device=dev)
-    Td = torch.empty((n_mom, g.nc), dtype=torch.float64, device=dev)
-    # pinned host buffers for `e2e`
-    Up, Vp, Op = (torch.from_numpy(x).pin_memory() for x in (Uh, Vh, Oh))
-    Fp = torch.empty((n_mom, g.nc, 2), dtype=torch.float64).pin_memory()
-    Tp = torch.empty((n_mom, g.nc), dtype=torch.float64).pin_memory()
-
-    sub_events = []   # (start, stop, n_sub) around every mm_substep call of the timed region
-
-    if args.full:   # the whole microscale step of Alg. 2 on this path: NEXT-2 + A0-A4 + NEXT-4
-        psi_full = torch.rand(g.nc, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(7))
-        mm.set_psi(psi_full)
-        F2_full = torch.empty((g.nx, g.ny, 2), dtype=torch.float64, device=dev)
-
-    def step(U, V, Om, F, T, record=False):
-        mm.set_filament_velocity(U, V, Om)                                  # A0
-        for k in range(n_mom):
-            if args.full:
-                mm.update_free_motors(None, None)                           # NEXT-2: M_b,coarse, cap, M_f
-            if record:
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record(stream)
-            if args.local_dt:   # NEXT-3: same macro interval, every configuration with its own local steps
-                mm.advance_local(w.moments_every * w.dt, args.cfl)
-            else:
-                mm.substep(w.moments_every, w.dt)                           # A1-A3 (+A4 fused into the last pass)
-            if record:
-                e1.record(stream)
-                sub_events.append((e0, e1, w.moments_every))
-            mm.moments(F[k], T[k])                                          # A4
-            if args.full:
-                mm.spread_force(F2_full)                                    # NEXT-4: Eq. 10
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def timed(nsteps, U, V, Om, F, T, record=False):
-        barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        l0 = mm.launch_count
-        e0.record(stream)
-        for _ in range(nsteps):
-            step(U, V, Om, F, T, record)
-        e1.record(stream)
-        barrier()
-        ms = shard.max_over_ranks(e0.elapsed_time(e1), dev)
-        return ms, mm.launch_count - l0
-
-    # ---- warm-up, then the timed region (inputs resident in HBM)
-    for _ in range(max(args.warmup, 0)):
-        step(Ud, Vd, Od, Fd, Td)
-    sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else local)
-    sampler.start()
-    ms, launches = timed(args.steps, Ud, Vd, Od, Fd, Td, record=True)
-    clocks = sampler.stop()
-    kname = mm.kernel_name
-    units_rank_step = g.cells * w.n_sub          # cell-updates one rank performs per step
-    local_info = None
-    if args.local_dt:
-        n_c = torch.empty(g.nc, dtype=torch.int32, device=dev)
-        mm.local_steps(n_c, None)
-        n_sum, n_max = int(n_c.sum().item()), int(n_c.max().item())
-        units_rank_step = g.inner * n_sum * n_mom
-        local_info = {"macro_dt": w.moments_every * w.dt, "cfl": args.cfl, "n_c_mean": round(n_sum / g.nc, 3),
-                      "n_c_max": n_max, "n_c_min": int(n_c.min().item()),
-                      "global_step_equivalent": round(g.cells * w.n_sub * world * args.steps / (ms * 1e-3) / 1e9, 2),
-                      "note": "value counts the cell-updates actually performed (sum of n_c); global_step_equivalent "
-                              "= rate at which the same physical time would need the global-dt substeps"}
-    updates_per_step = units_rank_step * world
-    value = shard.whole_job_rate(units_rank_step, args.steps, world, ms) / 1e9
-
-    # ---- dominant kernel: average launch duration over the timed region (CUDA events on the library's stream)
-    sub_ms = sum(a.elapsed_time(c) for a, c, _ in sub_events)
-    sub_n = sum(n for _, _, n in sub_events)
-    fuse_t = 1 if args.scheme == "rk2" else (args.fuse_t or mm.get_option(b.MM_OPT_FUSE_T))
-    launches_per_call = -(-w.moments_every // fuse_t)
-    if args.local_dt:
-        launches_per_call = -(-local_info["n_c_max"] // b.MM_LOCAL_FUSE_T)
-    n_launch = launches_per_call * len(sub_events)
-    peak, peak_src = measured_peaks()
-    alg_bytes = 2.0 * es * g.cells * sub_n                 # 2*sizeof(real) B per cell-update (T=1 count)
-    if args.local_dt:
-        alg_bytes = 2.0 * es * units_rank_step / n_mom * len(sub_events)
-    pass_bytes = 2.0 * es * g.cells * n_launch             # what one fused pass has to move: read once + write once
-    achieved = alg_bytes / (sub_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": kname, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
-                "frac": round(achieved / peak, 4), "traffic": None, "peak_source": peak_src,
-                "bytes_per_cell_update": 2 * es, "fuse_T": fuse_t, "launches": n_launch,
-                "avg_launch_ms": round(sub_ms / n_launch, 4),
-                "pass_gbs": round(pass_bytes / (sub_ms * 1e-3) / 1e9, 1),
-                "pass_frac": round(pass_bytes / (sub_ms * 1e-3) / 1e9 / peak, 4),
-                "kernel_share_of_step": round(sub_ms / ms, 4),
-                "note": "achieved = algorithmic bytes (2*sizeof(real) per cell-update, the one-substep-per-pass count of "
-                        "SURVEY 8(d)) / kernel time; a launch fuses fuse_T substeps into ONE read + ONE write of the density, "
-                        "so frac > 1 is temporal fusion, not a faster memory: pass_gbs/pass_frac = DRAM rate of the pass "
-                        "actually moved (= traffic / time), t1_* = the same kernel unfused"}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(traffic_file):
-        try:
-            with open(traffic_file) as f:
-                tr = json.load(f).get(f"configs[{idx}]", {})
-            roofline["traffic"] = tr.get("dram_bytes_per_launch")
-            roofline["traffic_source"] = tr.get("source")
-        except Exception:
-            pass
-
-    # ---- the same kernel unfused (T=1) for the T=1 roofline point (outside the timed region)
-    if not args.no_t1 and fuse_t != 1 and not args.local_dt:
-        mm.set_option(b.MM_OPT_FUSE_T, 1)
-        mm.substep(3, w.dt)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        e0.record(stream)
-        mm.substep(6, w.dt)
-        e1.record(stream)
-        torch.cuda.synchronize()
-        t1 = 2.0 * es * g.cells * 6 / (e0.elapsed_time(e1) * 1e-3) / 1e9
-        roofline["t1_gbs"] = round(t1, 1)
-        roofline["t1_frac"] = round(t1 / peak, 4)
-        roofline["t1_kernel"] = mm.kernel_name
-        mm.set_option(b.MM_OPT_FUSE_T, fuse_t)
-
-    # ---- optional: NEXT-4 motor-force spreading of the current density (macro cadence; outside the timed region)
-    spread_info = None
-    if args.spread:
-        psi = torch.rand(g.nc, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(7))
-        F2 = torch.empty((g.nx, g.ny, 2), dtype=torch.float64, device=dev)
-        mm.set_psi(psi)
-        mm.spread_force(F2)
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        for _ in range(3):
-            mm.spread_force(F2)
-        e1.record(stream)
-        torch.cuda.synchronize()
-        sms = e0.elapsed_time(e1) / 3
-        spread_info = {"ms_per_call": round(sms, 3), "density_read_gbs": round(g.cells * es / (sms * 1e-3) / 1e9, 1),
-                       "point_forces_per_call": g.nc * g.ns, "atomic_adds_per_call": g.nc * g.ns * 32,
-                       "grid": [g.nx, g.ny]}
-
-    # ---- optional: NEXT-2 free-motor coupling (macro cadence; outside the timed region; needs two buffers)
-    free_info = None
-    if args.free:
-        psi = torch.rand(g.nc, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(7))
-        mm.set_psi(psi)
-        Mf = torch.empty((g.nx, g.ny), dtype=torch.float64, device=dev)
-        mm.update_free_motors(None, Mf)
-        torch.cuda.synchronize()
-        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
-        e0.record(stream)
-        for _ in range(2):
-            mm.update_free_motors(None, Mf)
-        e1.record(stream)
-        mm.substep(w.moments_every, w.dt)        # warm-up of the coupled-source kernels
-        e1b = torch.cuda.Event(enable_timing=True)
-        e1b.record(stream)
-        mm.substep(2 * w.moments_every, w.dt)
-        e2.record(stream)
-        torch.cuda.synchronize()
-        cname = mm.kernel_name
-        free_info = {"update_ms_per_call": round(e0.elapsed_time(e1) / 2, 3), "atomic_adds_per_call": g.cells,
-                     "coupled_substep_kernel": cname,
-                     "coupled_substep_gcups": round(g.cells * 2 * w.moments_every / (e1b.elapsed_time(e2) * 1e-3) / 1e9, 2),
-                     "Mf_min": float(Mf.min().item()), "Mf_max": float(Mf.max().item())}
-        mm.set_option(b.MM_OPT_FREE_COUPLING, 0)
-
-    # ---- end to end: pinned host (U,V,Omega) in, moments out to pinned host, every step
-    for _ in range(2):
-        step(Up, Vp, Op, Fp, Tp)
-    ms_e2e, _ = timed(args.steps, Up, Vp, Op, Fp, Tp)
-    e2e = {"value": round(updates_per_step * args.steps / (ms_e2e * 1e-3) / 1e9, 2), "unit": UNIT,
-           "h2d_bytes_per_step": int(3 * g.nc * es), "d2h_bytes_per_step": int(n_mom * 3 * g.nc * 8),
-           "ms_per_step": round(ms_e2e / args.steps, 3),
-           "note": "density is resident state (PAPER.md:133,143); per-step host traffic is (U,V,Omega) in, moments out"}
+    mm, bufs = make_context(w, args, dev, stream, log)
+    r = measure(mm, w, idx, args, args.steps, args.warmup, dev, stream, world, log, full_protocol=True)
     mm.destroy()
-    del b0, b1
+    del mm, bufs
+    torch.cuda.empty_cache()
 
-    out = {"metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": round(ms / args.steps, 3), "higher_is_better": True,
+    out = {"metric": METRIC, "value": round(r["value"], 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": round(r["ms"] / args.steps, 3), "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": w.dtype, "data": "synthetic",
            "config": {"workload": f"configs[{idx}] {w.name}", "grid": [g.nx, g.ny, g.ntheta, g.ns, g.nxi, g.neta],
                       "cells_per_gpu": g.cells, "n_sub_per_step": w.n_sub, "moments_every": w.moments_every,
                       "dt": w.dt, "seed": w.seed, "parallelism": f"configs x{world} (no collective)",
                       "l2": "inputs larger than L2 (%s of %.1f GB)" % ("one density buffer, passes in place" if args.single_buffer else "two density buffers", g.cells * es / 1e9)},
-           "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "impl": "cuda"}
-    if spread_info:
-        out["spread_force"] = spread_info
-    if free_info:
-        out["free_motors"] = free_info
+           "clocks": r["clocks"], "e2e": r["e2e"], "gpu_launches": int(r["launches"]), "roofline": r["roofline"],
+           "roofline_hbm": r["roofline_hbm"], "impl": "cuda"}
+    out.update(r["extras"])
     if args.full:
         out["config"]["workload"] += "+full_step"
         out["full_step"] = {"per_macro_interval": "mm_update_free_motors, mm_substep (coupled source), mm_moments, mm_spread_force",
-                            "note": "value still counts cell-updates of the substeps only; the roofline object refers to the substep kernel"}
-    if local_info:
+                            "note": "value still counts cell-updates of the substeps only; the roofline objects refer to the substep kernel"}
+    if r["local_info"]:
         out["config"]["workload"] += "+local_dt"
-        out["local_dt"] = local_info
+        out["local_dt"] = r["local_info"]
+
+    # ---- the other single-GPU workloads of BASELINE.json, a few steps each (driver-visible fp64 / medium-grid numbers)
+    plain = not (args.full or args.local_dt or args.single_buffer or args.nx_mult > 1 or args.scheme != "euler")
+    if rank == 0 and world == 1 and plain and not args.no_per_config and args.config is None:
+        per = []
+        for j in range(len(mi.CONFIGS)):
+            if j == idx:
+                continue
+            wj = mi.CONFIGS[j]
+            fb, _ = torch.cuda.mem_get_info()
+            if 2 * wj.grid.cells * ES[wj.dtype] + (2 << 30) > fb:
+                per.append({"workload": f"configs[{j}] {wj.name}", "skipped": "does not fit"})
+                continue
+            mmj, bj = make_context(wj, args, dev, stream, log)
+            rj = measure(mmj, wj, j, args, 2, 1, dev, stream, 1, log, full_protocol=False)
+            mmj.destroy()
+            del mmj, bj
+            torch.cuda.empty_cache()
+            per.append({"workload": f"configs[{j}] {wj.name}", "dtype": wj.dtype, "value": round(rj["value"], 2), "unit": UNIT,
+                        "steps": 2, "warmup": 1, "e2e": rj["e2e"]["value"], "kernel": rj["kname"],
+                        "frac": rj["roofline"]["frac"], "fma_peak_tflops": rj["roofline"]["peak"],
+                        "hbm_pass_frac": rj["roofline_hbm"]["frac"], "t1_frac": rj["roofline_hbm"].get("t1_frac"),
+                        "t1_frac_nominal_8tbs": rj["roofline_hbm"].get("t1_frac_nominal_8tbs"), "clocks": rj["clocks"]})
+        out["per_config"] = per
     if rank == 0 and world == 1 and not args.no_cpu and not args.local_dt:
         out["cpu_baseline"] = cpu_baseline(w, target_s=args.cpu_seconds, log=log)
     if rank == 0:
@@ -448,9 +516,24 @@ def cpu_baseline(w, target_s=15.0, log=None):
     val = n * w.grid.inner * w.n_sub / t / 1e9
     if log:
         log(f"cpu_baseline: oracle on {n} configurations, {t:.1f} s, {val*1e3:.1f} M cell-updates/s on {cores} threads")
-    return {"value": round(val, 5), "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"first {n} of {w.grid.nc} configurations of the workload, all {w.n_sub} substeps + moments "
-                      f"every {w.moments_every}; fp64; gcc -O2 -fopenmp over configurations", "seconds": round(t, 2)}
+    out = {"value": round(val, 5), "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"first {n} of {w.grid.nc} configurations of the workload, all {w.n_sub} substeps + moments "
+                     f"every {w.moments_every}; fp64; gcc -O2 -fopenmp over configurations", "seconds": round(t, 2)}
+    # per-core figure (SURVEY.md 8(d) "additionally with 1 thread on configs[0]"): a child process, OMP_NUM_THREADS=1
+    try:
+        import subprocess
+        code = ("import sys, json; sys.path.insert(0, %r); import bench, mm_inputs as mi; w = mi.CONFIGS[0]; n = 24; "
+                "t = bench.oracle_sample(w, n)[0]; print(json.dumps([n, t]))" % ROOT)
+        res = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300,
+                             env={**os.environ, "OMP_NUM_THREADS": "1"})
+        n1, t1 = json.loads(res.stdout.strip().splitlines()[-1])
+        w0 = mi.CONFIGS[0]
+        out["one_thread_configs0"] = {"value": round(n1 * w0.grid.inner * w0.n_sub / t1 / 1e9, 5), "unit": UNIT, "cores": 1,
+                                      "sample": f"first {n1} of {w0.grid.nc} configurations of configs[0] fp64_tiny, all "
+                                                f"{w0.n_sub} substeps + moments; OMP_NUM_THREADS=1", "seconds": round(t1, 2)}
+    except Exception as e:   # the per-core figure is context: never fail the bench line over it
+        out["one_thread_configs0"] = {"error": str(e)[:200]}
+    return out
 
 
 def run_reference(args):
@@ -519,6 +602,7 @@ def main():
     ap.add_argument("--cfl", type=float, default=0.4, help="CFL number of --local-dt")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-t1", action="store_true", help="skip the unfused (T=1) roofline point")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of the other BASELINE workloads")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     args = ap.parse_args()
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -84,29 +84,34 @@ typedef struct {
 /* Tuning / test options for mm_set_option.  Defaults are what bench.py times. */
 typedef enum {
     MM_OPT_KERNEL = 0,       /* 0 auto (default: the fastest measured variant for the dtype and grid, DESIGN.md
-                                "Kernel selection"); 1 force the generic global-memory kernels (any grid, all
-                                flags); 2 force the warp-streamed 1-D-TMA kernels; 3 force the tiled-TMA kernels;
-                                4 force the coefficient-form kernels (the default where supported)
-                                (2, 3, 4: MM_ERR_INVALID_ARG from mm_substep if the grid/flags are unsupported) */
+                                "Kernel selection": kernel 5 where supported, else 1); 1 force the generic
+                                global-memory kernels (any grid, all flags); 2 force the warp-streamed 1-D-TMA
+                                kernels; 3 force the tiled-TMA kernels; 4 force the coefficient-form kernels
+                                (upwind planes of the fused levels in registers / shared memory); 5 force the
+                                upwind-sparse kernel (carries in tensor memory, run-time fuse depth)
+                                (2..5: MM_ERR_INVALID_ARG from mm_substep if the grid/flags are unsupported) */
     MM_OPT_FUSE_T = 1,       /* max substeps fused per HBM pass (temporal fusion), 1..MM_MAX_FUSE_T; mm_substep uses as
                                 few passes as this allows, of balanced depth (10 substeps at depth 6 = 5 + 5);
-                                default 10 (fp32) / 5 (fp64) */
+                                default MM_MAX_FUSE_T */
     MM_OPT_FUSE_MOMENTS = 2, /* 1 (default): the last pass of mm_substep also reduces the moments, so a
                                 following mm_moments is a copy; 0: mm_moments always runs its own pass */
-    MM_OPT_FREE_COUPLING = 4,/* 1: the source term of the substeps is k_on M_f(r0) from the table of the last
+    MM_OPT_INPLACE = 3,      /* 1: the coefficient-form, upwind-sparse, fused RK2 and local-step kernels update the
+                                current density buffer IN PLACE (plane j of the result depends on input planes <= j
+                                only, each already staged on the SM when plane j is stored, and one warp owns a
+                                configuration), the other buffer is not touched; same results, same speed, half the
+                                memory.  Default 0; always 1 for a context created with ONE density buffer
+                                (mm_create, dens_buf1 = NULL) */
+    MM_OPT_FREE_COUPLING = 4 /* 1: the source term of the substeps is k_on M_f(r0) from the table of the last
                                 mm_update_free_motors (which switches it on); 0: the constant k_on m_free again.
                                 MM_ERR_STATE when set to 1 before any mm_update_free_motors */
-    MM_OPT_INPLACE = 3       /* 1: the coefficient-form, fused RK2 and local-step kernels update the current density
-                                buffer IN PLACE (plane j of the result depends on input planes <= j only, each already
-                                staged on the SM when plane j is stored, and one warp owns a configuration), the other
-                                buffer is not touched; same results, same speed, half the memory.  Default 0; always 1
-                                for a context created with ONE density buffer (mm_create, dens_buf1 = NULL) */
 } mm_option;
-#define MM_MAX_FUSE_T 12  /* fp32 coefficient-form kernels on 16x16 offset planes; other coefficient-form kernels
-                             fuse at most 6, the streamed / tiled variants at most 4 (deeper settings are clamped) */
-#define MM_LOCAL_FUSE_T 4 /* levels per pass of mm_advance_local */
+#define MM_MAX_FUSE_T 12  /* kernel 5 (tensor-memory budget of a warp); kernel 4 fuses at most 10 (fp32, 16x16 offset
+                             planes) / 6, the streamed / tiled variants at most 4 (deeper settings are clamped) */
+#define MM_LOCAL_FUSE_T 4 /* levels per pass of mm_advance_local on kernel 4 (kernel 5 fuses MM_OPT_FUSE_T local steps) */
 
-/* Create a context.
+/* Create a context: the GPU-resident state of the microscale step -- "M_b ... reside[s] only on the GPU" between outer
+ * steps, "only the smaller, coarsened data is transferred to/from main memory"; two density buffers
+ * as the paper keeps two time levels, or one (in-place passes).
  *  grid, params : copied.  Invalid (MM_ERR_INVALID_ARG): any dim < 1, R <= 0, f_stall <= 0,
  *                 f_detach <= 0, s_hi <= s_lo, negative rates/speeds, 2*n_end_cells > ns, non-finite.
  *  dens_buf0/1  : device pointers to two density buffers of >= cells*sizeof(real) bytes each,
@@ -136,8 +141,12 @@ mm_status mm_get_density_range(mm_ctx *ctx, int64_t c_begin, int64_t n_configs, 
  * (the macro-timescale input; "Psi ... is transferred as before"). */
 mm_status mm_set_filament_velocity(mm_ctx *ctx, const void *U, const void *V, const void *Omega, int on_device);
 
-/* n_sub explicit substeps of size dt (S2-S7), asynchronous on the stream.  n_sub >= 0; dt > 0 and finite
- * when n_sub > 0.  MM_ERR_STATE unless density and velocities have been set. */
+/* n_sub explicit substeps of size dt of Eq. 4 (d_t M_b + d_s M_b = -k_off M_b + k_on M_f 1_{D_rc}) for
+ * every unit independently, the inner loop of Alg. 2 l.4-13 with the state staying on the GPU; in
+ * the discretisation BASELINE.json north_star (1)-(2) fixes (S2-S7: first-order upwind in s and (xi, eta),
+ * Bell-law and end detachment, attachment inside the disc, mask).  Asynchronous on the stream.  n_sub >= 0; dt > 0 and
+ * finite when n_sub > 0.  MM_ERR_STATE unless density and velocities have been set; MM_ERR_UNSTABLE with
+ * MM_FLAG_CHECK_DT when dt breaks the positivity bound S8. */
 mm_status mm_substep(mm_ctx *ctx, int32_t n_sub, double dt);
 
 /* local adaptive time step per independent unit ("We instead compute a local
@@ -172,10 +181,10 @@ mm_status mm_spread_force(mm_ctx *ctx, double *F2, int dst_on_device);
  *     M_b,coarse[n] = dtheta ds dxi deta sum_{cells -> n} Psi_c m;      M_total = params.m_free at every node;
  * where M_b,coarse[n] > M_total every cell of node n is scaled by M_total / M_b,coarse[n] (the density IS modified) and
  * M_b,coarse[n] = M_total; M_f[n] = M_total - M_b,coarse[n] >= 0.  The call stores M_f and switches the source of the
- * following substeps to k_on M_f(r0) 1_disc (MM_OPT_FREE_COUPLING), frozen until the next call.  With the coupled
- * source mm_substep runs the coefficient-form kernels (forward Euler on 16x16 / 8x8 offset planes) or the generic
- * kernels (any grid, RK2 + Superbee; two density buffers); mm_advance_local is refused.  Mb_coarse, M_free: [nx][ny] fp64 outputs, either may be NULL.  Needs mm_set_psi.  fp64 atomic adds: the
- * summation order varies from call to call. */
+ * following substeps to k_on M_f(r0) 1_disc (MM_OPT_FREE_COUPLING), frozen until the next call.
+ * With the coupled source mm_substep runs kernels 4 / 5 (forward Euler on 16x16 / 8x8 offset planes) or the generic
+ * kernels (any grid, RK2 + Superbee; two density buffers).
+ * Mb_coarse, M_free: [nx][ny] fp64 outputs, either may be NULL.  Needs mm_set_psi. */
 mm_status mm_update_free_motors(mm_ctx *ctx, double *Mb_coarse, double *M_free, int dst_on_device);
 
 /* Moments (S9) of the current density: force [Nc][2] = (Fx, Fy), torque [Nc]; always fp64
@@ -185,13 +194,19 @@ mm_status mm_moments(mm_ctx *ctx, double *force, double *torque, int dst_on_devi
 mm_status mm_set_option(mm_ctx *ctx, mm_option opt, int64_t value);
 mm_status mm_get_option(const mm_ctx *ctx, mm_option opt, int64_t *value); /* current setting; MM_ERR_INVALID_ARG on NULL / unknown */
 
+/* The second roof of the fused kernels ("measure and record the box's fp64 and fp32 FMA peaks with a
+ * small register-only microbenchmark"): runs a register-only FMA probe of the given dtype on every SM of the current
+ * device (about 10 ms, on the given cudaStream_t, synchronises it) and returns the rate in TFLOP/s (2 flops per FMA).
+ * Needs no context.  MM_ERR_CUDA without a device. */
+mm_status mm_measure_fma_peak(mm_dtype dtype, void *cuda_stream, double *tflops);
+
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t mm_launch_count(const mm_ctx *ctx);
 /* Name of the substep kernel variant the last mm_substep used ("stream<f64,16x16,T=2>", "generic<f64>", ...). */
 const char *mm_kernel_name(const mm_ctx *ctx);
 
-/* Destroy; frees library-owned buffers.  NULL is a no-op.  Does not synchronise borrowed buffers' users
- * beyond the context's own stream. */
+/* Destroy the context (the end of the resident state of PAPER.md:133): synchronises the context's stream, frees
+ * library-owned buffers; borrowed density buffers are left to their owner.  NULL is a no-op. */
 mm_status mm_destroy(mm_ctx *ctx);
 
 const char *mm_status_string(mm_status s);

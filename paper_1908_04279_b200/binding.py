@@ -20,7 +20,7 @@ MM_LOCAL_FUSE_T = 4
 EXPORTS = ["mm_create", "mm_set_density", "mm_get_density", "mm_set_density_range", "mm_get_density_range",
            "mm_set_filament_velocity", "mm_substep", "mm_moments", "mm_set_option", "mm_get_option", "mm_launch_count",
            "mm_kernel_name", "mm_destroy", "mm_status_string", "mm_last_error", "mm_advance_local", "mm_local_steps", "mm_set_psi",
-           "mm_spread_force", "mm_update_free_motors"]
+           "mm_spread_force", "mm_update_free_motors", "mm_measure_fma_peak"]
 
 
 class mm_grid(ctypes.Structure):
@@ -76,6 +76,7 @@ def lib():
         L.mm_status_string.restype = ctypes.c_char_p
         L.mm_last_error.argtypes = [vp]
         L.mm_last_error.restype = ctypes.c_char_p
+        L.mm_measure_fma_peak.argtypes = [ctypes.c_int, vp, ctypes.POINTER(dbl)]
         _lib = L
     return _lib
 
@@ -90,15 +91,50 @@ def _params_struct(p) -> mm_params:
                         "s_lo", "s_hi")), int(p.n_end_cells), int(p.flags))
 
 
-def _ptr(x):
-    """(address, on_device) of a torch tensor / numpy array / None."""
+_DTYPES = {"f32": ("float32", 4), "f64": ("float64", 8), "i32": ("int32", 4)}
+
+
+def _ptr(x, dtype: str | None = None, numel: int | None = None, what: str = "argument"):
+    """(address, on_device) of a torch tensor / numpy array / None.  With dtype ("f32", "f64", "i32") and numel the
+    element type and the element count are checked first: the C ABI takes plain pointers and would otherwise
+    reinterpret a wrong dtype or run past the end of a short array."""
     if x is None:
         return None, 0
-    if hasattr(x, "data_ptr"):  # torch tensor
-        assert x.is_contiguous()
+    torch_like = hasattr(x, "data_ptr")
+    if not (x.is_contiguous() if torch_like else x.flags.c_contiguous):
+        raise ValueError(f"{what}: must be contiguous")
+    if dtype is not None:
+        name = str(x.dtype).replace("torch.", "")
+        if name != _DTYPES[dtype][0]:
+            raise TypeError(f"{what}: expected {_DTYPES[dtype][0]}, got {name}")
+    if numel is not None:
+        n = int(x.numel()) if torch_like else int(x.size)
+        if n < numel:
+            raise ValueError(f"{what}: needs {numel} elements, got {n}")
+    if torch_like:
         return ctypes.c_void_p(x.data_ptr()), int(x.is_cuda)
-    assert x.flags.c_contiguous  # numpy
     return ctypes.c_void_p(x.ctypes.data), 0
+
+
+def _same_side(*pairs):
+    """All non-NULL pointer arguments of one call must live on the same side (host or device): one flag goes to C."""
+    sides = {dev for p, dev in pairs if p is not None}
+    if len(sides) > 1:
+        raise ValueError("mixing host arrays and device tensors in one call")
+    return sides.pop() if sides else 0
+
+
+def measure_fma_peak(dtype: str, stream: int | None = None) -> float:
+    """TFLOP/s of a register-only FMA probe of the given dtype on the current device (mm_measure_fma_peak)."""
+    L = lib()
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    out = ctypes.c_double()
+    st = L.mm_measure_fma_peak(MM_F64 if dtype == "f64" else MM_F32, ctypes.c_void_p(stream), ctypes.byref(out))
+    if st != MM_OK:
+        raise MMError(st, L.mm_status_string(st).decode(), L.mm_last_error(None).decode())
+    return float(out.value)
 
 
 class MM:
@@ -127,27 +163,28 @@ class MM:
             raise MMError(st, self._L.mm_status_string(st).decode(), self._L.mm_last_error(self._h).decode())
 
     def set_density(self, src):
-        p, dev = _ptr(src)
+        p, dev = _ptr(src, self.dtype, self.nc * self.inner, "density")
         self._check(self._L.mm_set_density(self._h, p, dev))
 
     def get_density(self, dst):
-        p, dev = _ptr(dst)
+        p, dev = _ptr(dst, self.dtype, self.nc * self.inner, "density")
         self._check(self._L.mm_get_density(self._h, p, dev))
         return dst
 
     def set_density_range(self, c_begin: int, n_configs: int, src):
-        p, dev = _ptr(src)
+        p, dev = _ptr(src, self.dtype, int(n_configs) * self.inner, "density range")
         self._check(self._L.mm_set_density_range(self._h, c_begin, n_configs, p, dev))
 
     def get_density_range(self, c_begin: int, n_configs: int, dst):
-        p, dev = _ptr(dst)
+        p, dev = _ptr(dst, self.dtype, int(n_configs) * self.inner, "density range")
         self._check(self._L.mm_get_density_range(self._h, c_begin, n_configs, p, dev))
         return dst
 
     def set_filament_velocity(self, U, V, Om):
-        (pu, d0), (pv, d1), (po, d2) = _ptr(U), _ptr(V), _ptr(Om)
-        assert d0 == d1 == d2
-        self._check(self._L.mm_set_filament_velocity(self._h, pu, pv, po, d0))
+        a = [_ptr(x, self.dtype, self.nc, n) for x, n in ((U, "U"), (V, "V"), (Om, "Omega"))]
+        if any(p is None for p, _ in a):
+            raise ValueError("U, V, Omega must all be given")
+        self._check(self._L.mm_set_filament_velocity(self._h, a[0][0], a[1][0], a[2][0], _same_side(*a)))
 
     def substep(self, n_sub: int, dt: float):
         self._check(self._L.mm_substep(self._h, int(n_sub), float(dt)))
@@ -156,28 +193,28 @@ class MM:
         self._check(self._L.mm_advance_local(self._h, float(dt), float(cfl)))
 
     def local_steps(self, n_steps, lam):
-        (pn, d0), (pl, d1) = _ptr(n_steps), _ptr(lam)
-        self._check(self._L.mm_local_steps(self._h, pn, pl, d0 if n_steps is not None else d1))
+        a, b = _ptr(n_steps, "i32", self.nc, "n_steps"), _ptr(lam, "f64", self.nc, "lambda")
+        self._check(self._L.mm_local_steps(self._h, a[0], b[0], _same_side(a, b)))
         return n_steps, lam
 
     def set_psi(self, psi):
-        pp, dev = _ptr(psi)
+        pp, dev = _ptr(psi, "f64", self.nc, "psi")
         self._check(self._L.mm_set_psi(self._h, pp, dev))
 
     def spread_force(self, F2):
-        pf, dev = _ptr(F2)
+        pf, dev = _ptr(F2, "f64", self.grid.nx * self.grid.ny * 2, "F2")
         self._check(self._L.mm_spread_force(self._h, pf, dev))
         return F2
 
     def update_free_motors(self, Mb_coarse=None, M_free=None):
-        (pb, d0), (pf, d1) = _ptr(Mb_coarse), _ptr(M_free)
-        self._check(self._L.mm_update_free_motors(self._h, pb, pf, d0 if Mb_coarse is not None else d1))
+        nn = self.grid.nx * self.grid.ny
+        a, b = _ptr(Mb_coarse, "f64", nn, "Mb_coarse"), _ptr(M_free, "f64", nn, "M_free")
+        self._check(self._L.mm_update_free_motors(self._h, a[0], b[0], _same_side(a, b)))
         return Mb_coarse, M_free
 
     def moments(self, force, torque):
-        (pf, d0), (pt, d1) = _ptr(force), _ptr(torque)
-        dev = d0 if force is not None else d1
-        self._check(self._L.mm_moments(self._h, pf, pt, dev))
+        a, b = _ptr(force, "f64", 2 * self.nc, "force"), _ptr(torque, "f64", self.nc, "torque")
+        self._check(self._L.mm_moments(self._h, a[0], b[0], _same_side(a, b)))
         return force, torque
 
     def set_option(self, opt: int, value: int):

@@ -8,6 +8,7 @@
 #include "mm_local.cuh"
 #include "mm_spread.cuh"
 #include "mm_free.cuh"
+#include "mm_peak.cuh"
 
 thread_local std::string g_create_err;
 
@@ -640,6 +641,45 @@ extern "C" mm_status mm_get_option(const mm_ctx *c, mm_option opt, int64_t *v)
     case MM_OPT_FREE_COUPLING: *v = c->coupled ? 1 : 0; return MM_OK;
     }
     return MM_ERR_INVALID_ARG;
+}
+
+// ---- the second roof: FMA issue peak of this device, measured (SURVEY.md 8(d) "measure and record the box's fp64 and
+// fp32 FMA peaks with a small register-only microbenchmark") ------------------------------------------------------------
+template <typename real>
+static mm_status fma_peak_impl(cudaStream_t stream, double *tflops)
+{
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return fail(nullptr, MM_ERR_CUDA, "no CUDA device");
+    real *out = nullptr;
+    if (cudaMalloc(&out, (size_t)sms * 1024 * sizeof(real)) != cudaSuccess) { cudaGetLastError(); return fail(nullptr, MM_ERR_NOMEM, "device allocation failed"); }
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = sizeof(real) == 8 ? 2048 : 4096;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {   // the first repetition is the warm-up
+        cudaEventRecord(e0, stream);
+        fma_peak_kernel<real><<<sms, 1024, 0, stream>>>(out, (real)0.999, (real)1e-3, iters);
+        cudaEventRecord(e1, stream);
+        if (cudaEventSynchronize(e1) != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double flops = 2.0 * (double)FMA_PEAK_PER_ITER * iters * 1024.0 * sms;
+        if (rep > 0 && ms > 0.f && flops / (ms * 1e-3) / 1e12 > best) best = flops / (ms * 1e-3) / 1e12;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess || best <= 0.0) return fail(nullptr, MM_ERR_CUDA, std::string("FMA peak probe failed: ") + cudaGetErrorString(e));
+    *tflops = best;
+    return MM_OK;
+}
+
+extern "C" mm_status mm_measure_fma_peak(mm_dtype dtype, void *cuda_stream, double *tflops)
+{
+    if (!tflops) return fail(nullptr, MM_ERR_INVALID_ARG, "NULL argument");
+    if (dtype != MM_F32 && dtype != MM_F64) return fail(nullptr, MM_ERR_INVALID_ARG, "bad dtype");
+    return dtype == MM_F64 ? fma_peak_impl<double>((cudaStream_t)cuda_stream, tflops) : fma_peak_impl<float>((cudaStream_t)cuda_stream, tflops);
 }
 
 extern "C" int64_t mm_launch_count(const mm_ctx *c) { return c ? c->launches : 0; }

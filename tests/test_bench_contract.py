@@ -31,18 +31,29 @@ def test_reference_arm_line():
 def test_cuda_arm_line_and_option_legs():
     d = run_bench("--config", "0", "--steps", "2", "--warmup", "3", "--cpu-seconds", "1", "--spread", "--free")
     for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
-              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "roofline_hbm", "cpu_baseline"):
         assert k in d, k
     assert d["n_gpus"] == 1 and d["steps"] == 2 and d["scaling"] == "weak" and d["dtype"] == "f64" and d["data"] == "synthetic"
     assert d["gpu_launches"] > 0 and d["value"] > 0 and d["e2e"]["value"] > 0
     assert d["e2e"]["h2d_bytes_per_step"] > 0 and d["e2e"]["d2h_bytes_per_step"] > 0
-    r = d["roofline"]
-    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-3
-    assert r["kernel"].startswith("coef<") and "traffic" in r
+    r, h = d["roofline"], d["roofline_hbm"]
+    # the fused kernel is bound by FMA issue: peak = the FMA probe of the same run; the HBM side has its own object
+    assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-3
+    assert 0 < r["frac"] < 1 and 0.5 * r["peak_nominal"] < r["peak"] < 1.1 * r["peak_nominal"] and "traffic" in r
+    assert r["kernel"].startswith("tm<") and r["flops_per_cell_update"] == 12
+    assert h["bound"] == "hbm" and h["unit"] == "GB/s" and abs(h["frac"] - h["achieved"] / h["peak"]) < 1e-3
+    for k in ("frac_nominal_8tbs", "effective_gbs", "effective_frac", "t1_gbs", "t1_frac", "t1_frac_nominal_8tbs"):
+        assert k in h, k
+    assert abs(h["effective_gbs"] / h["achieved"] - r["fuse_T"]) < 0.6          # a pass carries fuse_T substeps
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] > 0
+    one = d["cpu_baseline"]["one_thread_configs0"]
+    assert one["cores"] == 1 and 0 < one["value"] <= 1.5 * d["cpu_baseline"]["value"]
+    assert "per_config" not in d                                                # only the default (no --config) run adds it
     assert d["spread_force"]["ms_per_call"] > 0
-    assert d["free_motors"]["update_ms_per_call"] > 0 and d["free_motors"]["coupled_substep_kernel"].startswith("coef_mf<")
+    assert d["free_motors"]["update_ms_per_call"] > 0 and d["free_motors"]["coupled_substep_kernel"].startswith("tm_mf<")
     d = run_bench("--config", "0", "--steps", "1", "--warmup", "1", "--no-cpu", "--no-t1", "--scheme", "rk2")
     assert d["roofline"]["kernel"].startswith("rk2_fused<") and d["config"]["workload"].endswith("+rk2_superbee")
     d = run_bench("--config", "0", "--steps", "1", "--warmup", "1", "--no-cpu", "--local-dt")
-    assert d["roofline"]["kernel"].startswith("coef_local<") and d["local_dt"]["n_c_max"] >= d["local_dt"]["n_c_min"] >= 1
+    assert d["roofline"]["kernel"].startswith("tm_local<") and d["local_dt"]["n_c_max"] >= d["local_dt"]["n_c_min"] >= 1
+    d = run_bench("--config", "0", "--steps", "1", "--warmup", "1", "--no-cpu", "--no-t1", "--kernel", "4")
+    assert d["roofline"]["kernel"].startswith("coef<")
