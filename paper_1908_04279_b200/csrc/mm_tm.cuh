@@ -398,19 +398,23 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             if (j >= ns) break;   // ragged last chunk
             const real sj = kp.s_lo + (real(j) + real(0.5)) * kp.ds;
             if constexpr (MF) {
-                const unsigned short *nj = nod + j * (NXI + NETA);
-                int nodx[QA], nody[CB];
+                // the carry a plane sends downstream holds the source of the RECEIVING cell: while plane j is worked on,
+                // co.src is the (gathered) source of plane j+1; plane 0 receives its own source as the zero-inflow carry
+                auto gather = [&](int jj) {
+                    const unsigned short *nj = nod + jj * (NXI + NETA);
+                    int nodx[QA], nody[CB];
 #pragma unroll
-                for (int q = 0; q < QA; ++q) nodx[q] = (int)nj[a0 + q] * kp.ny;
+                    for (int q = 0; q < QA; ++q) nodx[q] = (int)nj[a0 + q] * kp.ny;
 #pragma unroll
-                for (int cb = 0; cb < CB; ++cb) nody[cb] = (int)nj[NXI + b0 + cb];
+                    for (int cb = 0; cb < CB; ++cb) nody[cb] = (int)nj[NXI + b0 + cb];
 #pragma unroll
-                for (int q = 0; q < QA; ++q)
+                    for (int q = 0; q < QA; ++q)
 #pragma unroll
-                    for (int cb = 0; cb < CB; ++cb)
-                        co.src[q][cb] = maskf[q][cb] * (kp.dt_kon * dtc * (real)kp.Mf[nodx[q] + nody[cb]]);
+                        for (int cb = 0; cb < CB; ++cb)
+                            co.src[q][cb] = maskf[q][cb] * (kp.dt_kon * dtc * (real)kp.Mf[nodx[q] + nody[cb]]);
+                };
                 if (j == 0) {
-                    // the carry into plane 0 is this plane's own source (zero inflow), at every level
+                    gather(0);
                     real p0[QA * CB];
 #pragma unroll
                     for (int q = 0; q < QA; ++q)
@@ -418,6 +422,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                         for (int cb = 0; cb < CB; ++cb) p0[q * CB + cb] = co.src[q][cb];
                     for (int lv = 0; lv < nlev; ++lv) tm_st<QA * CB>(tm_p + lv * CPL, p0);
                 }
+                gather(j + 1 < ns ? j + 1 : j);
             }
             // ---- level-independent coefficients of this plane
             uint32_t zxm = 0, zxp = 0, zem = 0, zep = 0;   // OR of the bit patterns: 0 <=> the whole set is +0

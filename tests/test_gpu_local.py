@@ -95,7 +95,7 @@ def test_local_coef_parity(dtype, nxi, dt_mult):
     g = Grid(5, 7, 20, 7, nxi, nxi)
     p = Params()
     n, name = check_local(g, p, dtype, dt_mult, omega_max=2.0)
-    assert name.startswith("coef_local<"), name
+    assert name.startswith("tm_local<"), name
     if dt_mult > 1:
         assert len(set(n.tolist())) > 1
 
@@ -108,6 +108,6 @@ def test_local_coef_equals_generic_and_moments_standalone():
     dt = 7.7 / orc.rate_bound(g, p, U, V, Om).mean()
     a = run_local(g, p, "f64", U, V, Om, m0, dt, 0.4, kernel=0)
     c = run_local(g, p, "f64", U, V, Om, m0, dt, 0.4, kernel=1)
-    assert a[5].startswith("coef_local<") and c[5].startswith("local_generic<")
+    assert a[5].startswith("tm_local<") and c[5].startswith("local_generic<")
     assert np.array_equal(a[1], c[1]) and p1_density(a[0], c[0]) < 1e-12
     assert np.allclose(a[3], c[3], rtol=0, atol=1e-13) and np.allclose(a[4], c[4], rtol=0, atol=1e-13)
