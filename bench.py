@@ -522,7 +522,7 @@ def cpu_baseline(w, target_s=15.0, log=None):
     # per-core figure (SURVEY.md 8(d) "additionally with 1 thread on configs[0]"): a child process, OMP_NUM_THREADS=1
     try:
         import subprocess
-        code = ("import sys, json; sys.path.insert(0, %r); import bench, mm_inputs as mi; w = mi.CONFIGS[0]; n = 24; "
+        code = ("import sys, json; sys.path.insert(0, %r); import bench, mm_inputs as mi; w = mi.CONFIGS[0]; n = 768; "
                 "t = bench.oracle_sample(w, n)[0]; print(json.dumps([n, t]))" % ROOT)
         res = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300,
                              env={**os.environ, "OMP_NUM_THREADS": "1"})

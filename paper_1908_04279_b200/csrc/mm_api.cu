@@ -334,9 +334,16 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
             t = (remaining + passes_left - 1) / passes_left;
             const bool mom = c->opt_fuse_mom && remaining == t;
             const bool inpl = c->opt_inplace != 0;
+            // auto: shallow passes run faster on the coefficient-form kernel, whose per-plane set-up is leaner (measured
+            // crossover, profiles/r02a_README.md: depth 8 in fp32, 6 in fp64); forced kernels are taken as asked
+            int pk = kind;
+            if (c->opt_kernel == 0 && kind == 5) {
+                const int coef_max = (c->dtype == MM_F32 && c->g.nxi == 16) ? 10 : 6;
+                if (t < (c->dtype == MM_F64 ? 6 : 8) && t <= coef_max) pk = 4;
+            }
             s = kind == 2   ? launch_stream(c, t, mom, dt, c->buf[c->cur], c->buf[c->cur ^ 1])
-                : kind == 4 ? launch_coef(c, t, mom, dt, c->buf[c->cur], c->buf[inpl ? c->cur : c->cur ^ 1])
-                : kind == 5 ? launch_tm(c, t, mom, dt, c->buf[c->cur], c->buf[inpl ? c->cur : c->cur ^ 1], false, 0, false)
+                : pk == 4 ? launch_coef(c, t, mom, dt, c->buf[c->cur], c->buf[inpl ? c->cur : c->cur ^ 1])
+                : pk == 5 ? launch_tm(c, t, mom, dt, c->buf[c->cur], c->buf[inpl ? c->cur : c->cur ^ 1], false, 0, false)
                             : launch_tile(c, t, mom, dt, c->cur, c->buf[c->cur ^ 1]);
             if (s == MM_OK && mom) c->mom_valid = true;
         }

@@ -36,11 +36,11 @@ def gpu_coupled(g, p, dtype, U, V, Om, m0, psi, n_sub, dt, kernel=0):
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("flags", [0, mi.FLAG_RK2_SUPERBEE])
-@pytest.mark.parametrize("kernel", [0, 1, 4])
+@pytest.mark.parametrize("kernel", [0, 1, 4, 5])
 @pytest.mark.parametrize("shape", [(6, 6, 8, 7, 16, 16), (5, 4, 4, 5, 6, 6), (8, 8, 4, 6, 8, 8)])
 def test_free_motor_coupling_parity(dtype, flags, shape, kernel):
-    if kernel == 4 and (flags or shape[4] not in (8, 16)):
-        pytest.skip("kernel 4 is forced only where the coefficient-form kernels apply")
+    if kernel in (4, 5) and (flags or shape[4] not in (8, 16)):
+        pytest.skip("kernels 4 and 5 are forced only where the coefficient-form kernels apply")
     g = Grid(*shape)
     big = Params(flags=flags, m_free=1e9)
     U, V, Om, m0 = random_inputs(g, big, dtype)
@@ -58,7 +58,8 @@ def test_free_motor_coupling_parity(dtype, flags, shape, kernel):
     ref = orc.run_coupled(g, p, U, V, Om, m_ref, 7, dt, Mf_ref)
     assert p1_density(out, ref) <= tol, name
     fast = kernel != 1 and flags == 0 and shape[4] in (8, 16)
-    assert name.startswith(("coef_mf<" if kernel == 4 else "tm_mf<") if fast else ("rk2_generic<" if flags else "generic<")), name
+    fam = {0: ("tm_mf<", "coef_mf<"), 4: ("coef_mf<",), 5: ("tm_mf<",)}   # auto picks by pass depth
+    assert name.startswith(fam[kernel] if fast else ("rk2_generic<" if flags else "generic<")), name
 
 
 def test_free_motor_option_and_errors():
@@ -80,12 +81,12 @@ def test_free_motor_option_and_errors():
     mm.substep(3, dt)
     a = np.empty_like(m0); mm.get_density(a)
     assert p1_density(a, orc.run(g, p, U, V, Om, m0, 3, dt)) < 1e-12      # uniform table == constant source
-    assert mm.kernel_name.startswith("tm_mf<")
+    assert mm.kernel_name.startswith(("tm_mf<", "coef_mf<"))
     with pytest.raises(MMError):
         mm.advance_local(dt, 0.4)                     # not with the coupled source
     mm.set_option(b.MM_OPT_FREE_COUPLING, 0)          # back to the fast path
     mm.substep(1, dt)
-    assert mm.kernel_name.startswith("tm<")
+    assert mm.kernel_name.startswith(("tm<", "coef<"))
     mm.destroy()
 
 
@@ -129,5 +130,5 @@ def test_full_microscale_step_against_the_oracle(dtype):
         assert ef <= tol and et <= tol, step
         F2_o = orc.spread_force(g, p, ref, psi)
         assert np.max(np.abs(F2 - F2_o)) / np.max(np.abs(F2_o)) <= tol, step
-    assert mm.kernel_name.startswith("tm_mf<")
+    assert mm.kernel_name.startswith(("tm_mf<", "coef_mf<"))
     mm.destroy()
