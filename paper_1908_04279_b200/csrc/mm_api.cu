@@ -130,7 +130,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->loc_lambda = nullptr; c->loc_n = c->loc_nmax = c->loc_list = c->loc_count = nullptr; c->loc_dt = nullptr;
     c->loc_valid = false;
     c->psi = c->fline = c->F2 = nullptr; c->psi_set = false;
-    c->Mf = c->Mbc = c->free_raw = c->free_factor = nullptr; c->free_any = nullptr; c->coupled = false;
+    c->Mf = c->Mbc = c->free_raw = c->free_factor = nullptr; c->free_fx = nullptr; c->free_any = nullptr; c->coupled = false;
     c->mom_valid = c->vel_set = false; c->tile_ok = false;
     c->dens_cov_count = 0;
     // measured defaults: the upwind-sparse tensor-memory kernel, at most MM_MAX_FUSE_T
@@ -196,7 +196,7 @@ extern "C" mm_status mm_destroy(mm_ctx *c)
     cudaFree(c->loc_lambda); cudaFree(c->loc_n); cudaFree(c->loc_nmax); cudaFree(c->loc_dt);
     cudaFree(c->loc_list); cudaFree(c->loc_count);
     cudaFree(c->psi); cudaFree(c->fline); cudaFree(c->F2);
-    cudaFree(c->Mf); cudaFree(c->Mbc); cudaFree(c->free_raw); cudaFree(c->free_factor); cudaFree(c->free_any);
+    cudaFree(c->Mf); cudaFree(c->Mbc); cudaFree(c->free_raw); cudaFree(c->free_factor); cudaFree(c->free_fx); cudaFree(c->free_any);
     delete c;
     return MM_OK;
 }
@@ -561,12 +561,41 @@ static mm_status free_impl(mm_ctx *c)
     const int64_t cap = (int64_t)c->sm_count * 8;
     if (blocks > cap) blocks = cap;
     real *dens = (real *)c->buf[c->cur];
-    free_cells_kernel<real, 0><<<(unsigned)blocks, 256, 0, c->stream>>>(q, c->nc, dens, c->psi, w, c->free_raw, nullptr, nullptr);
-    CUDA_TRY(c, cudaGetLastError());
-    free_cap_kernel<<<(nn + 255) / 256, 256, 0, c->stream>>>(nn, p.m_free, c->free_raw, c->free_factor, c->Mbc, c->Mf, c->free_any);
-    CUDA_TRY(c, cudaGetLastError());
-    free_cells_kernel<real, 1><<<(unsigned)blocks, 256, 0, c->stream>>>(q, c->nc, dens, nullptr, 0.0, nullptr, c->free_factor, c->free_any);
-    CUDA_TRY(c, cudaGetLastError());
+    // the BASELINE offset planes run the vector kernels
+    const int vw = (g.nxi == 16 && g.neta == 16) || (g.nxi == 8 && g.neta == 8) ? 1 : 0;
+    // a private copy of the table per CTA in shared memory where it fits: 96-bit fixed point (12 bytes per node) in the
+    // vector kernels, fp64 in the generic one
+    const size_t tab_bytes = vw ? (size_t)g.nx * (g.ny | 1) * 12 : (size_t)nn * sizeof(double);
+    const bool priv = tab_bytes <= 200 * 1024;
+    const bool fx = priv && vw;
+    double unit = 1.0;   // power of two >= M_total
+    if (p.m_free > 0) { int e = 0; std::frexp(p.m_free, &e); unit = std::ldexp(1.0, e); }
+    if (fx) CUDA_TRY(c, cudaMemsetAsync(c->free_fx, 0, (size_t)nn * 16, c->stream));
+    auto run = [&](auto kern0, auto kern1, int threads, size_t smem) -> mm_status {
+        int bps = 0;
+        mm_status ks = kernel_shape(c, (const void *)kern0, threads, smem, "free-motor deposit kernel", &bps);
+        if (ks != MM_OK) return ks;
+        const int wpb = threads / 32;
+        int64_t pb = (int64_t)c->sm_count * bps;
+        if (pb > (c->nc + wpb - 1) / wpb) pb = (c->nc + wpb - 1) / wpb;
+        kern0<<<(unsigned)pb, threads, smem, c->stream>>>(q, c->nc, dens, c->psi, w, c->free_raw, nullptr, nullptr, c->free_fx, 1.0 / unit);
+        CUDA_TRY(c, cudaGetLastError());
+        free_cap_kernel<<<(nn + 255) / 256, 256, 0, c->stream>>>(nn, p.m_free, c->free_raw, c->free_factor, c->Mbc, c->Mf, c->free_any,
+                                                                  fx ? c->free_fx : nullptr, unit);
+        CUDA_TRY(c, cudaGetLastError());
+        kern1<<<(unsigned)blocks, 256, 0, c->stream>>>(q, c->nc, dens, nullptr, 0.0, nullptr, c->free_factor, c->free_any, nullptr, 1.0);
+        CUDA_TRY(c, cudaGetLastError());
+        return MM_OK;
+    };
+    mm_status rs;
+#define MM_FREE_VEC(N_) (priv ? run(free_cells_vec_kernel<real, 0, true, N_, N_, 4>, free_cells_vec_kernel<real, 1, false, N_, N_, 4>, 512, tab_bytes) \
+                             : run(free_cells_vec_kernel<real, 0, false, N_, N_, 4>, free_cells_vec_kernel<real, 1, false, N_, N_, 4>, 256, 0))
+    if (vw && g.nxi == 16) rs = MM_FREE_VEC(16);
+    else if (vw) rs = MM_FREE_VEC(8);
+    else rs = priv ? run(free_cells_kernel<real, 0, true>, free_cells_kernel<real, 1, false>, 1024, tab_bytes)
+                   : run(free_cells_kernel<real, 0, false>, free_cells_kernel<real, 1, false>, 256, 0);
+#undef MM_FREE_VEC
+    if (rs != MM_OK) return rs;
     c->launches += 3;
     return MM_OK;
 }
@@ -577,16 +606,16 @@ extern "C" mm_status mm_update_free_motors(mm_ctx *c, double *Mb_coarse, double 
     if (c->dens_cov_count != c->nc || !c->psi_set) return fail(c, MM_ERR_STATE, "set density and psi first");
     const size_t nn = (size_t)c->g.nx * c->g.ny;
     if (!c->free_any) {   // allocated as a group, committed together
-        void *g[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
-        const size_t bytes[5] = {nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), sizeof(int)};
-        for (int i = 0; i < 5; ++i)
+        void *g[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+        const size_t bytes[6] = {nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * 16, sizeof(int)};
+        for (int i = 0; i < 6; ++i)
             if (cudaMalloc(&g[i], bytes[i]) != cudaSuccess) {
                 cudaGetLastError();
                 for (int k = 0; k < i; ++k) cudaFree(g[k]);
                 return fail(c, MM_ERR_NOMEM, "device allocation failed (free-motor tables)");
             }
         c->Mf = (double *)g[0]; c->Mbc = (double *)g[1]; c->free_raw = (double *)g[2]; c->free_factor = (double *)g[3];
-        c->free_any = (int *)g[4];
+        c->free_fx = (unsigned long long *)g[4]; c->free_any = (int *)g[5];
     }
     mm_status s = c->dtype == MM_F64 ? free_impl<double>(c) : free_impl<float>(c);
     if (s != MM_OK) return s;

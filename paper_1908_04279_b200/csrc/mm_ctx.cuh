@@ -8,6 +8,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include <cuda.h>
@@ -45,6 +46,7 @@ struct mm_ctx {
     double *psi, *fline, *F2;       // NEXT-4: filament density weights [nc], plane forces [nc][ns][2], fluid-grid force
     bool psi_set;
     double *Mf, *Mbc, *free_raw, *free_factor;   // NEXT-2: free / coarse bound motor tables [nx][ny], scratch
+    unsigned long long *free_fx;   // [nx][ny][2]: the coarse sums in 128-bit fixed point (mm_free.cuh)
     int *free_any;
     bool coupled;                   // the substep source is k_on M_f(r0) instead of k_on m_free
     CUtensorMap tmap[2];            // tiled-TMA views of buf[0], buf[1] (tile kernel)

@@ -40,12 +40,24 @@ __device__ __forceinline__ int wrap_floor(double r, int n)
 
 // MODE 0: raw[n] += w Psi_c m over all cells (fp64 atomic adds, macro cadence).  MODE 1: m *= f[n] (cap rescale), skipped
 // entirely when no node was capped.  One warp per configuration, lanes stride over the cells of each plane.
-template <typename real, int MODE>
-__global__ void __launch_bounds__(256) free_cells_kernel(const FreeGeom q, int64_t nc, real *__restrict__ dens,
+// PRIV (MODE 0): every CTA deposits into its OWN copy of the (x, y) table in shared memory (nx ny doubles, dynamic) with
+// shared-memory atomics and adds it to the global table once at the end: the 8.6 G deposits of configs[4] then contend
+// inside an SM only, and the global table sees nx ny atomics per CTA instead of one per cell (profiles/r02b_README.md).
+template <typename real, int MODE, bool PRIV = false>
+__global__ void __launch_bounds__(PRIV ? 1024 : 256) free_cells_kernel(const FreeGeom q, int64_t nc, real *__restrict__ dens,
                                                          const double *__restrict__ psi, double w, double *__restrict__ raw,
-                                                         const double *__restrict__ factor, const int *__restrict__ any_capped)
+                                                         const double *__restrict__ factor, const int *__restrict__ any_capped,
+                                                         unsigned long long * /*raw_fx: vector kernels only*/ = nullptr,
+                                                         double /*inv_unit*/ = 1.0)
 {
     if (MODE == 1 && *any_capped == 0) return;
+    extern __shared__ double free_tab[];
+    double *tab = raw;
+    if (PRIV) {
+        for (int i = threadIdx.x; i < q.nx * q.ny; i += blockDim.x) free_tab[i] = 0.0;
+        __syncthreads();
+        tab = free_tab;
+    }
     const int lane = threadIdx.x & 31;
     const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
     const int plane = q.nxi * q.neta;
@@ -87,7 +99,7 @@ __global__ void __launch_bounds__(256) free_cells_kernel(const FreeGeom q, int64
                 real *v = mc + (int64_t)j * plane + i;
                 if (MODE == 0) {
                     const double val = (double)*v;
-                    if (val != 0.0 && wp != 0.0) atomicAdd(&raw[n], wp * val);
+                    if (val != 0.0 && wp != 0.0) atomicAdd(&tab[n], wp * val);
                 } else {
                     const double f = factor[n];
                     if (f != 1.0) *v = (real)((double)*v * f);
@@ -95,14 +107,138 @@ __global__ void __launch_bounds__(256) free_cells_kernel(const FreeGeom q, int64
             }
         }
     }
+    if (PRIV) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < q.nx * q.ny; i += blockDim.x)
+            if (free_tab[i] != 0.0) atomicAdd(&raw[i], free_tab[i]);
+    }
+}
+
+// Exact accumulation in shared memory.  Shared-memory atomics are native for 32-bit integers only (fp64 and 64-bit
+// integer adds compile to compare-and-swap loops), so a private table holds every node as a 96-bit two's-complement
+// fixed-point number in three 32-bit limbs, value = (L2:L1 2^-32 + L0 2^-64) * unit with unit = the power of two >=
+// M_total: a deposit is 2 (rarely 3) native ATOMS.ADD, each returning the old limb so that exactly the add that wraps a
+// limb carries into the next.  Integer adds commute: the table does not depend on the order of the deposits; its
+// resolution (2^-64 unit per deposit, truncated) is far below the fp64 rounding of a node sum; range |sum| < 2^31 unit.
+__device__ __forceinline__ void fx_deposit(uint32_t *L0, uint32_t *L1, uint32_t *L2, int n, double q /* value / unit */)
+{
+    const double t = q * 4294967296.0;                            // exact
+    const long long i1 = __double2ll_rd(t);                       // floor: bits 2^-32 and up
+    const uint32_t x0 = __double2uint_rd((t - (double)i1) * 4294967296.0);   // the next 32 bits, truncated
+    const uint32_t x1 = (uint32_t)i1, x2 = (uint32_t)(i1 >> 32);
+    const uint32_t o0 = atomicAdd(&L0[n], x0);
+    const uint32_t t1 = x1 + ((o0 + x0 < o0) ? 1u : 0u);
+    uint32_t c1 = (t1 < x1) ? 1u : 0u;                            // x1 = 2^32 - 1 with a carry in: carry out, nothing to add
+    if (t1) { const uint32_t o1 = atomicAdd(&L1[n], t1); c1 |= (o1 + t1 < o1) ? 1u : 0u; }
+    if (x2 | c1) atomicAdd(&L2[n], x2 + c1);
+}
+
+// The same two passes for the BASELINE offset planes (16x16, 8x8; a plane tiles a warp with VW cells of one row per
+// 64/128-bit access, NV accesses per lane): PL planes are in flight per lane before any is consumed -- one 4-byte load
+// per lane and plane, as in the kernel above, leaves the pass bound by load latency -- the node of a cell is two table
+// look-ups by shuffle (the index separates), and with PRIV the deposits go to the CTA's fixed-point table.
+template <typename real, int MODE, bool PRIV, int NXI, int NETA, int PL>
+__global__ void __launch_bounds__(PRIV ? 512 : 256) free_cells_vec_kernel(const FreeGeom q, int64_t nc, real *__restrict__ dens,
+                                                                          const double *__restrict__ psi, double w,
+                                                                          double *__restrict__ raw, const double *__restrict__ factor,
+                                                                          const int *__restrict__ any_capped,
+                                                                          unsigned long long *__restrict__ raw_fx = nullptr,
+                                                                          double inv_unit = 1.0)
+{
+    constexpr int PLANE = NXI * NETA;
+    constexpr int VW = (16 / (int)sizeof(real)) * 32 <= PLANE ? 16 / (int)sizeof(real) : PLANE / 32;   // cells per access
+    constexpr int NV = PLANE / (32 * VW), LB = NETA / VW, RPV = 32 / LB;   // accesses per plane; lanes per row; rows per access
+    static_assert(NXI <= 16 && NETA <= 16 && VW >= 1 && NV * 32 * VW == PLANE && NETA % VW == 0 && 32 % LB == 0, "plane must tile a warp");
+    if (MODE == 1 && *any_capped == 0) return;
+    struct alignas(sizeof(real) * VW) Vec { real v[VW]; };
+    extern __shared__ double free_tab[];
+    const int nn = q.nx * q.ny;
+    // PRIV: the limb tables, rows padded to an odd stride -- the rows of a patch are ny apart in the global table, a
+    // multiple of 32 banks on the BASELINE grids (8-way conflicts on every atomic otherwise)
+    const int ldt = PRIV ? (q.ny | 1) : q.ny, nnp = q.nx * ldt;
+    uint32_t *L0 = reinterpret_cast<uint32_t *>(free_tab), *L1 = L0 + nnp, *L2 = L1 + nnp;
+    if (PRIV) {
+        for (int i = threadIdx.x; i < 3 * nnp; i += blockDim.x) L0[i] = 0u;
+        __syncthreads();
+    }
+    const int lane = threadIdx.x & 31;
+    const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    const int k16 = lane & 15, arow = lane / LB, b0 = (lane % LB) * VW;
+    const double off = lane < 16 ? __dadd_rn(-q.R, __dmul_rn(k16 + 0.5, q.dxi)) : __dadd_rn(-q.R, __dmul_rn(k16 + 0.5, q.deta));
+    const int64_t inner = (int64_t)PLANE * q.ns;
+    for (int64_t c = warp0; c < nc; c += nwarps) {
+        const int itheta = (int)(c % q.ntheta);
+        const int iy = (int)((c / q.ntheta) % q.ny), ix = (int)(c / ((int64_t)q.ntheta * q.ny));
+        const double theta = 2.0 * 3.14159265358979323846264338327950288 * (double)itheta / (double)q.ntheta;
+        const double cs = lane < 16 ? cos(theta) : sin(theta);
+        const double base = lane < 16 ? __ddiv_rn((double)ix, (double)q.nx) : __ddiv_rn((double)iy, (double)q.ny);
+        const double nd = lane < 16 ? (double)q.nx : (double)q.ny;
+        const double wp = MODE == 0 ? w * psi[c] : 0.0;
+        if (MODE == 0 && wp == 0.0) continue;
+        real *mc = dens + c * inner + lane * VW;
+        for (int j0 = 0; j0 < q.ns; j0 += PL) {
+            Vec v[PL][NV];
+#pragma unroll
+            for (int pl = 0; pl < PL; ++pl)
+#pragma unroll
+                for (int k = 0; k < NV; ++k)
+                    if (j0 + pl < q.ns) v[pl][k] = *reinterpret_cast<const Vec *>(mc + (int64_t)(j0 + pl) * PLANE + k * 32 * VW);
+#pragma unroll
+            for (int pl = 0; pl < PL; ++pl) {
+                const int j = j0 + pl;
+                if (j >= q.ns) break;
+                // lanes 0..15: x node of row a = lane (times ny); lanes 16..31: y node of column b = lane - 16; every
+                // operation rounded separately, exactly the oracle's expression (ties)
+                const double sj = __dadd_rn(q.s_lo, __dmul_rn(j + 0.5, q.ds));
+                const double r = __dmul_rn(__dsub_rn(__dadd_rn(base, __dmul_rn(sj, cs)), off), nd);
+                const int my_node = lane < 16 ? wrap_floor(__dadd_rn(r, 0.5), q.nx) * ldt : wrap_floor(__dadd_rn(r, 0.5), q.ny);
+                int nb[VW];
+#pragma unroll
+                for (int e = 0; e < VW; ++e) nb[e] = __shfl_sync(0xffffffffu, my_node, 16 + b0 + e);
+#pragma unroll
+                for (int k = 0; k < NV; ++k) {
+                    const int na = __shfl_sync(0xffffffffu, my_node, k * RPV + arow);
+                    bool dirty = false;
+#pragma unroll
+                    for (int e = 0; e < VW; ++e) {
+                        const int n = na + nb[e];
+                        if (MODE == 0) {
+                            const double val = (double)v[pl][k].v[e];
+                            if (val != 0.0) {
+                                if (PRIV) fx_deposit(L0, L1, L2, n, __dmul_rn(wp, val) * inv_unit);
+                                else atomicAdd(&raw[n], wp * val);
+                            }
+                        } else {
+                            const double f = factor[n];
+                            if (f != 1.0) { v[pl][k].v[e] = (real)((double)v[pl][k].v[e] * f); dirty = true; }
+                        }
+                    }
+                    if (MODE == 1 && dirty) *reinterpret_cast<Vec *>(mc + (int64_t)j * PLANE + k * 32 * VW) = v[pl][k];
+                }
+            }
+        }
+    }
+    if (PRIV) {
+        // add this CTA's table to the global one: 128-bit fixed point, {low 64 fraction bits, signed integer part}
+        __syncthreads();
+        for (int i = threadIdx.x; i < nn; i += blockDim.x) {
+            const int ip = (i / q.ny) * ldt + i % q.ny;
+            const unsigned long long lo = ((unsigned long long)L1[ip] << 32) | L0[ip];
+            long long hi = (long long)(int32_t)L2[ip];
+            if (lo) { const unsigned long long o = atomicAdd(&raw_fx[2 * i], lo); hi += (o + lo < o) ? 1 : 0; }
+            if (hi) atomicAdd(&raw_fx[2 * i + 1], (unsigned long long)hi);
+        }
+    }
 }
 
 // Per node: cap, factor, M_b,coarse, M_f.
+// raw_fx != NULL: the sums arrive as 128-bit fixed point in units of `unit` (see fx_deposit)
 __global__ void free_cap_kernel(int nn, double m_total, const double *__restrict__ raw, double *__restrict__ factor,
-                                double *__restrict__ Mbc, double *__restrict__ Mf, int *__restrict__ any_capped)
+                                double *__restrict__ Mbc, double *__restrict__ Mf, int *__restrict__ any_capped,
+                                const unsigned long long *__restrict__ raw_fx = nullptr, double unit = 1.0)
 {
     for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < nn; n += gridDim.x * blockDim.x) {
-        const double r = raw[n];
+        const double r = raw_fx ? ((double)(long long)raw_fx[2 * n + 1] + (double)raw_fx[2 * n] * 5.421010862427522e-20) * unit : raw[n];
         const bool over = r > m_total;
         factor[n] = over ? m_total / r : 1.0;
         const double capped = over ? m_total : r;
