@@ -101,9 +101,14 @@ typedef enum {
                                 configuration), the other buffer is not touched; same results, same speed, half the
                                 memory.  Default 0; always 1 for a context created with ONE density buffer
                                 (mm_create, dens_buf1 = NULL) */
-    MM_OPT_FREE_COUPLING = 4 /* 1: the source term of the substeps is k_on M_f(r0) from the table of the last
+    MM_OPT_FREE_COUPLING = 4,/* 1: the source term of the substeps is k_on M_f(r0) from the table of the last
                                 mm_update_free_motors (which switches it on); 0: the constant k_on m_free again.
                                 MM_ERR_STATE when set to 1 before any mm_update_free_motors */
+    MM_OPT_FREE_REFRESH = 5  /* k > 0: with the coupled source, mm_substep redoes the coarse reduction, the cap and M_f
+                                (what mm_update_free_motors does) before every k-th substep of a call -- Alg. 2's own
+                                cadence, where l.14-20 sit inside the inner loop, is k = 1; at most k
+                                substeps are then fused per pass.  0 (default): the table stays frozen between two
+                                mm_update_free_motors calls */
 } mm_option;
 #define MM_MAX_FUSE_T 12  /* kernel 5 (tensor-memory budget of a warp); kernel 4 fuses at most 10 (fp32, 16x16 offset
                              planes) / 6, the streamed / tiled variants at most 4 (deeper settings are clamped) */
@@ -155,8 +160,9 @@ mm_status mm_substep(mm_ctx *ctx, int32_t n_sub, double dt);
  * steps of equal size dt / n_c, where lambda_c is the S8 positivity rate maximised over the disc cells of c
  * (readings Q31-Q33 in DESIGN.md).  lambda_c and n_c are computed on the device in fp64 in every dtype; the number
  * of passes (max_c n_c) is read back once per call (one 4-byte copy; the call synchronises the stream for it).
- * dt > 0, cfl > 0, finite; MM_ERR_STATE unless density and velocities have been set; MM_ERR_INVALID_ARG with
- * MM_FLAG_RK2_SUPERBEE (not supported on this call yet). */
+ * With the coupled source (MM_OPT_FREE_COUPLING) the local steps take k_on M_f(r0) from the frozen table -- Alg. 2 as one
+ * loop (l.5 with l.20's M_f) -- on kernels 0 / 5.  dt > 0, cfl > 0, finite; MM_ERR_STATE unless density and velocities
+ * have been set; MM_ERR_INVALID_ARG with MM_FLAG_RK2_SUPERBEE (not supported on this call). */
 mm_status mm_advance_local(mm_ctx *ctx, double dt, double cfl);
 /* n_c [Nc] (int32) and lambda_c [Nc] (fp64) of the last mm_advance_local; either pointer may be NULL.
  * MM_ERR_STATE before the first mm_advance_local or after new velocities were set. */

@@ -322,6 +322,25 @@ int mmo_run_coupled(const mmo_grid *g, const mmo_params *p, int64_t c_first, int
     return run_impl(g, p, c_first, n_configs, U, V, Om, m, n_sub, dt, Mf);
 }
 
+/* Alg. 2 with the paper's cadence: the coarse reduction, the cap and M_f (l.14-20) sit INSIDE the
+ * inner loop `while t* < t*_end` (l.4), i.e. they are redone after inner steps, not once per macro step.  Here: before
+ * every `refresh`-th substep (substeps 0, refresh, 2 refresh, ...) mmo_free_motors is applied to the whole state (cap
+ * rescale included) and the following substeps take their source from the new table.  refresh = 1 is the paper's loop;
+ * refresh >= n_sub is one update followed by mmo_run_coupled.  m: ALL configurations; Mbc, Mf: the tables of the LAST
+ * update (outputs, [nx][ny]).  Nothing new is computed here: the function composes mmo_free_motors and run_impl. */
+int mmo_run_alg2(const mmo_grid *g, const mmo_params *p, const double *U, const double *V, const double *Om,
+                 double *m, const double *psi, int32_t n_sub, double dt, int32_t refresh, double *Mbc, double *Mf)
+{
+    const int64_t nc = (int64_t)g->nx * g->ny * g->ntheta;
+    if (refresh < 1 || !Mf) return -2;
+    for (int32_t n = 0; n < n_sub; n += refresh) {
+        int32_t k = n_sub - n < refresh ? n_sub - n : refresh;
+        if (mmo_free_motors(g, p, m, psi, Mbc, Mf) != 0) return -1;
+        if (run_impl(g, p, 0, nc, U, V, Om, m, k, dt, Mf) != 0) return -1;
+    }
+    return 0;
+}
+
 /* ---- local adaptive time step per independent unit ------------------------------------
  * "We instead compute a local dt* for each r0 at the beginning of each inner time step and update M_b at each r0
  * asynchronously"; Alg. 2 l.2-5: "Set t*_end = t + dt; for r0 in grid: while
@@ -372,9 +391,9 @@ int mmo_rate_bound(const mmo_grid *g, const mmo_params *p, int64_t c_first, int6
 
 /* Advance every configuration from t to t + dt with its own n_c equal local steps (see above); the scheme of each
  * local step is the one the flags select.  n_steps (may be NULL) receives n_c. */
-int mmo_advance_local(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
-                      const double *U, const double *V, const double *Om,
-                      double *m, double dt, double cfl, int32_t *n_steps)
+static int advance_local_impl(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
+                              const double *U, const double *V, const double *Om,
+                              double *m, double dt, double cfl, int32_t *n_steps, const double *Mf)
 {
     const size_t inner = (size_t)g->ns * g->nxi * g->neta;
     double *lambda = (double *)malloc(sizeof(double) * (size_t)(n_configs > 0 ? n_configs : 1));
@@ -386,11 +405,28 @@ int mmo_advance_local(const mmo_grid *g, const mmo_params *p, int64_t c_first, i
         double need = ceil(dt * lambda[c] / cfl);
         int32_t n_c = need < 1.0 ? 1 : (int32_t)need;
         if (n_steps) n_steps[c] = n_c;
-        if (mmo_run(g, p, c_first + c, 1, U + c, V + c, Om + c, m + (size_t)c * inner, n_c, dt / (double)n_c) != 0)
+        if (run_impl(g, p, c_first + c, 1, U + c, V + c, Om + c, m + (size_t)c * inner, n_c, dt / (double)n_c, Mf) != 0)
             fail = 1;
     }
     free(lambda);
     return fail ? -1 : 0;
+}
+
+int mmo_advance_local(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
+                      const double *U, const double *V, const double *Om,
+                      double *m, double dt, double cfl, int32_t *n_steps)
+{
+    return advance_local_impl(g, p, c_first, n_configs, U, V, Om, m, dt, cfl, n_steps, NULL);
+}
+
+/* Alg. 2 as ONE loop: the local steps of l.5 with the source k_on M_f(r0) of the given table (frozen
+ * over the macro step, reading Q42).  The step count does not depend on the source (reading Q32: lambda_c is the S8
+ * rate of advection and detachment), so n_c is the same as without the table. */
+int mmo_advance_local_coupled(const mmo_grid *g, const mmo_params *p, int64_t c_first, int64_t n_configs,
+                              const double *U, const double *V, const double *Om,
+                              double *m, double dt, double cfl, int32_t *n_steps, const double *Mf)
+{
+    return advance_local_impl(g, p, c_first, n_configs, U, V, Om, m, dt, cfl, n_steps, Mf);
 }
 
 /* S9: per-configuration moments; force [n][2], torque [n]; optional (may be NULL) test-only

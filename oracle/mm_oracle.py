@@ -61,6 +61,10 @@ def _load():
         lib.mmo_free_motors.argtypes = [vp, vp, vp, vp, vp, vp]
         lib.mmo_run_coupled.restype = ctypes.c_int
         lib.mmo_run_coupled.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, dbl, vp]
+        lib.mmo_run_alg2.restype = ctypes.c_int
+        lib.mmo_run_alg2.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, dbl, i32, vp, vp]
+        lib.mmo_advance_local_coupled.restype = ctypes.c_int
+        lib.mmo_advance_local_coupled.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, dbl, dbl, vp, vp]
         lib.mmo_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -118,10 +122,42 @@ def rate_bound(grid, params, U, V, Om, c_first: int = 0) -> np.ndarray:
     return lam
 
 
-def advance_local(grid, params, U, V, Om, m, dt: float, cfl: float, c_first: int = 0):
-    """Every configuration from t to t + dt with its own n_c = max(1, ceil(dt lambda_c / cfl)) equal local steps
-    (Alg. 2 l.2-5; readings Q31-Q33).  Returns (new fp64 density, n_c int32 array)."""
+def run_alg2(grid, params, U, V, Om, m, psi, n_sub: int, dt: float, refresh: int):
+    """Alg. 2 with the paper's cadence: before every `refresh`-th substep the coarse reduction, the
+    cap and M_f are redone on the whole state.  m: ALL configurations.  Returns (density, M_b,coarse, M_f of the last
+    update)."""
     lib = _load()
+    g, p = _grid(grid), _params(params)
+    nc = grid.nx * grid.ny * grid.ntheta
+    out = np.array(m, dtype=np.float64, order="C", copy=True)
+    assert out.size == nc * grid.ns * grid.nxi * grid.neta
+    U, V, Om, psi = _f64(U, nc), _f64(V, nc), _f64(Om, nc), _f64(psi, nc)
+    Mbc, Mf = np.empty((grid.nx, grid.ny)), np.empty((grid.nx, grid.ny))
+    rc = lib.mmo_run_alg2(ctypes.byref(g), ctypes.byref(p), U.ctypes.data, V.ctypes.data, Om.ctypes.data, out.ctypes.data,
+                          psi.ctypes.data, n_sub, dt, refresh, Mbc.ctypes.data, Mf.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"mmo_run_alg2 failed ({rc})")
+    return out.reshape(nc, grid.ns, grid.nxi, grid.neta), Mbc, Mf
+
+
+def advance_local(grid, params, U, V, Om, m, dt: float, cfl: float, c_first: int = 0, Mf=None):
+    """Every configuration from t to t + dt with its own n_c = max(1, ceil(dt lambda_c / cfl)) equal local steps
+    (Alg. 2 l.2-5; readings Q31-Q33); with Mf [nx][ny] the source is k_on M_f(r0) (reading Q42).
+    Returns (new fp64 density, n_c int32 array)."""
+    lib = _load()
+    if Mf is not None:
+        g, p = _grid(grid), _params(params)
+        inner = grid.ns * grid.nxi * grid.neta
+        out = np.array(m, dtype=np.float64, order="C", copy=True)
+        n = out.size // inner
+        U, V, Om = _f64(U, n), _f64(V, n), _f64(Om, n)
+        Mf = _f64(Mf, grid.nx * grid.ny)
+        nst = np.empty(n, np.int32)
+        rc = lib.mmo_advance_local_coupled(ctypes.byref(g), ctypes.byref(p), c_first, n, U.ctypes.data, V.ctypes.data,
+                                           Om.ctypes.data, out.ctypes.data, dt, cfl, nst.ctypes.data, Mf.ctypes.data)
+        if rc != 0:
+            raise MemoryError("oracle scratch allocation failed")
+        return out.reshape(n, grid.ns, grid.nxi, grid.neta), nst
     g, p = _grid(grid), _params(params)
     inner = grid.ns * grid.nxi * grid.neta
     out = np.array(m, dtype=np.float64, order="C", copy=True)

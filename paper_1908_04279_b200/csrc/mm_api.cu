@@ -136,6 +136,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     // measured defaults: the upwind-sparse tensor-memory kernel, at most MM_MAX_FUSE_T
     // substeps per pass (with MM_AUTO_KERNEL = 4: the coefficient-form kernel at depth 10 / 5)
     c->opt_kernel = 0; c->opt_fuse_t = MM_AUTO_KERNEL == 5 ? MM_MAX_FUSE_T : (dtype == MM_F64 ? 5 : 10); c->opt_fuse_mom = 1;
+    c->opt_free_refresh = 0;
     c->single = (b0 != nullptr && b1 == nullptr);
     c->opt_inplace = c->single ? 1 : 0;
     c->checked_dt = NAN; c->launches = 0; c->kname[0] = 0;
@@ -265,6 +266,8 @@ extern "C" mm_status mm_set_filament_velocity(mm_ctx *c, const void *U, const vo
     return MM_OK;
 }
 
+static mm_status refresh_free_motors(mm_ctx *c);   // NEXT-2, below
+
 extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
 {
     if (!c) return MM_ERR_INVALID_ARG;
@@ -301,6 +304,8 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
     if (fast && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernels do not support this grid/flags");
     if (kind == 3 && !c->tile_ok) return fail(c, MM_ERR_INVALID_ARG, "tile kernel does not support this grid/flags");
     c->mom_valid = false;
+    const int refresh = c->coupled ? c->opt_free_refresh : 0;
+    if (refresh > 0 && !c->psi_set) return fail(c, MM_ERR_STATE, "MM_OPT_FREE_REFRESH needs mm_set_psi");
     if (c->p.flags & MM_FLAG_RK2_SUPERBEE) {
         // kernel 0 (auto): the fused one-pass kernel where the grid is supported, else the generic stages; 1: generic
         if (c->opt_kernel != 0 && c->opt_kernel != 1)
@@ -310,13 +315,19 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         if (c->single && !fused)
             return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context runs RK2 + Superbee only on the fused in-place kernel (no coupled source, 16x16 or 8x8 offset planes)");
         for (int n = 0; n < n_sub; ++n) {
+            if (refresh > 0 && n % refresh == 0) { mm_status fs = refresh_free_motors(c); if (fs != MM_OK) return fs; }
             mm_status s = fused ? launch_rk2_fused_any(c, dt)
                                 : launch_rk2_generic(c, dt);
             if (s != MM_OK) return s;
         }
         return MM_OK;
     }
-    int remaining = n_sub;
+    // Alg. 2's cadence (MM_OPT_FREE_REFRESH = k > 0): the coarse reduction, cap and M_f are redone before every k-th
+    // substep, so a chunk of at most k substeps is fused between two updates
+    for (int n0 = 0; n0 < n_sub; n0 += (refresh > 0 ? refresh : n_sub)) {
+    int remaining = refresh > 0 ? (n_sub - n0 < refresh ? n_sub - n0 : refresh) : n_sub;
+    if (refresh > 0) { mm_status fs = refresh_free_motors(c); if (fs != MM_OK) return fs; c->mom_valid = false; }
+    const bool last_chunk = refresh <= 0 || n0 + remaining == n_sub;   // moments are fused into the call's last pass only
     while (remaining > 0) {
         mm_status s;
         int t = 1;
@@ -332,7 +343,7 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
             if (kind == 5 && tmax > tm_max_levels(c)) tmax = tm_max_levels(c);               // tensor-memory budget
             const int passes_left = (remaining + tmax - 1) / tmax;
             t = (remaining + passes_left - 1) / passes_left;
-            const bool mom = c->opt_fuse_mom && remaining == t;
+            const bool mom = c->opt_fuse_mom && remaining == t && last_chunk;
             const bool inpl = c->opt_inplace != 0;
             // auto: shallow passes run faster on the coefficient-form kernel, whose per-plane set-up is leaner (measured
             // crossover, profiles/r02a_README.md: depth 8 in fp32, 6 in fp64); forced kernels are taken as asked
@@ -350,6 +361,7 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
         if (s != MM_OK) return s;
         if (!(fast && c->opt_inplace)) c->cur ^= 1;
         remaining -= t;
+    }
     }
     return MM_OK;
 }
@@ -451,7 +463,10 @@ extern "C" mm_status mm_advance_local(mm_ctx *c, double dt, double cfl)
         return fail(c, MM_ERR_INVALID_ARG, "dt and cfl must be finite and > 0");
     if (c->p.flags & MM_FLAG_RK2_SUPERBEE)
         return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local drives the forward-Euler scheme only (no MM_FLAG_RK2_SUPERBEE yet)");
-    if (c->coupled) return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local does not take the free-motor coupled source yet");
+    if (c->coupled && !((c->opt_kernel == 0 || c->opt_kernel == 5) && MM_AUTO_KERNEL == 5 && stream_supported(c)))
+        return fail(c, MM_ERR_INVALID_ARG, "with the free-motor coupled source mm_advance_local runs on kernel 0 / 5 only (16x16 or 8x8 offset planes)");
+    if (c->coupled && (c->g.nx > 32767 || c->g.ny > 32767))
+        return fail(c, MM_ERR_INVALID_ARG, "the coupled coefficient-form kernels need nx, ny <= 32767");
     if (c->dens_cov_count != c->nc || !c->vel_set) return fail(c, MM_ERR_STATE, "set density and filament velocity first");
     if (c->nc > INT32_MAX) return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local keeps 32-bit configuration lists: nx*ny*ntheta must be < 2^31");
     if (!c->loc_count) {   // the group counts as allocated when its LAST member is (a failed call leaves no half group behind)
@@ -600,6 +615,11 @@ static mm_status free_impl(mm_ctx *c)
     return MM_OK;
 }
 
+static mm_status refresh_free_motors(mm_ctx *c)
+{
+    return c->dtype == MM_F64 ? free_impl<double>(c) : free_impl<float>(c);
+}
+
 extern "C" mm_status mm_update_free_motors(mm_ctx *c, double *Mb_coarse, double *M_free, int on_device)
 {
     if (!c) return MM_ERR_INVALID_ARG;
@@ -659,6 +679,9 @@ extern "C" mm_status mm_set_option(mm_ctx *c, mm_option opt, int64_t v)
     case MM_OPT_FREE_COUPLING:
         if (v && !c->Mf) return fail(c, MM_ERR_STATE, "no free-motor table yet: call mm_update_free_motors first");
         c->coupled = v != 0; return MM_OK;
+    case MM_OPT_FREE_REFRESH:
+        if (v < 0 || v > INT32_MAX) return fail(c, MM_ERR_INVALID_ARG, "MM_OPT_FREE_REFRESH >= 0");
+        c->opt_free_refresh = (int)v; return MM_OK;
     case MM_OPT_INPLACE:
         if (c->single && !v) return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context is always in place");
         c->opt_inplace = v ? 1 : 0; return MM_OK;
@@ -675,6 +698,7 @@ extern "C" mm_status mm_get_option(const mm_ctx *c, mm_option opt, int64_t *v)
     case MM_OPT_FUSE_MOMENTS: *v = c->opt_fuse_mom; return MM_OK;
     case MM_OPT_INPLACE: *v = c->opt_inplace; return MM_OK;
     case MM_OPT_FREE_COUPLING: *v = c->coupled ? 1 : 0; return MM_OK;
+    case MM_OPT_FREE_REFRESH: *v = c->opt_free_refresh; return MM_OK;
     }
     return MM_ERR_INVALID_ARG;
 }

@@ -34,7 +34,7 @@ struct mm_ctx {
     bool mom_valid, vel_set;
     std::vector<uint8_t> dens_cov;  // per configuration: density uploaded
     int64_t dens_cov_count;
-    int opt_kernel, opt_fuse_t, opt_fuse_mom, opt_inplace;
+    int opt_kernel, opt_fuse_t, opt_fuse_mom, opt_inplace, opt_free_refresh;
     bool single;                    // created with ONE density buffer: only the in-place kernels can run
     double checked_dt;              // dt the S8 check last passed with (NaN = none)
     int64_t launches;

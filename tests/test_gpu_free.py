@@ -82,8 +82,12 @@ def test_free_motor_option_and_errors():
     a = np.empty_like(m0); mm.get_density(a)
     assert p1_density(a, orc.run(g, p, U, V, Om, m0, 3, dt)) < 1e-12      # uniform table == constant source
     assert mm.kernel_name.startswith(("tm_mf<", "coef_mf<"))
+    mm.set_option(b.MM_OPT_KERNEL, 4)
     with pytest.raises(MMError):
-        mm.advance_local(dt, 0.4)                     # not with the coupled source
+        mm.advance_local(dt, 0.4)                     # coupled local steps: kernels 0 / 5 only
+    mm.set_option(b.MM_OPT_KERNEL, 0)
+    with pytest.raises(MMError):
+        mm.set_option(b.MM_OPT_FREE_REFRESH, -1)
     mm.set_option(b.MM_OPT_FREE_COUPLING, 0)          # back to the fast path
     mm.substep(1, dt)
     assert mm.kernel_name.startswith(("tm<", "coef<"))
@@ -132,3 +136,41 @@ def test_full_microscale_step_against_the_oracle(dtype):
         assert np.max(np.abs(F2 - F2_o)) / np.max(np.abs(F2_o)) <= tol, step
     assert mm.kernel_name.startswith(("tm_mf<", "coef_mf<"))
     mm.destroy()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("flags,kernel,shape", [(0, 0, (6, 6, 8, 7, 16, 16)), (0, 5, (8, 8, 4, 6, 8, 8)), (0, 1, (5, 4, 4, 5, 6, 6)),
+                                                (mi.FLAG_RK2_SUPERBEE, 0, (6, 6, 8, 7, 16, 16))])
+@pytest.mark.parametrize("refresh", [1, 3])
+def test_alg2_cadence_refresh_inside_substep(dtype, flags, kernel, shape, refresh):
+    """MM_OPT_FREE_REFRESH = k: mm_substep redoes the coarse reduction, the cap and M_f before every k-th substep
+    (k = 1: Alg. 2 l.14-20 inside the inner loop) -- against the oracle's mmo_run_alg2."""
+    from paper_1908_04279_b200 import MM, binding as b
+    from util import p2_moments
+    g = Grid(*shape)
+    big = Params(flags=flags, m_free=1e9)
+    U, V, Om, m0 = random_inputs(g, big, dtype)
+    psi = RNG.random(g.nc) * 30.0
+    _, raw, _ = orc.free_motors(g, big, m0, psi)
+    p = dataclasses.replace(big, m_free=float(np.quantile(raw, 0.6)))
+    dt = mi.benchmark_dt(g, p, 1.0)
+    mm = MM(g, p, dtype)
+    mm.set_option(b.MM_OPT_KERNEL, kernel)
+    mm.set_density(np.ascontiguousarray(m0, NPDT[dtype]))
+    mm.set_filament_velocity(*(np.ascontiguousarray(x, NPDT[dtype]) for x in (U, V, Om)))
+    mm.set_psi(psi)
+    mm.update_free_motors()                      # switches the coupled source on (its table is replaced at substep 0)
+    mm.set_option(b.MM_OPT_FREE_REFRESH, refresh)
+    assert mm.get_option(b.MM_OPT_FREE_REFRESH) == refresh
+    mm.substep(7, dt)
+    f, t = np.empty((g.nc, 2)), np.empty(g.nc)
+    mm.moments(f, t)
+    out = np.empty((g.nc, g.ns, g.nxi, g.neta), NPDT[dtype])
+    mm.get_density(out)
+    name = mm.kernel_name
+    mm.destroy()
+    ref, _, _ = orc.run_alg2(g, p, U, V, Om, m0, psi, 7, dt, refresh)
+    tol = TOL[dtype]
+    assert p1_density(out, ref) <= tol, name
+    ef, et = p2_moments(f, t, orc.moments(g, p, ref))
+    assert ef <= tol and et <= tol, name

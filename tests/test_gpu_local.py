@@ -111,3 +111,45 @@ def test_local_coef_equals_generic_and_moments_standalone():
     assert a[5].startswith("tm_local<") and c[5].startswith("local_generic<")
     assert np.array_equal(a[1], c[1]) and p1_density(a[0], c[0]) < 1e-12
     assert np.allclose(a[3], c[3], rtol=0, atol=1e-13) and np.allclose(a[4], c[4], rtol=0, atol=1e-13)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("nxi", [16, 8])
+def test_local_steps_with_the_coupled_source(dtype, nxi):
+    """Alg. 2 as one loop: local steps whose source is k_on M_f(r0) from the free-motor table (kernel 5, tm_mf_local)."""
+    import dataclasses
+    from paper_1908_04279_b200 import MM, binding as b
+    from util import NPDT, TOL, p1_density, p2_moments
+    g = Grid(5, 7, 12, 7, nxi, nxi)
+    big = Params(m_free=1e9)
+    U, V, Om, m0 = random_inputs(g, big, dtype, omega_max=2.0)
+    rng = np.random.default_rng(5)
+    psi = rng.random(g.nc) * 30.0
+    _, raw, _ = orc.free_motors(g, big, m0, psi)
+    p = dataclasses.replace(big, m_free=float(np.median(raw)))
+    dt = 9.5 / orc.rate_bound(g, p, U, V, Om).mean()            # several passes at depth 4, one at the default depth
+    for fuse_t in (4, None):
+        mm = MM(g, p, dtype)
+        if fuse_t:
+            mm.set_option(b.MM_OPT_FUSE_T, fuse_t)
+        mm.set_density(np.ascontiguousarray(m0, NPDT[dtype]))
+        mm.set_filament_velocity(U, V, Om)
+        mm.set_psi(psi)
+        Mf = np.empty((g.nx, g.ny))
+        mm.update_free_motors(None, Mf)
+        mm.advance_local(dt, 0.4)
+        n = np.empty(g.nc, np.int32)
+        mm.local_steps(n, None)
+        f, t = np.empty((g.nc, 2)), np.empty(g.nc)
+        mm.moments(f, t)
+        out = np.empty((g.nc, g.ns, g.nxi, g.neta), NPDT[dtype])
+        mm.get_density(out)
+        name = mm.kernel_name
+        mm.destroy()
+        capped, _, Mf_ref = orc.free_motors(g, p, m0, psi)
+        ref, n_ref = orc.advance_local(g, p, U, V, Om, capped, dt, 0.4, Mf=Mf_ref)
+        assert name.startswith("tm_mf_local<"), name
+        assert np.array_equal(n, n_ref) and len(set(n.tolist())) > 1
+        assert p1_density(out, ref) <= TOL[dtype], name
+        ef, et = p2_moments(f, t, orc.moments(g, p, ref))
+        assert ef <= TOL[dtype] and et <= TOL[dtype], name

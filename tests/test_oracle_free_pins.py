@@ -184,3 +184,49 @@ def test_n6_one_hot_table_feeds_exactly_the_cells_anchored_on_that_node():
     c0, n = 37, 29
     out = orc.run_coupled(g, p, z[:n], z[:n], z[:n], m0[c0:c0 + n], 1, dt, Mf, c_first=c0)
     assert np.array_equal(out, expect[c0:c0 + n])
+
+
+def test_n7_alg2_cadence():
+    """Alg. 2's loop redoes the coarse reduction, the cap and M_f inside the inner loop.  Pins of
+    `mmo_run_alg2` that do not go through it: (a) with pure detachment (no transport, k_on = 0) and a cap that never
+    binds, the coarse density after n substeps is known in closed form per node: every cell decays by its own
+    (1 - dt kappa)^n, so M_b,coarse of the last update = the binned sum of the decayed initial state -- computed here with
+    numpy from C2's formula, and M_f = M_total - it; (b) refresh >= n_sub is one update followed by the frozen-table run;
+    (c) refresh = 1 with Psi = 0 (nothing counts as bound: M_f = M_total at every update) is the constant-source run,
+    bitwise; (d) the bound-motor budget: while the cap binds, every update leaves M_b,coarse <= M_total exactly."""
+    g = Grid(4, 3, 4, 5, 4, 4)
+    # (a) closed form
+    p = Params(v0=0.0, k_on=0.0, m_free=1e9, R=0.2)
+    inside = mi.inside_mask(g.nxi, g.neta)
+    m0 = RNG.random((g.nc, g.ns, g.nxi, g.neta)) * inside
+    psi = RNG.random(g.nc) + 0.5
+    z = np.zeros(g.nc)
+    dt, n, k = 1e-4, 7, 3                                                       # dt kappa <= 0.25 everywhere
+    out, Mbc, Mf = orc.run_alg2(g, p, z, z, z, m0, psi, n, dt, k)
+    a = np.arange(g.nxi); xi = -p.R + (a + 0.5) * 2 * p.R / g.nxi
+    kap = p.k_off0 * np.exp(p.k_spring * np.sqrt(xi[:, None] ** 2 + xi[None, :] ** 2) / p.f_detach)
+    E = np.ones(g.ns); E[0] = E[-1] = p.end_detach_mult
+    decay = 1.0 - dt * kap[None, :, :] * E[:, None, None]                       # per substep, per (j, a, b)
+    assert (decay > 0.7).all() and np.max(np.abs(out - m0 * decay[None] ** n)) < 1e-14
+    last = (n - 1) // k * k                                                     # substep index of the last update
+    nodx, nody = _anchor_nodes_exact(g, 0.2)
+    w = (2 * np.pi / g.ntheta) * (1.0 / g.ns) * (2 * p.R / g.nxi) ** 2
+    expect = np.zeros((g.nx, g.ny))
+    np.add.at(expect, (nodx.reshape(-1), nody.reshape(-1)), (w * psi[:, None, None, None] * m0 * decay[None] ** last).reshape(-1))
+    assert np.max(np.abs(Mbc - expect)) < 1e-15 * p.m_free and np.max(np.abs(Mf - (p.m_free - expect))) < 1e-6
+    # (b), (c), (d) with transport and a binding cap
+    p = Params(m_free=1.0)
+    U, V, Om = RNG.random(g.nc) - 0.5, RNG.random(g.nc) - 0.5, 2 * RNG.random(g.nc) - 1
+    dt = mi.benchmark_dt(g, p, 1.0)
+    _, raw, _ = orc.free_motors(g, dataclasses.replace(p, m_free=1e9), m0, psi * 50)
+    p = dataclasses.replace(p, m_free=float(np.median(raw)))
+    once, Mbc1, Mf1 = orc.run_alg2(g, p, U, V, Om, m0, psi * 50, 6, dt, 6)
+    capped, Mbc_ref, Mf_ref = orc.free_motors(g, p, m0, psi * 50)
+    assert np.array_equal(once, orc.run_coupled(g, p, U, V, Om, capped, 6, dt, Mf_ref)) and np.array_equal(Mf1, Mf_ref)
+    every, Mbc2, Mf2 = orc.run_alg2(g, p, U, V, Om, m0, psi * 50, 6, dt, 1)
+    assert np.max(np.abs(every - once)) > 1e-6                                  # the cadence matters
+    assert (Mbc2 <= p.m_free).all() and (Mf2 >= 0).all()
+    _, Mbc0, _ = orc.run_alg2(g, p, U, V, Om, m0, psi * 50, 1, dt, 1)
+    assert (Mbc0 == p.m_free).any() and (Mbc0 < p.m_free).any()                 # the cap really binds at the start
+    free, _, Mf3 = orc.run_alg2(g, p, U, V, Om, m0, np.zeros(g.nc), 6, dt, 1)
+    assert np.array_equal(free, orc.run(g, p, U, V, Om, m0, 6, dt)) and np.array_equal(Mf3, np.full((g.nx, g.ny), p.m_free))

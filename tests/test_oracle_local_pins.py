@@ -106,3 +106,29 @@ def test_l4_units_are_independent():
     perm[[1, 1 + g.ntheta]] = perm[[1 + g.ntheta, 1]]
     out2, n2 = orc.advance_local(g, p, U[perm], V[perm], Om[perm], m[perm], dt, 0.4)
     assert np.array_equal(n2, n[perm]) and np.array_equal(out2, out[perm])
+
+
+def test_l5_local_steps_with_the_coupled_source():
+    """Alg. 2 is one loop: local steps (l.5) with the source k_on M_f(r0) (l.20 feeding Eq. 4).  `advance_local(Mf=...)`:
+    the step counts do not depend on the table; a uniform table M_f = m_free is the uncoupled call bitwise; every unit is
+    bitwise its own `run_coupled` with n_c steps of dt / n_c (ties the coupled local call to the pinned coupled run, N4 /
+    N6); and with a one-hot table, no transport and no detachment only the cells anchored on that node change."""
+    import dataclasses
+    g = Grid(4, 3, 4, 6, 6, 6)
+    p = Params(m_free=0.8)
+    rng = np.random.default_rng(77)
+    m0 = rng.random((g.nc, g.ns, g.nxi, g.neta)) * mi.inside_mask(g.nxi, g.neta)
+    U, V, Om = rng.random(g.nc) - 0.5, rng.random(g.nc) - 0.5, 4 * rng.random(g.nc) - 2
+    dt = 5.3 / orc.rate_bound(g, p, U, V, Om).mean()
+    plain, n_plain = orc.advance_local(g, p, U, V, Om, m0, dt, 0.4)
+    same, n_same = orc.advance_local(g, p, U, V, Om, m0, dt, 0.4, Mf=np.full((g.nx, g.ny), 0.8))
+    assert np.array_equal(n_plain, n_same) and np.array_equal(plain, same) and len(set(n_plain.tolist())) > 1
+    Mf = rng.random((g.nx, g.ny))
+    out, n_c = orc.advance_local(g, p, U, V, Om, m0, dt, 0.4, Mf=Mf)
+    assert np.array_equal(n_c, n_plain) and np.max(np.abs(out - plain)) > 1e-4
+    for c in (0, 5, g.nc - 1):
+        ref = orc.run_coupled(g, p, U[c:c + 1], V[c:c + 1], Om[c:c + 1], m0[c:c + 1], int(n_c[c]), dt / n_c[c], Mf, c_first=c)
+        assert np.array_equal(out[c:c + 1], ref)
+    # a slice of configurations keeps its global indices (theta AND the anchor's node)
+    part, _ = orc.advance_local(g, p, U[7:19], V[7:19], Om[7:19], m0[7:19], dt, 0.4, c_first=7, Mf=Mf)
+    assert np.array_equal(part, out[7:19])
