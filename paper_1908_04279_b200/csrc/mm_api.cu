@@ -316,9 +316,11 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
             return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context runs RK2 + Superbee only on the fused in-place kernel (no coupled source, 16x16 or 8x8 offset planes)");
         for (int n = 0; n < n_sub; ++n) {
             if (refresh > 0 && n % refresh == 0) { mm_status fs = refresh_free_motors(c); if (fs != MM_OK) return fs; }
-            mm_status s = fused ? launch_rk2_fused_any(c, dt)
+            const bool mom = fused && c->opt_fuse_mom && n == n_sub - 1;   // moments fused into the last pass
+            mm_status s = fused ? launch_rk2_fused_any(c, dt, mom)
                                 : launch_rk2_generic(c, dt);
             if (s != MM_OK) return s;
+            if (mom) c->mom_valid = true;
         }
         return MM_OK;
     }

@@ -10,6 +10,7 @@
 #include "mm_common.cuh"
 #include "mm_ptx.cuh"
 #include "mm_coef.cuh"   // CoefCfg, CVec, and_mask, rabs
+#include "mm_tm.cuh"     // tensor memory as lane-private scratch
 
 namespace mm {
 
@@ -127,11 +128,40 @@ template <typename real> __device__ __forceinline__ real superbee_half_slope(rea
     return (rcopysign(real(0.25), a) + rcopysign(real(0.25), b)) * t;   // sigma / 2
 }
 
-// KEEPC: keep the coefficient set of plane i-1 in registers for stage 2 of the next iteration (fp32); when false
-// (fp64, where 40 more doubles do not fit) stage 2 rebuilds the set of plane i-2 from the constants block.
+// The coefficient set of plane i-1 (40 values per lane), built for stage 1, is needed again by stage 2 one iteration
+// later: it waits in the warp's block of TENSOR MEMORY (one tcgen05.st, one tcgen05.ld per plane) instead of 40
+// registers (fp32: 254 registers, the occupancy limit) or a second build (fp64, where it did not fit: 0.7 KB of spills
+// per thread in round 1).  KEEPC = true keeps the round-1 register variant selectable.
+// mom != 0: the S9 moments of the new density are reduced in the same pass (as in mm_coef.cuh).
+template <typename real, int QA, int CB>
+struct Rk2Tm {
+    static constexpr int NCV = 5 * QA * CB;                                          // coefficient values per lane
+    static constexpr int NSV = 4 * QA * CB;                                          // stage-2 state values per lane
+    static constexpr int CW = NCV * (int)sizeof(real) / 4;                            // columns of one coefficient set
+    // two coefficient slots (iteration parity: the set of plane i-1 is parked as soon as stage 1 has used it, while
+    // the set of plane i-2 is still waiting for stage 2) + the stage-2 state
+    static constexpr int COLS = tm_pow2_ge((2 * NCV + NSV) * (int)sizeof(real) / 4) < 32 ? 32 : tm_pow2_ge((2 * NCV + NSV) * (int)sizeof(real) / 4);
+};
+// N reals to / from consecutive columns, N = sum of powers of two >= 2
+template <int N, typename real>
+__device__ __forceinline__ void tm_st_any(uint32_t ta, const real *v)
+{
+    constexpr int H = tm_pow2_ge(N) == N ? N : tm_pow2_ge(N) / 2;
+    tm_st<H>(ta, *reinterpret_cast<const real(*)[H]>(v));
+    if constexpr (N > H) tm_st_any<N - H, real>(ta + H * (int)sizeof(real) / 4, v + H);
+}
+template <int N, typename real>
+__device__ __forceinline__ void tm_ld_any(uint32_t ta, real *v)
+{
+    constexpr int H = tm_pow2_ge(N) == N ? N : tm_pow2_ge(N) / 2;
+    tm_ld<H>(ta, *reinterpret_cast<real(*)[H]>(v));
+    if constexpr (N > H) tm_ld_any<N - H, real>(ta + H * (int)sizeof(real) / 4, v + H);
+}
+
 template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, int MINB, bool PM, bool CS, bool KEEPC>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
-    rk2_fused_kernel(const __grid_constant__ KParams<real> kp, const real *__restrict__ in, real *__restrict__ out)
+    rk2_fused_kernel(const __grid_constant__ KParams<real> kp, const real *__restrict__ in, real *__restrict__ out,
+                     double *__restrict__ force, double *__restrict__ torque, int mom)
 {
     using Cfg = CoefCfg<real, NXI, NETA, CB, P, D, WARPS, CS>;
     constexpr int LB = Cfg::LB, G = Cfg::G, QA = Cfg::QA, PLANE = Cfg::PLANE, NK = Cfg::NK, NKV = Cfg::NKV;
@@ -147,18 +177,27 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + Cfg::TABLE_BYTES + (size_t)WARPS * Cfg::WARP_BYTES) +
                      warp * D;
 
+    using TmR = Rk2Tm<real, QA, CB>;
+    static_assert(WARPS == 4, "one tensor-memory lane quarter per warp");
+    uint32_t *tm_slot = reinterpret_cast<uint32_t *>(smem_raw + Cfg::SMEM_BYTES);
     for (int i = threadIdx.x; i < PLANE; i += WARPS * 32) kap_s[i] = kp.kappa[i];
     if (lane == 0) {
 #pragma unroll
         for (int d = 0; d < D; ++d) mbar_init(&full[d], 1);
         mbar_fence_init();
     }
+    if (!KEEPC && warp == 0) tm_alloc(tm_slot, TmR::COLS);
+    tm_fence_before_sync();
     __syncthreads();
+    tm_fence_after_sync();
+    const uint32_t tm_cta = KEEPC ? 0u : *tm_slot;
+    const uint32_t tm_c = tm_cta + ((uint32_t)(warp * 32) << 16);   // this warp's lane quarter
 
     const int g = lane / LB, lb = lane - g * LB;
     const int a0 = g * QA, b0 = lb * CB;
     const bool is_g0 = (g == 0), is_gtop = (g == G - 1), is_l0 = (lb == 0), is_lr = (lb == LB - 1);
     real maskf[QA][CB], srcm[QA][CB], xiq[QA], etab[CB];
+    real FX = 0, FY = 0, TQ = 0, ctc = 0, stc = 0;
     int maskw[QA][CB];
 #pragma unroll
     for (int q = 0; q < QA; ++q) {
@@ -295,6 +334,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
         {
             real acc[QA][CB];
             offsets(x1, Cn, acc);
+            if constexpr (!KEEPC) tm_st_any<TmR::NCV, real>(tm_c + (i & 1) * TmR::CW, &Cn[0][0][0]);   // park it for stage 2 of the next iteration
             const bool valid1 = (j1 >= 0) && (j1 < ns);
 #pragma unroll
             for (int q = 0; q < QA; ++q)
@@ -310,13 +350,26 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
         }
         // ---- stage 2 on plane i-2:  m^{n+1} = mask m + D(m*)
         real bs[QA][CB], Fh2[QA][CB], o[QA][CB];
+        if constexpr (!KEEPC) {   // the state of stage 2 (m*_{i-2}, its difference and lower-face flux, m_{i-2}) waits in tensor memory too
+            real s2[4][QA][CB];
+            tm_wait_st();
+            tm_ld_any<TmR::NSV, real>(tm_c + 2 * TmR::CW, &s2[0][0][0]);
+            tm_wait_ld();
+#pragma unroll
+            for (int q = 0; q < QA; ++q)
+#pragma unroll
+                for (int cb = 0; cb < CB; ++cb) {
+                    xs[q][cb] = s2[0][q][cb]; as_[q][cb] = s2[1][q][cb]; Flo2[q][cb] = s2[2][q][cb]; base2[q][cb] = s2[3][q][cb];
+                }
+        }
         {
             real acc[QA][CB];
             if constexpr (KEEPC) {
                 offsets(xs, Cp, acc);
             } else {
                 real C2[5][QA][CB];
-                build(j2, C2);
+                tm_ld_any<TmR::NCV, real>(tm_c + ((i + 1) & 1) * TmR::CW, &C2[0][0][0]);   // the set of plane i-2, parked one iteration ago
+                tm_wait_ld();
                 offsets(xs, C2, acc);
             }
 #pragma unroll
@@ -339,12 +392,49 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     for (int e = 0; e < VW; ++e) v.v[e] = o[q][v4 * VW + e];
                     *reinterpret_cast<V128 *>(oc + (int64_t)j2 * PLANE + (a0 + q) * NETA + b0 + v4 * VW) = v;
                 }
+            if (mom) {   // S9 partial sums of the new density
+                const real sj2 = kp.s_lo + (real(j2) + real(0.5)) * kp.ds;
+                real fxp = 0, fyp = 0;
+#pragma unroll
+                for (int q = 0; q < QA; ++q) {
+                    real rs = o[q][0];
+#pragma unroll
+                    for (int cb = 1; cb < CB; ++cb) rs += o[q][cb];
+                    fxp = fma(xiq[q], rs, fxp);
+                }
+#pragma unroll
+                for (int cb = 0; cb < CB; ++cb) {
+                    real csum = o[0][cb];
+#pragma unroll
+                    for (int q = 1; q < QA; ++q) csum += o[q][cb];
+                    fyp = fma(etab[cb], csum, fyp);
+                }
+                FX += fxp;
+                FY += fyp;
+                TQ = fma(sj2, ctc * fyp - stc * fxp, TQ);
+            }
         }
         // ---- rotate the state
+        if constexpr (!KEEPC) {
+            real s2[4][QA][CB];
+#pragma unroll
+            for (int q = 0; q < QA; ++q)
+#pragma unroll
+                for (int cb = 0; cb < CB; ++cb) {
+                    s2[0][q][cb] = ms[q][cb]; s2[1][q][cb] = bs[q][cb]; s2[2][q][cb] = Fh2[q][cb]; s2[3][q][cb] = x1[q][cb];
+                }
+            tm_st_any<TmR::NSV, real>(tm_c + 2 * TmR::CW, &s2[0][0][0]);
+        }
 #pragma unroll
         for (int q = 0; q < QA; ++q)
 #pragma unroll
             for (int cb = 0; cb < CB; ++cb) {
+                if constexpr (!KEEPC) {   // only stage 1's state stays in registers
+                    x1[q][cb] = y[q][cb];
+                    a1[q][cb] = b1[q][cb];
+                    Flo1[q][cb] = Fh1[q][cb];
+                    continue;
+                }
                 base2[q][cb] = x1[q][cb];
                 x1[q][cb] = y[q][cb];
                 a1[q][cb] = b1[q][cb];
@@ -368,6 +458,17 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             oc = out + c * inner;
             const int kth = (int)(c % kp.ntheta);
             const real ct = kp.cos_t[kth], st = kp.sin_t[kth];
+            ctc = ct; stc = st;
+            FX = FY = TQ = real(0);
+            if constexpr (!KEEPC) {   // the parked set read by the first (ghost) stage 2 of this configuration: zeros
+                real z[TmR::NCV + TmR::NSV];
+#pragma unroll
+                for (int e = 0; e < TmR::NCV + TmR::NSV; ++e) z[e] = real(0);
+                tm_wait_st();
+                tm_st_any<TmR::NCV, real>(tm_c, z);
+                tm_st_any<TmR::NCV, real>(tm_c + TmR::CW, z);
+                tm_st_any<TmR::NSV, real>(tm_c + 2 * TmR::CW, z);
+            }
             const real U = kp.U[c], Vv = kp.V[c], Om = kp.Om[c];
             hbx = -hdx * Om * st;
             hbe = hde * Om * ct;
@@ -417,7 +518,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
 
         mbar_wait(&full[slot], phase);
         const real *sp = ring + (size_t)slot * P * PLANE;
-#pragma unroll
+        constexpr int UNRP = sizeof(real) == 8 ? 1 : P;   // fp64: one copy of the iteration body (register pressure)
+#pragma unroll UNRP
         for (int pl = 0; pl < P; ++pl) {
             const int j = ch * P + pl;
             if (j < ns) {
@@ -447,9 +549,23 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 for (int cb = 0; cb < CB; ++cb) z[q][cb] = real(0);
 #pragma unroll 1
             for (int e = 0; e < 2; ++e) iter(ns + e, z);
+            if (mom) {   // S9: fp64 from the cross-lane reduction on
+                double fx = warp_sum((double)FX), fy = warp_sum((double)FY), tq = warp_sum((double)TQ);
+                if (lane == 0) {
+                    force[2 * c] = kp.mom_scale * fx;
+                    force[2 * c + 1] = kp.mom_scale * fy;
+                    torque[c] = kp.mom_scale * tq;
+                }
+            }
             ch = 0;
             ++k;
         }
+    }
+    if constexpr (!KEEPC) {
+        tm_wait_st();
+        tm_fence_before_sync();
+        __syncthreads();
+        if (warp == 0) tm_dealloc(tm_cta, TmR::COLS);
     }
 }
 

@@ -127,7 +127,7 @@ __device__ __forceinline__ void tm_st(uint32_t ta, const double (&v)[N])
 __device__ __forceinline__ uint32_t rbits_or(uint32_t o, float v) { return o | __float_as_uint(v); }
 __device__ __forceinline__ uint32_t rbits_or(uint32_t o, double v) { return o | (uint32_t)__double2hiint(v) | (uint32_t)__double2loint(v); }
 
-constexpr int tm_pow2_ge(int n) { int p = 1; while (p < n) p *= 2; return p; }
+__host__ __device__ constexpr int tm_pow2_ge(int n) { int p = 1; while (p < n) p *= 2; return p; }
 
 template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, int MINB>
 struct TmCfg {
