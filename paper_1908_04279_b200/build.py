@@ -21,7 +21,8 @@ MM_H = os.path.join(os.path.dirname(HERE), "include", "mm.h")
 UNITS = ("mm_api", "mm_launch_tm", "mm_launch_coef", "mm_launch_stream_tile", "mm_launch_rk2")
 SOURCES = [os.path.join(CSRC, u + ".cu") for u in UNITS]
 CFLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
-LFLAGS = ["-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a"]
+LFLAGS = ["-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a",
+          "-Xlinker", "--version-script=" + os.path.join(CSRC, "libmm.map")]
 
 
 def nvcc() -> str:
@@ -65,7 +66,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
                 if rc != 0:
                     raise subprocess.CalledProcessError(rc, cmd)
     objs = [os.path.join(OBJ, u + ".o") for u in UNITS]
-    if jobs or _stale(SO, objs):
+    if jobs or _stale(SO, objs + [os.path.join(CSRC, "libmm.map")]):
         subprocess.check_call([cc] + LFLAGS + ["-o", SO] + objs)
     return SO
 

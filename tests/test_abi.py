@@ -22,6 +22,12 @@ def test_library_exports_every_declared_symbol():
     L = b.lib()
     for name in declared:
         assert hasattr(L, name), name
+    # ... and nothing else: launchers and kernel stubs stay local (csrc/libmm.map)
+    import subprocess
+    from paper_1908_04279_b200 import build as mm_build
+    out = subprocess.run(["nm", "-D", "--defined-only", mm_build.SO], capture_output=True, text=True).stdout
+    exported = {l.split()[-1] for l in out.splitlines() if len(l.split()) == 3 and l.split()[1] in "TDBR"}
+    assert exported == declared, exported ^ declared
 
 
 def test_struct_layout_matches_header():
