@@ -20,8 +20,9 @@
  * C2 pure detachment closed form, C3 exact shift at CFL=1, C4 steady-state recursion,
  * C5 brute-force/analytic moments on 2x2x2x4x3x3, C6 single-cell delta column, C7 point
  * symmetry, C8 independence/additivity, C9 positivity/affinity; the NEXT-row functions further down by R1-R7
- * (RK2 + Superbee), L1-L4 (local time step), F1-F5 (force spreading), N1-N5 (free-motor coupling).  No function is
- * unpinned.
+ * (RK2 + Superbee), L1-L5 (local time step; L5: with the coupled source), F1-F5 (force spreading), N1-N7 (free-motor
+ * coupling; N6: which node a cell's coupled source is read from, one-hot tables against the exact-rational anchor map;
+ * N7: Alg. 2's cadence, mmo_run_alg2).  No function is unpinned.
  *
  * Second scheme (flag MMO_RK2_SUPERBEE): the paper's own integrator --
  * Runge-Kutta 2 through the half step (Alg. 2 l.9-10: "Compute M_b(t^* + dt^* / 2)",
