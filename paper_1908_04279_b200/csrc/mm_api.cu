@@ -131,7 +131,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->loc_valid = false;
     c->psi = c->fline = c->F2 = nullptr; c->psi_set = false;
     c->Mf = c->Mbc = c->free_raw = c->free_factor = nullptr; c->free_fx = nullptr; c->free_any = nullptr; c->coupled = false;
-    c->mom_valid = c->vel_set = false; c->tile_ok = false;
+    c->mom_valid = c->vel_set = false; c->tile_ok = false; c->fline_valid = false;
     c->dens_cov_count = 0;
     // measured defaults: the upwind-sparse tensor-memory kernel, at most MM_MAX_FUSE_T
     // substeps per pass (with MM_AUTO_KERNEL = 4: the coefficient-form kernel at depth 10 / 5)
@@ -227,7 +227,7 @@ extern "C" mm_status mm_set_density_range(mm_ctx *c, int64_t c_begin, int64_t n,
     if (s != MM_OK) return s;
     for (int64_t i = c_begin; i < c_begin + n; ++i)
         if (!c->dens_cov[(size_t)i]) { c->dens_cov[(size_t)i] = 1; c->dens_cov_count++; }
-    c->mom_valid = false;
+    c->mom_valid = false; c->fline_valid = false;
     return MM_OK;
 }
 extern "C" mm_status mm_set_density(mm_ctx *c, const void *src, int on_device)
@@ -303,7 +303,7 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
     if (kind == 2 && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "streamed kernel does not support this grid/flags");
     if (fast && !stream_supported(c)) return fail(c, MM_ERR_INVALID_ARG, "coefficient-form kernels do not support this grid/flags");
     if (kind == 3 && !c->tile_ok) return fail(c, MM_ERR_INVALID_ARG, "tile kernel does not support this grid/flags");
-    c->mom_valid = false;
+    c->mom_valid = false; c->fline_valid = false;
     const int refresh = c->coupled ? c->opt_free_refresh : 0;
     if (refresh > 0 && !c->psi_set) return fail(c, MM_ERR_STATE, "MM_OPT_FREE_REFRESH needs mm_set_psi");
     if (c->p.flags & MM_FLAG_RK2_SUPERBEE) {
@@ -328,7 +328,7 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
     // substep, so a chunk of at most k substeps is fused between two updates
     for (int n0 = 0; n0 < n_sub; n0 += (refresh > 0 ? refresh : n_sub)) {
     int remaining = refresh > 0 ? (n_sub - n0 < refresh ? n_sub - n0 : refresh) : n_sub;
-    if (refresh > 0) { mm_status fs = refresh_free_motors(c); if (fs != MM_OK) return fs; c->mom_valid = false; }
+    if (refresh > 0) { mm_status fs = refresh_free_motors(c); if (fs != MM_OK) return fs; c->mom_valid = false; c->fline_valid = false; }
     const bool last_chunk = refresh <= 0 || n0 + remaining == n_sub;   // moments are fused into the call's last pass only
     while (remaining > 0) {
         mm_status s;
@@ -358,7 +358,7 @@ extern "C" mm_status mm_substep(mm_ctx *c, int32_t n_sub, double dt)
                 : pk == 4 ? launch_coef(c, t, mom, dt, c->buf[c->cur], c->buf[inpl ? c->cur : c->cur ^ 1])
                 : pk == 5 ? launch_tm(c, t, mom, dt, c->buf[c->cur], c->buf[inpl ? c->cur : c->cur ^ 1], false, 0, false)
                             : launch_tile(c, t, mom, dt, c->cur, c->buf[c->cur ^ 1]);
-            if (s == MM_OK && mom) c->mom_valid = true;
+            if (s == MM_OK && mom) { c->mom_valid = true; c->fline_valid = (pk == 5 && c->fline != nullptr); }
         }
         if (s != MM_OK) return s;
         if (!(fast && c->opt_inplace)) c->cur ^= 1;
@@ -397,7 +397,7 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     const int32_t nmax = nmm[0], nmin = -nmm[1];
     c->loc_valid = true;
-    c->mom_valid = false;
+    c->mom_valid = false; c->fline_valid = false;
     // kernel choice: 0 auto = the coefficient-form local-step kernel where the grid is supported, else (or 1) generic
     if (c->opt_kernel != 0 && c->opt_kernel != 1 && c->opt_kernel != 4 && c->opt_kernel != 5)
         return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local runs on kernel 0 (auto), 1 (generic), 4 (coefficient form) or 5 (upwind-sparse)");
@@ -439,7 +439,7 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
             }
             if (s != MM_OK) return s;
         }
-        if (c->opt_fuse_mom) c->mom_valid = true;
+        if (c->opt_fuse_mom) { c->mom_valid = true; c->fline_valid = tm && c->fline != nullptr; }
         return MM_OK;
     }
     if (c->single) return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context runs only the in-place kernels");
@@ -521,11 +521,15 @@ static mm_status spread_impl(mm_ctx *c)
     int64_t blocks = (c->nc + 7) / 8;
     const int64_t cap = (int64_t)c->sm_count * 8;
     if (blocks > cap) blocks = cap;
-    if (plane % VWF == 0)
-        plane_force_kernel<real, VWF><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, dens, c->fline);
-    else
-        plane_force_kernel<real, 1><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, dens, c->fline);
-    CUDA_TRY(c, cudaGetLastError());
+    if (!c->fline_valid) {   // else: the last pass of mm_substep / mm_advance_local already wrote the plane forces
+        if (plane % VWF == 0)
+            plane_force_kernel<real, VWF><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, dens, c->fline);
+        else
+            plane_force_kernel<real, 1><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, dens, c->fline);
+        CUDA_TRY(c, cudaGetLastError());
+        c->launches++;
+        c->fline_valid = true;
+    }
     CUDA_TRY(c, cudaMemsetAsync(c->F2, 0, (size_t)c->g.nx * c->g.ny * 2 * sizeof(double), c->stream));
     const int64_t total = c->nc * c->g.ns * 4;
     int64_t sb = (total + 255) / 256;
@@ -534,7 +538,7 @@ static mm_status spread_impl(mm_ctx *c)
     spread_kernel<<<(unsigned)sb, 256, 0, c->stream>>>(c->nc, c->g.ns, c->g.nx, c->g.ny, c->g.ntheta, c->p.s_lo,
                                                        (c->p.s_hi - c->p.s_lo) / c->g.ns, c->psi, c->fline, c->F2);
     CUDA_TRY(c, cudaGetLastError());
-    c->launches += 2;
+    c->launches += 1;
     return MM_OK;
 }
 
@@ -642,7 +646,7 @@ extern "C" mm_status mm_update_free_motors(mm_ctx *c, double *Mb_coarse, double 
     mm_status s = c->dtype == MM_F64 ? free_impl<double>(c) : free_impl<float>(c);
     if (s != MM_OK) return s;
     c->coupled = true;
-    c->mom_valid = false;     // the cap may have rescaled the density
+    c->mom_valid = false; c->fline_valid = false;     // the cap may have rescaled the density
     const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     if (Mb_coarse) CUDA_TRY(c, cudaMemcpyAsync(Mb_coarse, c->Mbc, nn * sizeof(double), kind, c->stream));
     if (M_free) CUDA_TRY(c, cudaMemcpyAsync(M_free, c->Mf, nn * sizeof(double), kind, c->stream));

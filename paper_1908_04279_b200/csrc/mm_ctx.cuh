@@ -44,7 +44,7 @@ struct mm_ctx {
     void *loc_dt;
     bool loc_valid;
     double *psi, *fline, *F2;       // NEXT-4: filament density weights [nc], plane forces [nc][ns][2], fluid-grid force
-    bool psi_set;
+    bool psi_set, fline_valid;      // fline_valid: fline holds the plane forces of the CURRENT density
     double *Mf, *Mbc, *free_raw, *free_factor;   // NEXT-2: free / coarse bound motor tables [nx][ny], scratch
     unsigned long long *free_fx;   // [nx][ny][2]: the coarse sums in 128-bit fixed point (mm_free.cuh)
     int *free_any;

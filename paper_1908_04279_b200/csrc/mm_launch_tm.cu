@@ -38,14 +38,14 @@ struct TmShape {
     using Cfg = TmCfg<real, NXI, NETA, CB, P, D, WARPS, MINB>;
 };
 
-template <typename real, int NXI, int NETA, int CB, bool MF, bool LOC>
+template <typename real, int NXI, int NETA, int CB, bool MF, bool LOC, bool PF>
 static mm_status launch_tm_inst(mm_ctx *c, int nlev, bool mom, double dt, const void *in, void *out, int32_t done, bool use_list)
 {
     constexpr bool local = LOC;
     using S = TmShape<real, NXI, NETA, CB>;
     using Cfg = typename S::Cfg;
     constexpr int WARPS = S::WARPS;
-    auto kern = substep_tm_kernel<real, NXI, NETA, CB, S::P, S::D, WARPS, S::MINB, MF, LOC>;
+    auto kern = substep_tm_kernel<real, NXI, NETA, CB, S::P, S::D, WARPS, S::MINB, MF, LOC, PF>;
     if (nlev < 1 || nlev > Cfg::TMAX) return fail(c, MM_ERR_INVALID_ARG, "fuse depth beyond the tensor-memory budget of the kernel");
     // MF: the warps' node tables (16-bit, ns * (NXI + NETA) entries each) sit behind the regular layout
     const size_t smem = MF ? ((Cfg::SMEM_BYTES + 15) / 16) * 16 + (size_t)WARPS * c->g.ns * (NXI + NETA) * 2 : Cfg::SMEM_BYTES;
@@ -77,7 +77,8 @@ static mm_status launch_tm_inst(mm_ctx *c, int nlev, bool mom, double dt, const 
                                                            mom ? 1 : 0, local ? c->loc_n : nullptr,
                                                            local ? (const real *)c->loc_dt : nullptr, done,
                                                            (local && use_list) ? c->loc_list : nullptr,
-                                                           (local && use_list) ? c->loc_count : nullptr);
+                                                           (local && use_list) ? c->loc_count : nullptr,
+                                                           PF ? c->fline : nullptr);
     CUDA_TRY(c, cudaGetLastError());
     c->launches++;
     snprintf(c->kname, sizeof c->kname, "%s<%s,%dx%d,CB=%d,T%s%d%s>", MF ? (local ? "tm_mf_local" : "tm_mf") : (local ? "tm_local" : "tm"),
@@ -89,11 +90,13 @@ template <typename real, int NXI, int NETA, int CB>
 static mm_status launch_tm_shape(mm_ctx *c, int nlev, bool mom, double dt, const void *in, void *out, bool local, int32_t done,
                                  bool use_list)
 {
-    if (local)
-        return c->coupled ? launch_tm_inst<real, NXI, NETA, CB, true, true>(c, nlev, mom, dt, in, out, done, use_list)
-                          : launch_tm_inst<real, NXI, NETA, CB, false, true>(c, nlev, mom, dt, in, out, done, use_list);
-    return c->coupled ? launch_tm_inst<real, NXI, NETA, CB, true, false>(c, nlev, mom, dt, in, out, done, use_list)
-                      : launch_tm_inst<real, NXI, NETA, CB, false, false>(c, nlev, mom, dt, in, out, done, use_list);
+    // PF: the pass that reduces the moments also stores the plane forces when mm_spread_force is in use
+    const bool pf = mom && c->fline != nullptr;
+#define MM_TM_GO(MF_, LOC_) (pf ? launch_tm_inst<real, NXI, NETA, CB, MF_, LOC_, true>(c, nlev, mom, dt, in, out, done, use_list) \
+                                : launch_tm_inst<real, NXI, NETA, CB, MF_, LOC_, false>(c, nlev, mom, dt, in, out, done, use_list))
+    if (local) return c->coupled ? MM_TM_GO(true, true) : MM_TM_GO(false, true);
+    return c->coupled ? MM_TM_GO(true, false) : MM_TM_GO(false, false);
+#undef MM_TM_GO
 }
 
 mm_status launch_tm(mm_ctx *c, int nlev, bool mom, double dt, const void *in, void *out, bool local, int32_t done, bool use_list)

@@ -169,18 +169,25 @@ __device__ __forceinline__ void tm_level(const TmCoef<real, QA, CB> &k, const re
         if (!(SK & 8)) rt[q] = shfl_down_r(xi[q][0], 1);
         if (!(SK & 4)) lf[q] = shfl_up_r(xi[q][CB - 1], 1);
     }
-    real Pn[QA * CB];
+    tm_wait_ld();
+    // the old carry is consumed at once (its registers die before the new one is staged for the store)
 #pragma unroll
     for (int q = 0; q < QA; ++q)
 #pragma unroll
-        for (int cb = 0; cb < CB; ++cb) Pn[q * CB + cb] = fma(k.csm[q][cb], xi[q][cb], k.src[q][cb]);
-    tm_wait_ld();
-    tm_st<QA * CB>(ta, Pn);
+        for (int cb = 0; cb < CB; ++cb) xo[q][cb] = fma(k.c0j[q][cb], xi[q][cb], Pl[q * CB + cb]);
+    {
+        real Pn[QA * CB];
+#pragma unroll
+        for (int q = 0; q < QA; ++q)
+#pragma unroll
+            for (int cb = 0; cb < CB; ++cb) Pn[q * CB + cb] = fma(k.csm[q][cb], xi[q][cb], k.src[q][cb]);
+        tm_st<QA * CB>(ta, Pn);
+    }
 #pragma unroll
     for (int q = 0; q < QA; ++q)
 #pragma unroll
         for (int cb = 0; cb < CB; ++cb) {
-            real acc = fma(k.c0j[q][cb], xi[q][cb], Pl[q * CB + cb]);
+            real acc = xo[q][cb];
             if (!(SK & 1) && q > 0) acc = fma(k.cxm[q][cb], xi[q > 0 ? q - 1 : 0][cb], acc);
             if (!(SK & 2) && q + 1 < QA) acc = fma(k.cxp[q][cb], xi[q + 1 < QA ? q + 1 : 0][cb], acc);
             if (!(SK & 4) && cb > 0) acc = fma(k.cem[q][cb], xi[q][cb > 0 ? cb - 1 : 0], acc);
@@ -218,12 +225,13 @@ __device__ __forceinline__ void tm_plane(const TmCoef<real, QA, CB> &k, real (&x
 // nlev: substeps this pass fuses (<= TmCfg::TMAX); mom: also reduce the S9 moments.  Local-step mode (LOC):
 // configuration c takes clamp(n_steps[c] - done, 0, nlev) steps of its own size dt_c[c]; `kp` then carries the factors
 // per unit dt; `list` as in mm_coef.cuh.
-template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, int MINB, bool MF, bool LOC>
+template <typename real, int NXI, int NETA, int CB, int P, int D, int WARPS, int MINB, bool MF, bool LOC, bool PF = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
     substep_tm_kernel(const __grid_constant__ KParams<real> kp, const real *__restrict__ in, real *__restrict__ out,
                       double *__restrict__ force, double *__restrict__ torque, int nlev_pass, int mom,
                       const int32_t *__restrict__ n_steps, const real *__restrict__ dt_c, int32_t done,
-                      const int32_t *__restrict__ list, const int32_t *__restrict__ list_count)
+                      const int32_t *__restrict__ list, const int32_t *__restrict__ list_count,
+                      double *__restrict__ fline)
 {
     using Cfg = TmCfg<real, NXI, NETA, CB, P, D, WARPS, MINB>;
     using Co = typename Cfg::Co;
@@ -530,6 +538,17 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 FX += fxp;
                 FY += fyp;
                 TQ = fma(sj, ct * fyp - st * fxp, TQ);
+                if (PF && last_pass) {   // PF: compiled only into the instances launched with a plane-force buffer
+                    // NEXT-4: the spring force carried by this plane, f_j(c) = -k dxi deta sum_ab (xi_a, eta_b) m, is the
+                    // pair of sums just formed: reduce both across the warp in one butterfly (lanes 0-15 gather the xi
+                    // sum, lanes 16-31 the eta sum) and store them for mm_spread_force -- no separate read of the density
+                    real a = (lane & 16) ? fyp : fxp;
+                    const real b = (lane & 16) ? fxp : fyp;
+                    a += __shfl_xor_sync(0xffffffffu, b, 16);
+#pragma unroll
+                    for (int o = 8; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                    if ((lane & 15) == 0) fline[(c * ns + j) * 2 + (lane >> 4)] = (kp.mom_scale / kp.geo_ds) * (double)a;
+                }
             }
         }
         // every lane has consumed this slot (its values fed the stores above): refill it
