@@ -157,12 +157,14 @@ mm_status mm_substep(mm_ctx *ctx, int32_t n_sub, double dt);
 /* local adaptive time step per independent unit ("We instead compute a local
  * dt* for each r0 ... and update M_b at each r0 asynchronously"; Alg. 2 l.2-5).
  * Advances EVERY configuration c from t to t + dt with its own n_c = max(1, ceil(dt lambda_c / cfl)) forward-Euler
- * steps of equal size dt / n_c, where lambda_c is the S8 positivity rate maximised over the disc cells of c
+ * steps (or RK2 + Superbee steps, see below) of equal size dt / n_c, where lambda_c is the S8 positivity rate maximised over the disc cells of c
  * (readings Q31-Q33 in DESIGN.md).  lambda_c and n_c are computed on the device in fp64 in every dtype; the number
  * of passes (max_c n_c) is read back once per call (one 4-byte copy; the call synchronises the stream for it).
  * With the coupled source (MM_OPT_FREE_COUPLING) the local steps take k_on M_f(r0) from the frozen table -- Alg. 2 as one
  * loop (l.5 with l.20's M_f) -- on kernels 0 / 5.  dt > 0, cfl > 0, finite; MM_ERR_STATE unless density and velocities
- * have been set; MM_ERR_INVALID_ARG with MM_FLAG_RK2_SUPERBEE (not supported on this call). */
+ * have been set.  With MM_FLAG_RK2_SUPERBEE every local step is the paper's two-stage scheme (Alg. 2 l.5 driving
+ * l.9-10) on the generic stage kernels: any grid, coupled source or not, two density buffers (single-buffer context:
+ * MM_ERR_INVALID_ARG), two launches per local step. */
 mm_status mm_advance_local(mm_ctx *ctx, double dt, double cfl);
 /* n_c [Nc] (int32) and lambda_c [Nc] (fp64) of the last mm_advance_local; either pointer may be NULL.
  * MM_ERR_STATE before the first mm_advance_local or after new velocities were set. */

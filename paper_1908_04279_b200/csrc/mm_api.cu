@@ -398,6 +398,15 @@ static mm_status advance_local_impl(mm_ctx *c, double dt, double cfl)
     const int32_t nmax = nmm[0], nmin = -nmm[1];
     c->loc_valid = true;
     c->mom_valid = false; c->fline_valid = false;
+    if (c->p.flags & MM_FLAG_RK2_SUPERBEE) {
+        // Alg. 2 as one loop with the paper's scheme (l.5 driving l.9-10), any grid, coupled source or not: the generic
+        // stage kernels, one local step of every unfinished unit per pair of launches
+        for (int32_t step = 0; step < nmax; ++step) {
+            mm_status s = launch_rk2_local_generic(c, step);
+            if (s != MM_OK) return s;
+        }
+        return MM_OK;
+    }
     // kernel choice: 0 auto = the coefficient-form local-step kernel where the grid is supported, else (or 1) generic
     if (c->opt_kernel != 0 && c->opt_kernel != 1 && c->opt_kernel != 4 && c->opt_kernel != 5)
         return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local runs on kernel 0 (auto), 1 (generic), 4 (coefficient form) or 5 (upwind-sparse)");
@@ -463,11 +472,11 @@ extern "C" mm_status mm_advance_local(mm_ctx *c, double dt, double cfl)
     if (!c) return MM_ERR_INVALID_ARG;
     if (!(std::isfinite(dt) && dt > 0) || !(std::isfinite(cfl) && cfl > 0))
         return fail(c, MM_ERR_INVALID_ARG, "dt and cfl must be finite and > 0");
-    if (c->p.flags & MM_FLAG_RK2_SUPERBEE)
-        return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local drives the forward-Euler scheme only (no MM_FLAG_RK2_SUPERBEE yet)");
-    if (c->coupled && !((c->opt_kernel == 0 || c->opt_kernel == 5) && MM_AUTO_KERNEL == 5 && stream_supported(c)))
+    const bool rk2 = (c->p.flags & MM_FLAG_RK2_SUPERBEE) != 0;
+    if (rk2 && c->single) return fail(c, MM_ERR_INVALID_ARG, "local RK2 + Superbee steps run on the generic stages: two density buffers");
+    if (!rk2 && c->coupled && !((c->opt_kernel == 0 || c->opt_kernel == 5) && MM_AUTO_KERNEL == 5 && stream_supported(c)))
         return fail(c, MM_ERR_INVALID_ARG, "with the free-motor coupled source mm_advance_local runs on kernel 0 / 5 only (16x16 or 8x8 offset planes)");
-    if (c->coupled && (c->g.nx > 32767 || c->g.ny > 32767))
+    if (!rk2 && c->coupled && (c->g.nx > 32767 || c->g.ny > 32767))
         return fail(c, MM_ERR_INVALID_ARG, "the coupled coefficient-form kernels need nx, ny <= 32767");
     if (c->dens_cov_count != c->nc || !c->vel_set) return fail(c, MM_ERR_STATE, "set density and filament velocity first");
     if (c->nc > INT32_MAX) return fail(c, MM_ERR_INVALID_ARG, "mm_advance_local keeps 32-bit configuration lists: nx*ny*ntheta must be < 2^31");

@@ -128,5 +128,6 @@ mm_status launch_coef(mm_ctx *c, int T, bool mom, double dt, const void *in, voi
 mm_status launch_coef_local(mm_ctx *c, bool mom, const void *in, void *out, int32_t done, bool use_list);
 mm_status launch_rk2_generic(mm_ctx *c, double dt);                                                     // mm_launch_rk2.cu
 mm_status launch_rk2_fused_any(mm_ctx *c, double dt, bool mom);
+mm_status launch_rk2_local_generic(mm_ctx *c, int32_t step);
 int tm_max_levels(const mm_ctx *c);                                                                     // mm_launch_tm.cu
 mm_status launch_tm(mm_ctx *c, int nlev, bool mom, double dt, const void *in, void *out, bool local, int32_t done, bool use_list);

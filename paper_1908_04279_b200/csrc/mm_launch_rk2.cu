@@ -19,6 +19,29 @@ static mm_status launch_rk2_generic_t(mm_ctx *c, double dt)
     return MM_OK;
 }
 
+// One LOCAL RK2 + Superbee step of every unit that still owes one (step < n_c), each with its own dt_c (generic stages)
+template <typename real>
+static mm_status launch_rk2_local_generic_t(mm_ctx *c, int32_t step)
+{
+    int64_t blocks = (c->cells + 255) / 256;
+    const int64_t cap = (int64_t)c->sm_count * 64;
+    if (blocks > cap) blocks = cap;
+    real *A = (real *)c->buf[c->cur], *B = (real *)c->buf[c->cur ^ 1];
+    const KParams<real> kp = make_kparams<real>(c, 1.0);   // per unit dt
+    rk2_stage_generic_kernel<real><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, A, A, B, c->loc_n, (const real *)c->loc_dt, step, real(0.5));
+    CUDA_TRY(c, cudaGetLastError());
+    rk2_stage_generic_kernel<real><<<(unsigned)blocks, 256, 0, c->stream>>>(kp, A, B, A, c->loc_n, (const real *)c->loc_dt, step, real(1));
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches += 2;
+    snprintf(c->kname, sizeof c->kname, "rk2_local_generic<%s>", sizeof(real) == 8 ? "f64" : "f32");
+    return MM_OK;
+}
+
+mm_status launch_rk2_local_generic(mm_ctx *c, int32_t step)
+{
+    return c->dtype == MM_F64 ? launch_rk2_local_generic_t<double>(c, step) : launch_rk2_local_generic_t<float>(c, step);
+}
+
 // One RK2 + Superbee substep in one HBM pass (rk2_fused_kernel): reads buf[cur], writes buf[cur^1].
 #ifndef MM_RK2_MINB_F32
 #define MM_RK2_MINB_F32 2

@@ -32,10 +32,14 @@ template <typename real> __device__ __forceinline__ real superbee_slope(real a, 
 
 // One RK2 stage, one thread per cell, any grid, all flags:  out = inside ? base + dt L(state) : 0, with the
 // dt-dependent factors of `kp` built for this stage's dt.  `base` and `out` may alias (stage 2).
+// Local-step mode (n_steps != NULL; NEXT-3 with NEXT-1, Alg. 2 l.5 driving l.9-10): `kp` carries the factors per unit
+// dt, configuration c takes the stage with dt = stage * dt_c[c] while step < n_steps[c] and is left untouched after.
 template <typename real>
 __global__ void __launch_bounds__(256) rk2_stage_generic_kernel(const __grid_constant__ KParams<real> kp,
                                                                 const real *base, const real *__restrict__ state,
-                                                                real *out)
+                                                                real *out, const int32_t *__restrict__ n_steps = nullptr,
+                                                                const real *__restrict__ dt_c = nullptr, int32_t step = 0,
+                                                                real stage = real(1))
 {
     const int ns = kp.ns, nxi = kp.nxi, neta = kp.neta;
     const int64_t plane = (int64_t)nxi * neta, inner = plane * ns, total = inner * kp.nc;
@@ -43,6 +47,7 @@ __global__ void __launch_bounds__(256) rk2_stage_generic_kernel(const __grid_con
     for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
          idx += (int64_t)gridDim.x * blockDim.x) {
         const int64_t c = idx / inner;
+        if (n_steps && step >= n_steps[c]) continue;   // this unit has reached t + dt
         int rem = (int)(idx - c * inner);
         const int j = rem / (int)plane;
         rem -= j * (int)plane;
@@ -96,9 +101,17 @@ __global__ void __launch_bounds__(256) rk2_stage_generic_kernel(const __grid_con
         // ---- reactions (S6) and update (S7) from the base level
         const bool endc = (j < kp.n_end) || (j >= ns - kp.n_end);
         const real kap = kp.kappa[rem];
-        real acc = base[idx] - kp.dt_ds * div_s - kp.dt_dxi * (Fxh - Fxl) - kp.dt_deta * (Feh - Fel);
-        acc += source_increment(kp, c, j, a, b) - kp.dt * kap * m;
-        if (endc) acc -= kp.dt_endx * kap * m;
+        real acc;
+        if (n_steps) {   // factors per unit dt, scaled by this unit's stage step
+            real rhs = -kp.dt_ds * div_s - kp.dt_dxi * (Fxh - Fxl) - kp.dt_deta * (Feh - Fel);
+            rhs += source_increment(kp, c, j, a, b) - kp.dt * kap * m;
+            if (endc) rhs -= kp.dt_endx * kap * m;
+            acc = fma(stage * dt_c[c], rhs, base[idx]);
+        } else {
+            acc = base[idx] - kp.dt_ds * div_s - kp.dt_dxi * (Fxh - Fxl) - kp.dt_deta * (Feh - Fel);
+            acc += source_increment(kp, c, j, a, b) - kp.dt * kap * m;
+            if (endc) acc -= kp.dt_endx * kap * m;
+        }
         out[idx] = kp.inside[rem] ? acc : real(0);
     }
 }

@@ -75,11 +75,13 @@ def test_local_errors():
     with pytest.raises(MMError):
         mm.local_steps(np.empty(g.nc, np.int32), None)
     mm.destroy()
-    mm = MM(g, Params(flags=mi.FLAG_RK2_SUPERBEE), "f64")
+    import torch
+    one = torch.zeros(g.cells, dtype=torch.float64, device="cuda:0")
+    mm = MM(g, Params(flags=mi.FLAG_RK2_SUPERBEE), "f64", buf0=one)      # single-buffer context
     U, V, Om, m0 = random_inputs(g, Params(), "f64")
     mm.set_density(m0); mm.set_filament_velocity(U, V, Om)
     with pytest.raises(MMError):
-        mm.advance_local(0.1, 0.4)            # RK2 not supported on this call yet
+        mm.advance_local(0.1, 0.4)            # local RK2 steps need the second density buffer
     with pytest.raises(MMError):
         MM(g, Params(), "f64").advance_local(-1.0, 0.4)
     mm.destroy()
@@ -153,3 +155,43 @@ def test_local_steps_with_the_coupled_source(dtype, nxi):
         assert p1_density(out, ref) <= TOL[dtype], name
         ef, et = p2_moments(f, t, orc.moments(g, p, ref))
         assert ef <= TOL[dtype] and et <= TOL[dtype], name
+
+
+# ------------------------------------------------------------------ local steps of the paper's own scheme (NEXT-3 x NEXT-1)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", [(2, 2, 4, 6, 5, 4), (2, 3, 6, 9, 16, 16)])
+def test_local_rk2_parity(dtype, shape):
+    """Alg. 2 l.5 (dt_c from the CFL bound) driving l.9-10 (RK2 + Superbee): every unit takes its own n_c two-stage steps."""
+    g = Grid(*shape)
+    p = Params(flags=mi.FLAG_RK2_SUPERBEE)
+    n, name = check_local(g, p, dtype, 5.3, omega_max=2.0)
+    assert name.startswith("rk2_local_generic<") and len(set(n.tolist())) > 1
+
+
+def test_local_rk2_with_the_coupled_source():
+    import dataclasses
+    from paper_1908_04279_b200 import MM
+    g = Grid(4, 5, 6, 7, 8, 8)
+    big = Params(m_free=1e9, flags=mi.FLAG_RK2_SUPERBEE)
+    U, V, Om, m0 = random_inputs(g, big, "f64", omega_max=2.0)
+    psi = np.random.default_rng(6).random(g.nc) * 30.0
+    _, raw, _ = orc.free_motors(g, big, m0, psi)
+    p = dataclasses.replace(big, m_free=float(np.median(raw)))
+    dt = 4.5 / orc.rate_bound(g, p, U, V, Om).mean()
+    mm = MM(g, p, "f64")
+    mm.set_density(m0); mm.set_filament_velocity(U, V, Om); mm.set_psi(psi)
+    mm.update_free_motors(None, None)
+    mm.advance_local(dt, 0.4)
+    n = np.empty(g.nc, np.int32)
+    mm.local_steps(n, None)
+    f, t = np.empty((g.nc, 2)), np.empty(g.nc)
+    mm.moments(f, t)
+    out = np.empty_like(m0)
+    mm.get_density(out)
+    mm.destroy()
+    capped, _, Mf_ref = orc.free_motors(g, p, m0, psi)
+    ref, n_ref = orc.advance_local(g, p, U, V, Om, capped, dt, 0.4, Mf=Mf_ref)
+    assert np.array_equal(n, n_ref) and len(set(n.tolist())) > 1
+    assert p1_density(out, ref) <= TOL["f64"]
+    ef, et = p2_moments(f, t, orc.moments(g, p, ref))
+    assert ef <= TOL["f64"] and et <= TOL["f64"]

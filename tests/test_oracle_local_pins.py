@@ -106,6 +106,12 @@ def test_l4_units_are_independent():
     perm[[1, 1 + g.ntheta]] = perm[[1 + g.ntheta, 1]]
     out2, n2 = orc.advance_local(g, p, U[perm], V[perm], Om[perm], m[perm], dt, 0.4)
     assert np.array_equal(n2, n[perm]) and np.array_equal(out2, out[perm])
+    # ... and each is bitwise its own run of n_c RK2 + Superbee substeps of dt / n_c (ties the local RK2 call to `run`
+    # with the flag, which pins R1-R7 fix)
+    assert len(set(n.tolist())) > 1
+    for c in (0, 3, g.nc - 1):
+        ref = orc.run(g, p, U[c:c + 1], V[c:c + 1], Om[c:c + 1], m[c:c + 1], int(n[c]), dt / n[c], c_first=c)
+        assert np.array_equal(ref[0], out[c])
 
 
 def test_l5_local_steps_with_the_coupled_source():
