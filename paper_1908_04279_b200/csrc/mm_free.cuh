@@ -133,6 +133,19 @@ __device__ __forceinline__ void fx_deposit(uint32_t *L0, uint32_t *L1, uint32_t 
     if (x2 | c1) atomicAdd(&L2[n], x2 + c1);
 }
 
+// old = L[addr]; L[addr] += x -- skipped (old = 0) when x == 0; a predicated ATOMS, no branch around it
+__device__ __forceinline__ uint32_t atoms_add_nz(uint32_t saddr, uint32_t x)
+{
+    uint32_t o;
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\tmov.u32 %0, 0;\n\t@p atom.shared.add.u32 %0, [%1], %2;\n\t}"
+                 : "=r"(o) : "r"(saddr), "r"(x) : "memory");
+    return o;
+}
+__device__ __forceinline__ void reds_add_nz(uint32_t saddr, uint32_t x)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %1, 0;\n\t@p red.shared.add.u32 [%0], %1;\n\t}" :: "r"(saddr), "r"(x) : "memory");
+}
+
 // The same two passes for the BASELINE offset planes (16x16, 8x8; a plane tiles a warp with VW cells of one row per
 // 64/128-bit access, NV accesses per lane): PL planes are in flight per lane before any is consumed -- one 4-byte load
 // per lane and plane, as in the kernel above, leaves the pass bound by load latency -- the node of a cell is two table
@@ -175,6 +188,7 @@ __global__ void __launch_bounds__(PRIV ? 512 : 256) free_cells_vec_kernel(const 
         const double nd = lane < 16 ? (double)q.nx : (double)q.ny;
         const double wp = MODE == 0 ? w * psi[c] : 0.0;
         if (MODE == 0 && wp == 0.0) continue;
+        const double wps = wp * inv_unit * 4294967296.0;   // powers of two: wps * m rounds as wp * m
         real *mc = dens + c * inner + lane * VW;
         for (int j0 = 0; j0 < q.ns; j0 += PL) {
             Vec v[PL][NV];
@@ -195,6 +209,67 @@ __global__ void __launch_bounds__(PRIV ? 512 : 256) free_cells_vec_kernel(const 
                 int nb[VW];
 #pragma unroll
                 for (int e = 0; e < VW; ++e) nb[e] = __shfl_sync(0xffffffffu, my_node, 16 + b0 + e);
+                if (MODE == 0 && PRIV) {
+                    // the NV * VW deposits of this lane's cells as three rounds of independent, unconditional atomics
+                    // (limb 0 of every cell, then limb 1 with the carries, then -- rarely -- limb 2): one chain of
+                    // returning ATOMS at a time leaves the pass bound by their latency, a branch around each by issue.
+                    // The limbs come from two round-down additions of 1.5 * 2^52 (floor of |t| < 2^51 in the low mantissa
+                    // bits) instead of three 64-bit conversions; a deposit outside that range takes fx_deposit.
+                    constexpr int NB = NV * VW;
+                    constexpr double MG = 6755399441055744.0;   // 1.5 * 2^52, bits 0x43380000'00000000
+                    uint32_t n[NB];   // byte address of the node's limb 0 in shared memory
+                    uint32_t x0[NB], x1[NB], x2[NB], bad = 0u;
+                    const uint32_t sL0 = (uint32_t)__cvta_generic_to_shared(L0), limb = (uint32_t)nnp * 4u;
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) {
+                        const int na = __shfl_sync(0xffffffffu, my_node, k * RPV + arow);
+#pragma unroll
+                        for (int e = 0; e < VW; ++e) {
+                            const int i = k * VW + e;
+                            n[i] = sL0 + (uint32_t)(na + nb[e]) * 4u;
+                            const double t = __dmul_rn(wps, (double)v[pl][k].v[e]);   // (w psi m / unit) 2^32, rounded as w psi m
+                            const double tm = __dadd_rd(t, MG);
+                            const double r = t - (tm - MG);                              // exact, in [0, 1)
+                            x0[i] = (uint32_t)__double2loint(__fma_rd(r, 4294967296.0, MG));
+                            x1[i] = (uint32_t)__double2loint(tm);
+                            const uint32_t hi = (uint32_t)__double2hiint(tm);
+                            x2[i] = hi - 0x43380000u;
+                            bad |= (hi ^ 0x43300000u) & 0xfff00000u;
+                        }
+                    }
+                    if (bad) {   // |t| >= 2^51 (a single deposit of 2^19 units or more) or not finite
+#pragma unroll
+                        for (int k = 0; k < NV; ++k)
+#pragma unroll
+                            for (int e = 0; e < VW; ++e) {
+                                const double val = (double)v[pl][k].v[e];
+                                if (val != 0.0) fx_deposit(L0, L1, L2, (int)((n[k * VW + e] - sL0) >> 2), __dmul_rn(wp, val) * inv_unit);
+                            }
+                        continue;
+                    }
+                    uint32_t any2 = 0u;
+#pragma unroll
+                    for (int i = 0; i < NB; ++i) {
+                        uint32_t o;
+                        asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(o) : "r"(n[i]), "r"(x0[i]) : "memory");
+                        // x1 += carry of limb 0; x0 = carry out of that
+                        asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %2, %3;\n\taddc.cc.u32 %0, %0, 0;\n\taddc.u32 %1, 0, 0;\n\t}"
+                            : "+r"(x1[i]), "=r"(x0[i]) : "r"(o), "r"(x0[i]));
+                    }
+#pragma unroll
+                    for (int i = 0; i < NB; ++i) {
+                        uint32_t o;
+                        asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(o) : "r"(n[i] + limb), "r"(x1[i]) : "memory");
+                        asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %3;\n\t}"
+                            : "+r"(x2[i]) : "r"(o), "r"(x1[i]), "r"(x0[i]));
+                        any2 |= x2[i];
+                    }
+                    if (any2) {
+#pragma unroll
+                        for (int i = 0; i < NB; ++i) reds_add_nz(n[i] + 2u * limb, x2[i]);
+                    }
+                    continue;
+                }
 #pragma unroll
                 for (int k = 0; k < NV; ++k) {
                     const int na = __shfl_sync(0xffffffffu, my_node, k * RPV + arow);

@@ -62,6 +62,29 @@ def test_free_motor_coupling_parity(dtype, flags, shape, kernel):
     assert name.startswith(fam[kernel] if fast else ("rk2_generic<" if flags else "generic<")), name
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_free_motor_deposits_of_every_magnitude(dtype):
+    """The fixed-point deposit of the vectorised pass has two routes: |deposit| < 2^19 units of the table (the limbs come
+    from round-down additions) and the rest (conversions, `fx_deposit`).  A density whose cells span 7 decades, with
+    M_total chosen so that the largest node sum is 2^29 units, sends cells down both."""
+    g = Grid(6, 6, 8, 7, 16, 16)
+    big = Params(m_free=1e30)
+    U, V, Om, m0 = random_inputs(g, big, dtype)
+    rng = np.random.default_rng(31)
+    m0 = np.ascontiguousarray(m0 * np.where(rng.random(m0.shape) < 0.003, 1e7, 1.0), NPDT[dtype])
+    psi = rng.random(g.nc) * 30.0
+    _, raw, _ = orc.free_motors(g, big, m0, psi)
+    p = dataclasses.replace(big, m_free=float(raw.max()) / 2.0 ** 29)
+    Mbc, Mf, capped, _, _ = gpu_coupled(g, p, dtype, U, V, Om, m0, psi, 0, 1e-3)
+    m_ref, Mbc_ref, Mf_ref = orc.free_motors(g, p, m0, psi)
+    tol = TOL[dtype]
+    assert np.max(np.abs(Mbc - Mbc_ref)) / p.m_free <= tol and np.max(np.abs(Mf - Mf_ref)) / p.m_free <= tol
+    assert p1_density(capped, m_ref) <= tol
+    # the cap factor of a node is M_total / (its raw sum): the rescaled cells carry the sums to rounding
+    nz = np.abs(m_ref) > 0
+    assert np.max(np.abs(capped[nz] / m_ref[nz] - 1.0)) <= (1e-11 if dtype == "f64" else 3e-7)
+
+
 def test_free_motor_option_and_errors():
     from paper_1908_04279_b200 import MM, MMError, binding as b
     g = Grid(4, 4, 4, 6, 8, 8)
