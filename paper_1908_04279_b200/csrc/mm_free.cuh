@@ -133,6 +133,12 @@ __device__ __forceinline__ void fx_deposit(uint32_t *L0, uint32_t *L1, uint32_t 
     if (x2 | c1) atomicAdd(&L2[n], x2 + c1);
 }
 
+// the same out of line: the rare route of the vector kernel (a deposit of 2^19 units or more)
+__device__ __noinline__ void fx_deposit_rare(uint32_t *L0, uint32_t *L1, uint32_t *L2, int n, double q)
+{
+    fx_deposit(L0, L1, L2, n, q);
+}
+
 // old = L[addr]; L[addr] += x -- skipped (old = 0) when x == 0; a predicated ATOMS, no branch around it
 __device__ __forceinline__ uint32_t atoms_add_nz(uint32_t saddr, uint32_t x)
 {
@@ -150,8 +156,11 @@ __device__ __forceinline__ void reds_add_nz(uint32_t saddr, uint32_t x)
 // 64/128-bit access, NV accesses per lane): PL planes are in flight per lane before any is consumed -- one 4-byte load
 // per lane and plane, as in the kernel above, leaves the pass bound by load latency -- the node of a cell is two table
 // look-ups by shuffle (the index separates), and with PRIV the deposits go to the CTA's fixed-point table.
+#ifndef MM_FREE_PRIV_THREADS_F32
+#define MM_FREE_PRIV_THREADS_F32 512   // 768 threads (80 registers): spills in the deposit rounds, 11.4 -> 19.3 ms on configs[4]
+#endif
 template <typename real, int MODE, bool PRIV, int NXI, int NETA, int PL>
-__global__ void __launch_bounds__(PRIV ? 512 : 256) free_cells_vec_kernel(const FreeGeom q, int64_t nc, real *__restrict__ dens,
+__global__ void __launch_bounds__(PRIV ? (sizeof(real) == 4 ? MM_FREE_PRIV_THREADS_F32 : 512) : 256) free_cells_vec_kernel(const FreeGeom q, int64_t nc, real *__restrict__ dens,
                                                                           const double *__restrict__ psi, double w,
                                                                           double *__restrict__ raw, const double *__restrict__ factor,
                                                                           const int *__restrict__ any_capped,
@@ -243,7 +252,7 @@ __global__ void __launch_bounds__(PRIV ? 512 : 256) free_cells_vec_kernel(const 
 #pragma unroll
                             for (int e = 0; e < VW; ++e) {
                                 const double val = (double)v[pl][k].v[e];
-                                if (val != 0.0) fx_deposit(L0, L1, L2, (int)((n[k * VW + e] - sL0) >> 2), __dmul_rn(wp, val) * inv_unit);
+                                if (val != 0.0) fx_deposit_rare(L0, L1, L2, (int)((n[k * VW + e] - sL0) >> 2), __dmul_rn(wp, val) * inv_unit);
                             }
                         continue;
                     }
