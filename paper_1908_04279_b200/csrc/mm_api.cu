@@ -130,6 +130,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->loc_lambda = nullptr; c->loc_n = c->loc_nmax = c->loc_list = c->loc_count = nullptr; c->loc_dt = nullptr;
     c->loc_valid = false;
     c->psi = c->fline = c->F2 = nullptr; c->psi_set = false;
+    c->Mf_f32 = nullptr;
     c->Mf = c->Mbc = c->free_raw = c->free_factor = nullptr; c->free_fx = nullptr; c->free_any = nullptr; c->coupled = false;
     c->mom_valid = c->vel_set = false; c->tile_ok = false; c->fline_valid = false;
     c->dens_cov_count = 0;
@@ -197,7 +198,7 @@ extern "C" mm_status mm_destroy(mm_ctx *c)
     cudaFree(c->loc_lambda); cudaFree(c->loc_n); cudaFree(c->loc_nmax); cudaFree(c->loc_dt);
     cudaFree(c->loc_list); cudaFree(c->loc_count);
     cudaFree(c->psi); cudaFree(c->fline); cudaFree(c->F2);
-    cudaFree(c->Mf); cudaFree(c->Mbc); cudaFree(c->free_raw); cudaFree(c->free_factor); cudaFree(c->free_fx); cudaFree(c->free_any);
+    cudaFree(c->Mf_f32); cudaFree(c->Mf); cudaFree(c->Mbc); cudaFree(c->free_raw); cudaFree(c->free_factor); cudaFree(c->free_fx); cudaFree(c->free_any);
     delete c;
     return MM_OK;
 }
@@ -611,7 +612,7 @@ static mm_status free_impl(mm_ctx *c)
         kern0<<<(unsigned)pb, threads, smem, c->stream>>>(q, c->nc, dens, c->psi, w, c->free_raw, nullptr, nullptr, c->free_fx, 1.0 / unit);
         CUDA_TRY(c, cudaGetLastError());
         free_cap_kernel<<<(nn + 255) / 256, 256, 0, c->stream>>>(nn, p.m_free, c->free_raw, c->free_factor, c->Mbc, c->Mf, c->free_any,
-                                                                  fx ? c->free_fx : nullptr, unit);
+                                                                  fx ? c->free_fx : nullptr, unit, c->Mf_f32);
         CUDA_TRY(c, cudaGetLastError());
         kern1<<<(unsigned)blocks, 256, 0, c->stream>>>(q, c->nc, dens, nullptr, 0.0, nullptr, c->free_factor, c->free_any, nullptr, 1.0);
         CUDA_TRY(c, cudaGetLastError());
@@ -641,16 +642,17 @@ extern "C" mm_status mm_update_free_motors(mm_ctx *c, double *Mb_coarse, double 
     if (c->dens_cov_count != c->nc || !c->psi_set) return fail(c, MM_ERR_STATE, "set density and psi first");
     const size_t nn = (size_t)c->g.nx * c->g.ny;
     if (!c->free_any) {   // allocated as a group, committed together
-        void *g[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-        const size_t bytes[6] = {nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * 16, sizeof(int)};
-        for (int i = 0; i < 6; ++i)
+        void *g[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+        const size_t bytes[7] = {nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * 16,
+                                 nn * sizeof(float), sizeof(int)};
+        for (int i = 0; i < 7; ++i)
             if (cudaMalloc(&g[i], bytes[i]) != cudaSuccess) {
                 cudaGetLastError();
                 for (int k = 0; k < i; ++k) cudaFree(g[k]);
                 return fail(c, MM_ERR_NOMEM, "device allocation failed (free-motor tables)");
             }
         c->Mf = (double *)g[0]; c->Mbc = (double *)g[1]; c->free_raw = (double *)g[2]; c->free_factor = (double *)g[3];
-        c->free_fx = (unsigned long long *)g[4]; c->free_any = (int *)g[5];
+        c->free_fx = (unsigned long long *)g[4]; c->Mf_f32 = (float *)g[5]; c->free_any = (int *)g[6];
     }
     mm_status s = c->dtype == MM_F64 ? free_impl<double>(c) : free_impl<float>(c);
     if (s != MM_OK) return s;

@@ -342,7 +342,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 for (int q = 0; q < QA; ++q)
 #pragma unroll
                     for (int cb = 0; cb < CB; ++cb) {
-                        const real sv = kp.dt_kon * (real)kp.Mf[nodx[q] + nody[cb]];
+                        const real sv = kp.dt_kon * __ldg(&kp.Mf_r[nodx[q] + nody[cb]]);
                         srcm[q][cb] = PM ? sv : maskf[q][cb] * sv;
                     }
             }

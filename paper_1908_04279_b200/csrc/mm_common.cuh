@@ -29,6 +29,8 @@ struct KParams {
     const real *kappa;                 // [nxi*neta], k_off0 * exp(k r_ab / f_d) evaluated in fp64 (S6)
     const uint8_t *inside;             // [nxi*neta], 1 inside the capture disc (S1)
     const double *Mf;                  // NULL, or the free-motor table [nx][ny] (NEXT-2); generic kernels only
+    const real *Mf_r;                  // the same table rounded to `real` (fp64 contexts: the table itself): what the
+                                       // coefficient-form kernels gather -- no conversion per cell, half the bytes in L1
     int32_t nx, ny;
     double geo_R, geo_dxi, geo_deta, geo_ds, geo_s_lo;   // fp64 geometry for the anchor map (never rounded to fp32)
 };

@@ -319,7 +319,8 @@ __global__ void __launch_bounds__(PRIV ? (sizeof(real) == 4 ? MM_FREE_PRIV_THREA
 // raw_fx != NULL: the sums arrive as 128-bit fixed point in units of `unit` (see fx_deposit)
 __global__ void free_cap_kernel(int nn, double m_total, const double *__restrict__ raw, double *__restrict__ factor,
                                 double *__restrict__ Mbc, double *__restrict__ Mf, int *__restrict__ any_capped,
-                                const unsigned long long *__restrict__ raw_fx = nullptr, double unit = 1.0)
+                                const unsigned long long *__restrict__ raw_fx = nullptr, double unit = 1.0,
+                                float *__restrict__ Mf_f32 = nullptr)
 {
     for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < nn; n += gridDim.x * blockDim.x) {
         const double r = raw_fx ? ((double)(long long)raw_fx[2 * n + 1] + (double)raw_fx[2 * n] * 5.421010862427522e-20) * unit : raw[n];
@@ -328,6 +329,7 @@ __global__ void free_cap_kernel(int nn, double m_total, const double *__restrict
         const double capped = over ? m_total : r;
         Mbc[n] = capped;
         Mf[n] = m_total - capped;
+        if (Mf_f32) Mf_f32[n] = (float)(m_total - capped);
         if (over) *any_capped = 1;
     }
 }

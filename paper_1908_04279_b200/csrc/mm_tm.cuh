@@ -203,18 +203,34 @@ __device__ __forceinline__ void tm_level(const TmCoef<real, QA, CB> &k, const re
 // All `nlev` levels of one plane, in place in x.  The loop is rolled by two: the plane values alternate between x and
 // y, so no register copies are needed (an odd count ends with one copy per plane).  Rolled by four it runs at less than
 // half the speed: 9 variants x 7 level bodies no longer fit the instruction cache (profiles/r02a_README.md).
-template <int SK, typename real, int QA, int CB, int LB, int CPL>
+// COMPACT (the coupled-source kernels, whose per-plane code is longer): an odd count leaves the loop after its first
+// half instead of running a third copy of the level body -- 7 KB less hot code, which keeps the plane loop under the
+// instruction-cache cliff; the plain kernels lose 2 % to the extra branch per pair of levels and keep the tail copy.
+template <int SK, bool COMPACT, typename real, int QA, int CB, int LB, int CPL>
 __device__ __forceinline__ void tm_plane(const TmCoef<real, QA, CB> &k, real (&x)[QA][CB], uint32_t tbase, int nlev)
 {
     real y[QA][CB];
-    int lv = 0;
+    bool odd = false;
+    if constexpr (COMPACT) {
 #pragma unroll 1
-    for (; lv + 2 <= nlev; lv += 2) {
-        tm_level<SK, real, QA, CB, LB>(k, x, y, tbase + lv * CPL);
-        tm_level<SK, real, QA, CB, LB>(k, y, x, tbase + lv * CPL + CPL);
+        for (int lv = 0; lv < nlev; lv += 2) {
+            tm_level<SK, real, QA, CB, LB>(k, x, y, tbase + lv * CPL);
+            if (lv + 1 == nlev) { odd = true; break; }
+            tm_level<SK, real, QA, CB, LB>(k, y, x, tbase + lv * CPL + CPL);
+        }
+    } else {
+        int lv = 0;
+#pragma unroll 1
+        for (; lv + 2 <= nlev; lv += 2) {
+            tm_level<SK, real, QA, CB, LB>(k, x, y, tbase + lv * CPL);
+            tm_level<SK, real, QA, CB, LB>(k, y, x, tbase + lv * CPL + CPL);
+        }
+        if (lv < nlev) {
+            tm_level<SK, real, QA, CB, LB>(k, x, y, tbase + lv * CPL);
+            odd = true;
+        }
     }
-    if (lv < nlev) {
-        tm_level<SK, real, QA, CB, LB>(k, x, y, tbase + lv * CPL);
+    if (odd) {
 #pragma unroll
         for (int q = 0; q < QA; ++q)
 #pragma unroll
@@ -308,6 +324,21 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     bool last_pass = true;
     real FX = 0, FY = 0, TQ = 0;
 
+    // MF: co.src of s-plane jj = mask dt k_on M_f(node of the cell's anchor), through this warp's node tables
+    auto gather = [&](int jj) {
+        const unsigned short *nj = nod + jj * (NXI + NETA);
+        int nodx[QA], nody[CB];
+#pragma unroll
+        for (int q = 0; q < QA; ++q) nodx[q] = (int)nj[a0 + q] * kp.ny;
+#pragma unroll
+        for (int cb = 0; cb < CB; ++cb) nody[cb] = (int)nj[NXI + b0 + cb];
+#pragma unroll
+        for (int q = 0; q < QA; ++q)
+#pragma unroll
+            for (int cb = 0; cb < CB; ++cb)
+                co.src[q][cb] = maskf[q][cb] * (kp.dt_kon * dtc * __ldg(&kp.Mf_r[nodx[q] + nody[cb]]));
+    };
+
     int64_t k = 0, c = 0;
     int ch = 0, slot = 0;
     uint32_t phase = 0;
@@ -385,8 +416,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             }
             tm_wait_st();   // the previous configuration's last carries have landed
             tm_st<NKP>(tm_k, kc);
-            if (!MF) {
-                // zero inflow at s_lo (S5): the carry into plane 0 is the source alone, at every level
+            {
+                // zero inflow at s_lo (S5): the carry into plane 0 is the source alone (MF: its own, gathered), at every level
+                if constexpr (MF) gather(0);
                 real p0[QA * CB];
 #pragma unroll
                 for (int q = 0; q < QA; ++q)
@@ -405,33 +437,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             const int j = ch * P + pl;
             if (j >= ns) break;   // ragged last chunk
             const real sj = kp.s_lo + (real(j) + real(0.5)) * kp.ds;
-            if constexpr (MF) {
-                // the carry a plane sends downstream holds the source of the RECEIVING cell: while plane j is worked on,
-                // co.src is the (gathered) source of plane j+1; plane 0 receives its own source as the zero-inflow carry
-                auto gather = [&](int jj) {
-                    const unsigned short *nj = nod + jj * (NXI + NETA);
-                    int nodx[QA], nody[CB];
-#pragma unroll
-                    for (int q = 0; q < QA; ++q) nodx[q] = (int)nj[a0 + q] * kp.ny;
-#pragma unroll
-                    for (int cb = 0; cb < CB; ++cb) nody[cb] = (int)nj[NXI + b0 + cb];
-#pragma unroll
-                    for (int q = 0; q < QA; ++q)
-#pragma unroll
-                        for (int cb = 0; cb < CB; ++cb)
-                            co.src[q][cb] = maskf[q][cb] * (kp.dt_kon * dtc * (real)kp.Mf[nodx[q] + nody[cb]]);
-                };
-                if (j == 0) {
-                    gather(0);
-                    real p0[QA * CB];
-#pragma unroll
-                    for (int q = 0; q < QA; ++q)
-#pragma unroll
-                        for (int cb = 0; cb < CB; ++cb) p0[q * CB + cb] = co.src[q][cb];
-                    for (int lv = 0; lv < nlev; ++lv) tm_st<QA * CB>(tm_p + lv * CPL, p0);
-                }
-                gather(j + 1 < ns ? j + 1 : j);
-            }
+            // MF: the carry a plane sends downstream holds the source of the RECEIVING cell: while plane j is worked on,
+            // co.src is the (gathered) source of plane j+1 (plane 0 received its own with the zero-inflow carry above)
+            if constexpr (MF) gather(j + 1 < ns ? j + 1 : j);
             // ---- level-independent coefficients of this plane
             uint32_t zxm = 0, zxp = 0, zem = 0, zep = 0;   // OR of the bit patterns: 0 <=> the whole set is +0
             {
@@ -495,7 +503,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             {
                 const int vx = __all_sync(0xffffffffu, zxm == 0) ? 1 : (__all_sync(0xffffffffu, zxp == 0) ? 2 : 0);
                 const int ve = __all_sync(0xffffffffu, zem == 0) ? 1 : (__all_sync(0xffffffffu, zep == 0) ? 2 : 0);
-#define MM_TM_VARIANT(SK_) tm_plane<SK_, real, QA, CB, LB, CPL>(co, x, tm_p, nlev)
+#define MM_TM_VARIANT(SK_) tm_plane<SK_, MF, real, QA, CB, LB, CPL>(co, x, tm_p, nlev)
                 switch (vx * 3 + ve) {
                 case 0: MM_TM_VARIANT(0); break;
                 case 1: MM_TM_VARIANT(4); break;
