@@ -619,7 +619,7 @@ static mm_status free_impl(mm_ctx *c)
         return MM_OK;
     };
     mm_status rs;
-#define MM_FREE_VEC(N_) (priv ? run(free_cells_vec_kernel<real, 0, true, N_, N_, 4>, free_cells_vec_kernel<real, 1, false, N_, N_, 4>, sizeof(real) == 4 ? MM_FREE_PRIV_THREADS_F32 : 512, tab_bytes) \
+#define MM_FREE_VEC(N_) (priv ? run(free_cells_vec_kernel<real, 0, true, N_, N_, MM_FREE_PRIV_PL>, free_cells_vec_kernel<real, 1, false, N_, N_, 4>, sizeof(real) == 4 ? MM_FREE_PRIV_THREADS_F32 : 512, tab_bytes) \
                              : run(free_cells_vec_kernel<real, 0, false, N_, N_, 4>, free_cells_vec_kernel<real, 1, false, N_, N_, 4>, 256, 0))
     if (vw && g.nxi == 16) rs = MM_FREE_VEC(16);
     else if (vw) rs = MM_FREE_VEC(8);

@@ -156,8 +156,11 @@ __device__ __forceinline__ void reds_add_nz(uint32_t saddr, uint32_t x)
 // 64/128-bit access, NV accesses per lane): PL planes are in flight per lane before any is consumed -- one 4-byte load
 // per lane and plane, as in the kernel above, leaves the pass bound by load latency -- the node of a cell is two table
 // look-ups by shuffle (the index separates), and with PRIV the deposits go to the CTA's fixed-point table.
+#ifndef MM_FREE_PRIV_PL
+#define MM_FREE_PRIV_PL 4   // planes in flight per lane
+#endif
 #ifndef MM_FREE_PRIV_THREADS_F32
-#define MM_FREE_PRIV_THREADS_F32 512   // 768 threads (80 registers): spills in the deposit rounds, 11.4 -> 19.3 ms on configs[4]
+#define MM_FREE_PRIV_THREADS_F32 512   // 640 threads (96 registers): 12.8 ms on configs[4] instead of 11.2; 768 (80, spills): 19.3
 #endif
 template <typename real, int MODE, bool PRIV, int NXI, int NETA, int PL>
 __global__ void __launch_bounds__(PRIV ? (sizeof(real) == 4 ? MM_FREE_PRIV_THREADS_F32 : 512) : 256) free_cells_vec_kernel(const FreeGeom q, int64_t nc, real *__restrict__ dens,
@@ -243,10 +246,10 @@ __global__ void __launch_bounds__(PRIV ? (sizeof(real) == 4 ? MM_FREE_PRIV_THREA
                             x1[i] = (uint32_t)__double2loint(tm);
                             const uint32_t hi = (uint32_t)__double2hiint(tm);
                             x2[i] = hi - 0x43380000u;
-                            bad |= (hi ^ 0x43300000u) & 0xfff00000u;
+                            bad |= hi ^ 0x43300000u;   // exponent field 0x433 <=> tm in [2^52, 2^53)
                         }
                     }
-                    if (bad) {   // |t| >= 2^51 (a single deposit of 2^19 units or more) or not finite
+                    if (bad >> 20) {   // |t| >= 2^51 (a single deposit of 2^19 units or more) or not finite
 #pragma unroll
                         for (int k = 0; k < NV; ++k)
 #pragma unroll
