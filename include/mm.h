@@ -195,6 +195,27 @@ mm_status mm_spread_force(mm_ctx *ctx, double *F2, int dst_on_device);
  * Mb_coarse, M_free: [nx][ny] fp64 outputs, either may be NULL.  Needs mm_set_psi. */
 mm_status mm_update_free_motors(mm_ctx *ctx, double *Mb_coarse, double *M_free, int dst_on_device);
 
+/* The same update (Eq. 5-6; Alg. 2 l.14-20; readings Q38-Q42) WITHOUT a context and
+ * without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it): no cudaMalloc / cudaFree / allocating library routine is called, now or at first use.  The
+ * node tables the three kernels pass between them live in ONE file-scope device array of MM_NOALLOC_MAX_NODES * 32 +
+ * 256 bytes (512.25 KB), which every GPU that loads the library holds until exit.
+ *   grid, params : as for mm_create (only the geometry and m_free = M_total are used); HOST pointers.
+ *   density      : DEVICE pointer, canonical layout [ix][iy][itheta][j][a][b], `dtype` elements; IN/OUT -- cells of a node
+ *                  above the cap are rescaled in place, as mm_update_free_motors does with the context's density.
+ *   psi          : DEVICE pointer, [nc] fp64 (the filament density Psi per configuration).
+ *   Mb_coarse, M_free : DEVICE pointers, [nx][ny] fp64 OUTPUTS, both required.
+ *   cuda_stream  : all work is enqueued on it; the call does not synchronise.  The device the stream belongs to must be
+ *                  current.
+ * Same kernels and kernel choice as mm_update_free_motors; where both take the fixed-point route the results are
+ * bitwise equal.  MM_ERR_INVALID_ARG (message via mm_last_error(NULL)) when nx * ny > MM_NOALLOC_MAX_NODES, a pointer is
+ * NULL or the geometry is invalid.  Every call on a device shares the array, which keeps the last call's contents (each
+ * call clears what must start at zero): calls that overlap on the GPU -- two streams with no ordering between them --
+ * RACE; order them (same stream, or events).  It does not touch any mm_ctx. */
+#define MM_NOALLOC_MAX_NODES 16384   /* nx * ny, e.g. 128 x 128 (BASELINE configs[4]) */
+mm_status mm_free_motors_noalloc(const mm_grid *grid, const mm_params *params, mm_dtype dtype, void *density,
+                                 const double *psi, double *Mb_coarse, double *M_free, void *cuda_stream);
+
 /* Moments (S9) of the current density: force [Nc][2] = (Fx, Fy), torque [Nc]; always fp64
  * (macroscale data stays double precision).  Either pointer may be NULL to skip it. */
 mm_status mm_moments(mm_ctx *ctx, double *force, double *torque, int dst_on_device);

@@ -20,7 +20,8 @@ MM_LOCAL_FUSE_T = 4
 EXPORTS = ["mm_create", "mm_set_density", "mm_get_density", "mm_set_density_range", "mm_get_density_range",
            "mm_set_filament_velocity", "mm_substep", "mm_moments", "mm_set_option", "mm_get_option", "mm_launch_count",
            "mm_kernel_name", "mm_destroy", "mm_status_string", "mm_last_error", "mm_advance_local", "mm_local_steps", "mm_set_psi",
-           "mm_spread_force", "mm_update_free_motors", "mm_measure_fma_peak"]
+           "mm_spread_force", "mm_update_free_motors", "mm_measure_fma_peak", "mm_free_motors_noalloc"]
+MM_NOALLOC_MAX_NODES = 16384
 
 
 class mm_grid(ctypes.Structure):
@@ -65,6 +66,7 @@ def lib():
         L.mm_set_psi.argtypes = [vp, vp, ctypes.c_int]
         L.mm_spread_force.argtypes = [vp, vp, ctypes.c_int]
         L.mm_update_free_motors.argtypes = [vp, vp, vp, ctypes.c_int]
+        L.mm_free_motors_noalloc.argtypes = [ctypes.POINTER(mm_grid), ctypes.POINTER(mm_params), ctypes.c_int, vp, vp, vp, vp, vp]
         L.mm_set_option.argtypes = [vp, ctypes.c_int, i64]
         L.mm_get_option.argtypes = [vp, ctypes.c_int, ctypes.POINTER(i64)]
         L.mm_launch_count.argtypes = [vp]
@@ -135,6 +137,27 @@ def measure_fma_peak(dtype: str, stream: int | None = None) -> float:
     if st != MM_OK:
         raise MMError(st, L.mm_status_string(st).decode(), L.mm_last_error(None).decode())
     return float(out.value)
+
+
+def free_motors_noalloc(grid, params, dtype: str, density, psi, Mb_coarse, M_free, stream: int | None = None):
+    """mm_free_motors_noalloc: the free-motor update without a context and without any allocation (fixed device
+    scratch, nx * ny <= MM_NOALLOC_MAX_NODES).  Every array is a DEVICE tensor; `density` is rescaled in place where a
+    node is capped; Mb_coarse and M_free are outputs.  Calls that overlap on the GPU race (one shared scratch array)."""
+    L = lib()
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    nn, nc = grid.nx * grid.ny, grid.nx * grid.ny * grid.ntheta
+    args = (_ptr(density, dtype, nc * grid.ns * grid.nxi * grid.neta, "density"), _ptr(psi, "f64", nc, "psi"),
+            _ptr(Mb_coarse, "f64", nn, "Mb_coarse"), _ptr(M_free, "f64", nn, "M_free"))
+    if any(p is None or not dev for p, dev in args):
+        raise ValueError("free_motors_noalloc: density, psi, Mb_coarse and M_free must all be device tensors")
+    g, p = _grid_struct(grid), _params_struct(params)
+    st = L.mm_free_motors_noalloc(ctypes.byref(g), ctypes.byref(p), MM_F64 if dtype == "f64" else MM_F32, args[0][0],
+                                  args[1][0], args[2][0], args[3][0], ctypes.c_void_p(stream))
+    if st != MM_OK:
+        raise MMError(st, L.mm_status_string(st).decode(), L.mm_last_error(None).decode())
+    return Mb_coarse, M_free
 
 
 class MM:

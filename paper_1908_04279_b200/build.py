@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libmm.so")
 MM_H = os.path.join(os.path.dirname(HERE), "include", "mm.h")
-UNITS = ("mm_api", "mm_launch_tm", "mm_launch_coef", "mm_launch_stream_tile", "mm_launch_rk2")
+UNITS = ("mm_api", "mm_launch_tm", "mm_launch_coef", "mm_launch_stream_tile", "mm_launch_rk2", "mm_noalloc")
 SOURCES = [os.path.join(CSRC, u + ".cu") for u in UNITS]
 CFLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 LFLAGS = ["-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a",
