@@ -104,6 +104,10 @@ typedef enum {
     MM_OPT_FREE_COUPLING = 4,/* 1: the source term of the substeps is k_on M_f(r0) from the table of the last
                                 mm_update_free_motors (which switches it on); 0: the constant k_on m_free again.
                                 MM_ERR_STATE when set to 1 before any mm_update_free_motors */
+    MM_OPT_SPREAD_ATOMIC = 6,/* 0 (default): mm_spread_force gathers -- for a fixed (theta, j) the 4 x 4 stencil is the same
+                                at every (x, y), so every fluid node sums its shifted sources in a fixed order
+                                (reproducible bit for bit); 1: the first version, one fp64 atomic add per point force
+                                and stencil node (summation order varies from call to call) */
     MM_OPT_FREE_REFRESH = 5  /* k > 0: with the coupled source, mm_substep redoes the coarse reduction, the cap and M_f
                                 (what mm_update_free_motors does) before every k-th substep of a call -- Alg. 2's own
                                 cadence, where l.14-20 sit inside the inner loop, is k = 1; at most k
@@ -177,9 +181,12 @@ mm_status mm_local_steps(mm_ctx *ctx, int32_t *n_steps, double *lambda, int dst_
  * Peskin's 4-point kernel phi per direction:
  *     F2[gx][gy][.] = dtheta ds sum_{c,j} Psi_c f_j(c) phi(nx (X - X_g)_x) phi(ny (X - X_g)_y).
  * mm_set_psi : Psi [Nc], fp64 (macroscale data stays double), copied.
- * mm_spread_force : F2 [nx][ny][2] fp64, OVERWRITTEN with the spread force of the current density; fp64 atomic adds,
- *                   so the summation order (not the value beyond rounding) varies from call to call.
- *                   MM_ERR_STATE unless density and Psi have been set. */
+ * mm_spread_force : F2 [nx][ny][2] fp64, OVERWRITTEN with the spread force of the current density.  Computed as a
+ *                   gather in a fixed summation order: the same inputs give the same bits (MM_OPT_SPREAD_ATOMIC = 1:
+ *                   fp64 atomic adds, order varies from call to call).  The head's node coordinate is evaluated as
+ *                   ix + s_j cos(theta) nx (translation-invariant), the oracle's ((ix/nx) + s_j cos(theta)) nx to
+ *                   rounding.  MM_ERR_STATE unless density and Psi have been set; MM_ERR_INVALID_ARG when ntheta * ns >
+ *                   2097120. */
 mm_status mm_set_psi(mm_ctx *ctx, const double *psi, int src_on_device);
 mm_status mm_spread_force(mm_ctx *ctx, double *F2, int dst_on_device);
 

@@ -14,6 +14,7 @@ MM_F32, MM_F64 = 0, 1
 MM_OK, MM_ERR_INVALID_ARG, MM_ERR_CUDA, MM_ERR_NOMEM, MM_ERR_STATE, MM_ERR_UNSTABLE = 0, -1, -2, -3, -4, -5
 MM_FLAG_S_PERIODIC, MM_FLAG_OFFSET_PERIODIC_NOMASK, MM_FLAG_CHECK_DT = 1, 2, 4
 MM_OPT_KERNEL, MM_OPT_FUSE_T, MM_OPT_FUSE_MOMENTS, MM_OPT_INPLACE, MM_OPT_FREE_COUPLING, MM_OPT_FREE_REFRESH = 0, 1, 2, 3, 4, 5
+MM_OPT_SPREAD_ATOMIC = 6
 MM_MAX_FUSE_T = 12
 MM_LOCAL_FUSE_T = 4
 

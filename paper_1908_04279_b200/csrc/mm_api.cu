@@ -129,7 +129,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->inside = nullptr; c->mom_force = c->mom_torque = nullptr; c->flag_dev = nullptr;
     c->loc_lambda = nullptr; c->loc_n = c->loc_nmax = c->loc_list = c->loc_count = nullptr; c->loc_dt = nullptr;
     c->loc_valid = false;
-    c->psi = c->fline = c->F2 = nullptr; c->psi_set = false;
+    c->psi = c->fline = c->F2 = c->spread_G = c->spread_part = nullptr; c->psi_set = false; c->opt_spread_atomic = 0;
     c->Mf_f32 = nullptr;
     c->Mf = c->Mbc = c->free_raw = c->free_factor = nullptr; c->free_fx = nullptr; c->free_any = nullptr; c->coupled = false;
     c->mom_valid = c->vel_set = false; c->tile_ok = false; c->fline_valid = false;
@@ -197,7 +197,7 @@ extern "C" mm_status mm_destroy(mm_ctx *c)
     cudaFree(c->mom_force); cudaFree(c->mom_torque); cudaFree(c->flag_dev);
     cudaFree(c->loc_lambda); cudaFree(c->loc_n); cudaFree(c->loc_nmax); cudaFree(c->loc_dt);
     cudaFree(c->loc_list); cudaFree(c->loc_count);
-    cudaFree(c->psi); cudaFree(c->fline); cudaFree(c->F2);
+    cudaFree(c->psi); cudaFree(c->fline); cudaFree(c->F2); cudaFree(c->spread_G); cudaFree(c->spread_part);
     cudaFree(c->Mf_f32); cudaFree(c->Mf); cudaFree(c->Mbc); cudaFree(c->free_raw); cudaFree(c->free_factor); cudaFree(c->free_fx); cudaFree(c->free_any);
     delete c;
     return MM_OK;
@@ -540,15 +540,32 @@ static mm_status spread_impl(mm_ctx *c)
         c->launches++;
         c->fline_valid = true;
     }
-    CUDA_TRY(c, cudaMemsetAsync(c->F2, 0, (size_t)c->g.nx * c->g.ny * 2 * sizeof(double), c->stream));
-    const int64_t total = c->nc * c->g.ns * 4;
-    int64_t sb = (total + 255) / 256;
-    const int64_t scap = (int64_t)c->sm_count * 32;
-    if (sb > scap) sb = scap;
-    spread_kernel<<<(unsigned)sb, 256, 0, c->stream>>>(c->nc, c->g.ns, c->g.nx, c->g.ny, c->g.ntheta, c->p.s_lo,
-                                                       (c->p.s_hi - c->p.s_lo) / c->g.ns, c->psi, c->fline, c->F2);
+    const double ds = (c->p.s_hi - c->p.s_lo) / c->g.ns;
+    const int nn = c->g.nx * c->g.ny, nt = c->g.ntheta * c->g.ns;
+    if (c->opt_spread_atomic) {   // the first version: one thread per point force and stencil column, fp64 atomic adds
+        CUDA_TRY(c, cudaMemsetAsync(c->F2, 0, (size_t)nn * 2 * sizeof(double), c->stream));
+        const int64_t total = c->nc * c->g.ns * 4;
+        int64_t sb = (total + 255) / 256;
+        const int64_t scap = (int64_t)c->sm_count * 32;
+        if (sb > scap) sb = scap;
+        spread_kernel<<<(unsigned)sb, 256, 0, c->stream>>>(c->nc, c->g.ns, c->g.nx, c->g.ny, c->g.ntheta, c->p.s_lo, ds, c->psi,
+                                                           c->fline, c->F2);
+        CUDA_TRY(c, cudaGetLastError());
+        c->launches += 1;
+        return MM_OK;
+    }
+    // gather: scale + transpose the plane forces, one thread per target node and chunk of (theta, j) pairs, chunks summed
+    const int nchunks = (nt + SPREAD_CH - 1) / SPREAD_CH;
+    const double w0 = 2.0 * 3.14159265358979323846264338327950288 / (double)c->g.ntheta * ds;
+    spread_transpose_kernel<<<dim3((unsigned)((nn + 31) / 32), (unsigned)((nt + 31) / 32)), dim3(32, 8), 0, c->stream>>>(
+        nn, c->g.ntheta, c->g.ns, w0, c->psi, (const double2 *)c->fline, (double2 *)c->spread_G);
     CUDA_TRY(c, cudaGetLastError());
-    c->launches += 1;
+    spread_gather_kernel<<<dim3((unsigned)((nn + 255) / 256), (unsigned)nchunks), 256, 0, c->stream>>>(
+        c->g.nx, c->g.ny, c->g.ntheta, c->g.ns, c->p.s_lo, ds, (const double2 *)c->spread_G, (double2 *)c->spread_part);
+    CUDA_TRY(c, cudaGetLastError());
+    spread_sum_kernel<<<(unsigned)((nn + 255) / 256), 256, 0, c->stream>>>(nn, nchunks, (const double2 *)c->spread_part, (double2 *)c->F2);
+    CUDA_TRY(c, cudaGetLastError());
+    c->launches += 3;
     return MM_OK;
 }
 
@@ -557,15 +574,20 @@ extern "C" mm_status mm_spread_force(mm_ctx *c, double *F2, int on_device)
     if (!c) return MM_ERR_INVALID_ARG;
     if (!F2) return fail(c, MM_ERR_INVALID_ARG, "NULL destination");
     if (c->dens_cov_count != c->nc || !c->psi_set) return fail(c, MM_ERR_STATE, "set density and psi first");
-    if (!c->F2) {   // allocated as a pair, committed together
-        void *a = nullptr, *b = nullptr;
+    if ((int64_t)c->g.ntheta * c->g.ns > 65535LL * 32)
+        return fail(c, MM_ERR_INVALID_ARG, "mm_spread_force: ntheta * ns must be <= 2097120");
+    if (!c->F2) {   // allocated as a group, committed together
+        void *a = nullptr, *b = nullptr, *g = nullptr, *pt = nullptr;
+        const size_t nchunks = ((size_t)c->g.ntheta * c->g.ns + SPREAD_CH - 1) / SPREAD_CH;
         if (cudaMalloc(&a, (size_t)c->nc * c->g.ns * 2 * sizeof(double)) != cudaSuccess ||
-            cudaMalloc(&b, (size_t)c->g.nx * c->g.ny * 2 * sizeof(double)) != cudaSuccess) {
+            cudaMalloc(&b, (size_t)c->g.nx * c->g.ny * 2 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&g, (size_t)c->nc * c->g.ns * 2 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&pt, nchunks * c->g.nx * c->g.ny * 2 * sizeof(double)) != cudaSuccess) {
             cudaGetLastError();
-            cudaFree(a);
+            cudaFree(a); cudaFree(b); cudaFree(g);
             return fail(c, MM_ERR_NOMEM, "device allocation failed (spreading buffers)");
         }
-        c->fline = (double *)a; c->F2 = (double *)b;
+        c->fline = (double *)a; c->F2 = (double *)b; c->spread_G = (double *)g; c->spread_part = (double *)pt;
     }
     mm_status s = c->dtype == MM_F64 ? spread_impl<double>(c) : spread_impl<float>(c);
     if (s != MM_OK) return s;
@@ -702,6 +724,7 @@ extern "C" mm_status mm_set_option(mm_ctx *c, mm_option opt, int64_t v)
     case MM_OPT_INPLACE:
         if (c->single && !v) return fail(c, MM_ERR_INVALID_ARG, "a single-buffer context is always in place");
         c->opt_inplace = v ? 1 : 0; return MM_OK;
+    case MM_OPT_SPREAD_ATOMIC: c->opt_spread_atomic = v ? 1 : 0; return MM_OK;
     }
     return fail(c, MM_ERR_INVALID_ARG, "unknown option");
 }
@@ -716,6 +739,7 @@ extern "C" mm_status mm_get_option(const mm_ctx *c, mm_option opt, int64_t *v)
     case MM_OPT_INPLACE: *v = c->opt_inplace; return MM_OK;
     case MM_OPT_FREE_COUPLING: *v = c->coupled ? 1 : 0; return MM_OK;
     case MM_OPT_FREE_REFRESH: *v = c->opt_free_refresh; return MM_OK;
+    case MM_OPT_SPREAD_ATOMIC: *v = c->opt_spread_atomic; return MM_OK;
     }
     return MM_ERR_INVALID_ARG;
 }

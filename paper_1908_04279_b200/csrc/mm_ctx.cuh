@@ -44,6 +44,8 @@ struct mm_ctx {
     void *loc_dt;
     bool loc_valid;
     double *psi, *fline, *F2;       // NEXT-4: filament density weights [nc], plane forces [nc][ns][2], fluid-grid force
+    double *spread_G, *spread_part; // ... scaled plane forces transposed to [theta][j][node][2], per-chunk partial sums
+    int opt_spread_atomic;
     bool psi_set, fline_valid;      // fline_valid: fline holds the plane forces of the CURRENT density
     float *Mf_f32;                               // fp32 contexts: M_f rounded to fp32 (written with the table)
     double *Mf, *Mbc, *free_raw, *free_factor;   // NEXT-2: free / coarse bound motor tables [nx][ny], scratch

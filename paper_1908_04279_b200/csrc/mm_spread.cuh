@@ -89,4 +89,101 @@ __global__ void __launch_bounds__(256) spread_kernel(int64_t nc, int ns, int nx,
     }
 }
 
+// ---- spreading as a GATHER (default).  The head of (ix, iy, itheta, j) sits at node coordinates (ix + t_x, iy + t_y)
+// with t = s_j p(theta) (nx, ny): for a fixed pair (itheta, j) the stencil -- its integer offset floor(t) and its 4 x 4
+// weights -- is the same for every (ix, iy), so
+//     F2[g] = sum_{theta,j} sum_{u,v} w_{theta,j}(u, v) G_{theta,j}[g - floor(t) - (u, v)],   G = dtheta ds Psi f_j,
+// 2048 shifted 4 x 4 stencils over 128 x 128 fields at configs[4] instead of 1.07 G atomic adds, and a sum in a fixed
+// order.  Three kernels: (1) scale and transpose the plane forces to G[tj][node] (tj = itheta ns + j), so that the
+// nodes a warp reads are contiguous; (2) one thread per target node and chunk of SPREAD_CH pairs tj; (3) the chunks
+// summed in order.
+constexpr int SPREAD_CH = 32;
+
+__global__ void __launch_bounds__(256) spread_transpose_kernel(int nn, int ntheta, int ns, double w, const double *__restrict__ psi,
+                                                               const double2 *__restrict__ fl, double2 *__restrict__ G)
+{
+    __shared__ double2 tile[32][33];
+    const int nt = ntheta * ns;
+    const int n0 = blockIdx.x * 32, tj0 = blockIdx.y * 32;
+    for (int r = threadIdx.y; r < 32; r += 8) {   // rows: nodes; columns: tj (contiguous in fl)
+        const int node = n0 + r, tj = tj0 + threadIdx.x;
+        if (node < nn && tj < nt) {
+            const double2 f = fl[(int64_t)node * nt + tj];
+            const double ws = w * psi[(int64_t)node * ntheta + tj / ns];
+            tile[r][threadIdx.x] = make_double2(ws * f.x, ws * f.y);
+        }
+    }
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += 8) {   // rows: tj; columns: nodes (contiguous in G)
+        const int tj = tj0 + r, node = n0 + threadIdx.x;
+        if (node < nn && tj < nt) G[(int64_t)tj * nn + node] = tile[threadIdx.x][r];
+    }
+}
+
+__global__ void __launch_bounds__(256) spread_gather_kernel(int nx, int ny, int ntheta, int ns, double s_lo, double ds,
+                                                            const double2 *__restrict__ G, double2 *__restrict__ part)
+{
+    __shared__ double wgt[SPREAD_CH][16];
+    __shared__ int off[SPREAD_CH][2];
+    const int nn = nx * ny, nt = ntheta * ns;
+    const int tj0 = blockIdx.y * SPREAD_CH;
+    const int ntj = min(SPREAD_CH, nt - tj0);
+    if ((int)threadIdx.x < ntj) {   // the stencil of pair tj: offset reduced to [0, n), weights phi(frac - u) phi(frac - v)
+        const int tj = tj0 + threadIdx.x, itheta = tj / ns, j = tj - itheta * ns;
+        const double theta = 2.0 * 3.14159265358979323846264338327950288 * (double)itheta / (double)ntheta;
+        const double sj = s_lo + (j + 0.5) * ds;
+        const double tx = sj * cos(theta) * nx, ty = sj * sin(theta) * ny;
+        const double bx = floor(tx), by = floor(ty);
+        double wx[4], wy[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { wx[u] = peskin4(tx - (bx + (u - 1))); wy[u] = peskin4(ty - (by + (u - 1))); }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int v = 0; v < 4; ++v) wgt[threadIdx.x][u * 4 + v] = wx[u] * wy[v];
+        long ox = (long)bx % nx, oy = (long)by % ny;
+        off[threadIdx.x][0] = (int)(ox < 0 ? ox + nx : ox);
+        off[threadIdx.x][1] = (int)(oy < 0 ? oy + ny : oy);
+    }
+    __syncthreads();
+    const int node = blockIdx.x * 256 + threadIdx.x;
+    if (node >= nn) return;
+    const int gx = node / ny, gy = node - gx * ny;
+    double ax = 0.0, ay = 0.0;
+    for (int t = 0; t < ntj; ++t) {
+        const double2 *Gt = G + (int64_t)(tj0 + t) * nn;
+        // the source of stencil point (u, v) is the node g - offset - (u, v): start at u = v = -1, step down with wrap
+        int sx = gx - off[t][0] + 1, sy0 = gy - off[t][1] + 1;
+        sx = sx < 0 ? sx + nx : (sx >= nx ? sx - nx : sx);
+        sy0 = sy0 < 0 ? sy0 + ny : (sy0 >= ny ? sy0 - ny : sy0);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            int sy = sy0;
+#pragma unroll
+            for (int v = 0; v < 4; ++v) {
+                const double2 g = Gt[sx * ny + sy];
+                const double w = wgt[t][u * 4 + v];
+                ax = fma(w, g.x, ax);
+                ay = fma(w, g.y, ay);
+                sy = sy == 0 ? ny - 1 : sy - 1;
+            }
+            sx = sx == 0 ? nx - 1 : sx - 1;
+        }
+    }
+    part[(int64_t)blockIdx.y * nn + node] = make_double2(ax, ay);
+}
+
+__global__ void __launch_bounds__(256) spread_sum_kernel(int nn, int nchunks, const double2 *__restrict__ part, double2 *__restrict__ F2)
+{
+    const int node = blockIdx.x * 256 + threadIdx.x;
+    if (node >= nn) return;
+    double ax = 0.0, ay = 0.0;
+    for (int k = 0; k < nchunks; ++k) {
+        const double2 p = part[(int64_t)k * nn + node];
+        ax += p.x;
+        ay += p.y;
+    }
+    F2[node] = make_double2(ax, ay);
+}
+
 }  // namespace mm

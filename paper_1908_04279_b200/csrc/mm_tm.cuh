@@ -150,6 +150,13 @@ struct TmCoef {
     real c0j[QA][CB], cxm[QA][CB], cxp[QA][CB], cem[QA][CB], cep[QA][CB], csm[QA][CB], src[QA][CB];
 };
 
+#ifndef MM_TM_XSTAT
+#define MM_TM_XSTAT 1
+#endif
+// d = a * b + c, kept in program order among its kind (volatile): see tm_level
+__device__ __forceinline__ void fma_ord(float &d, float a, float b, float c) { asm volatile("fma.rn.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c)); }
+__device__ __forceinline__ void fma_ord(double &d, double a, double b, double c) { d = fma(a, b, c); }
+
 // One level of one plane: xo = level lv+1 from xi = level lv and the carry P of level lv (tensor memory, at `ta`), and
 // the new carry for the plane downstream.  SK: bit 0 = no cxm terms (all exactly 0 on this plane), 1 = no cxp, 2 = no
 // cem, 3 = no cep.
@@ -170,6 +177,42 @@ __device__ __forceinline__ void tm_level(const TmCoef<real, QA, CB> &k, const re
         if (!(SK & 4)) lf[q] = shfl_up_r(xi[q][CB - 1], 1);
     }
     tm_wait_ld();
+#if MM_TM_XSTAT
+    if constexpr (sizeof(real) == 4) {
+        // x-stationary, in program order: the (up to) six FMAs that read one xi are adjacent, so that the operand is
+        // read once from the register file (.reuse) -- a three-register FFMA with no reused operand holds the dispatch
+        // port for two cycles (profiles/r02a_README.md).  xo starts as the carry; each product is added exactly once.
+#pragma unroll
+        for (int q = 0; q < QA; ++q)
+#pragma unroll
+            for (int cb = 0; cb < CB; ++cb) xo[q][cb] = Pl[q * CB + cb];
+        real Pn[QA * CB];
+#pragma unroll
+        for (int q = 0; q < QA; ++q)
+#pragma unroll
+            for (int cb = 0; cb < CB; ++cb) {
+                const real xv = xi[q][cb];
+                fma_ord(xo[q][cb], k.c0j[q][cb], xv, xo[q][cb]);
+                fma_ord(Pn[q * CB + cb], k.csm[q][cb], xv, k.src[q][cb]);
+                if (!(SK & 1) && q + 1 < QA) fma_ord(xo[q + 1 < QA ? q + 1 : 0][cb], k.cxm[q + 1 < QA ? q + 1 : 0][cb], xv, xo[q + 1 < QA ? q + 1 : 0][cb]);
+                if (!(SK & 2) && q > 0) fma_ord(xo[q > 0 ? q - 1 : 0][cb], k.cxp[q > 0 ? q - 1 : 0][cb], xv, xo[q > 0 ? q - 1 : 0][cb]);
+                if (!(SK & 4) && cb + 1 < CB) fma_ord(xo[q][cb + 1 < CB ? cb + 1 : 0], k.cem[q][cb + 1 < CB ? cb + 1 : 0], xv, xo[q][cb + 1 < CB ? cb + 1 : 0]);
+                if (!(SK & 8) && cb > 0) fma_ord(xo[q][cb > 0 ? cb - 1 : 0], k.cep[q][cb > 0 ? cb - 1 : 0], xv, xo[q][cb > 0 ? cb - 1 : 0]);
+            }
+        tm_st<QA * CB>(ta, Pn);
+#pragma unroll
+        for (int cb = 0; cb < CB; ++cb) {
+            if (!(SK & 1)) fma_ord(xo[0][cb], k.cxm[0][cb], dn[cb], xo[0][cb]);
+            if (!(SK & 2)) fma_ord(xo[QA - 1][cb], k.cxp[QA - 1][cb], up[cb], xo[QA - 1][cb]);
+        }
+#pragma unroll
+        for (int q = 0; q < QA; ++q) {
+            if (!(SK & 4)) fma_ord(xo[q][0], k.cem[q][0], lf[q], xo[q][0]);
+            if (!(SK & 8)) fma_ord(xo[q][CB - 1], k.cep[q][CB - 1], rt[q], xo[q][CB - 1]);
+        }
+        return;
+    }
+#endif
     // the old carry is consumed at once (its registers die before the new one is staged for the store)
 #pragma unroll
     for (int q = 0; q < QA; ++q)

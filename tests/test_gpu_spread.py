@@ -1,6 +1,7 @@
 """GPU parity of the motor-force spreading (mm_set_psi / mm_spread_force) against the oracle.
 
-The GPU sums with fp64 atomic adds, so the order differs from the oracle's and from run to run: the comparison is
+The GPU sums in another order than the oracle (a gather per fluid node in a fixed order by default; fp64 atomic adds,
+whose order also differs from run to run, with MM_OPT_SPREAD_ATOMIC): the comparison is
 relative to the cancellation-free scale of a node, max_g |F2| of the oracle (all terms of a node share the sign of
 f_j up to the mix of configurations; the force field is O(1) everywhere on these inputs)."""
 import numpy as np
@@ -15,9 +16,11 @@ pytestmark = pytest.mark.gpu
 RNG = np.random.default_rng(1357)
 
 
-def gpu_spread(g, p, dtype, m0, psi, n_sub=0, dt=0.0, vel=None):
-    from paper_1908_04279_b200 import MM
+def gpu_spread(g, p, dtype, m0, psi, n_sub=0, dt=0.0, vel=None, atomic=0, twice=False):
+    from paper_1908_04279_b200 import MM, binding as b
     mm = MM(g, p, dtype)
+    mm.set_option(b.MM_OPT_SPREAD_ATOMIC, atomic)
+    assert mm.get_option(b.MM_OPT_SPREAD_ATOMIC) == atomic
     mm.set_density(np.ascontiguousarray(m0, NPDT[dtype]))
     if n_sub:
         mm.set_filament_velocity(*(np.ascontiguousarray(x, NPDT[dtype]) for x in vel))
@@ -25,20 +28,28 @@ def gpu_spread(g, p, dtype, m0, psi, n_sub=0, dt=0.0, vel=None):
     mm.set_psi(np.ascontiguousarray(psi, np.float64))
     F = np.empty((g.nx, g.ny, 2))
     mm.spread_force(F)
+    if twice:               # the gather sums in a fixed order: a second call returns the same bits
+        F_again = np.empty_like(F)
+        mm.spread_force(F_again)
+        assert np.array_equal(F, F_again)
     out = np.empty((g.nc, g.ns, g.nxi, g.neta), NPDT[dtype])
     mm.get_density(out)
     mm.destroy()
     return F, out
 
 
+# the last three: a grid narrower than the stencil (it wraps onto itself), (theta, j) pairs over several ragged chunks,
+# a node count that fills neither a transpose tile nor a gather block
+@pytest.mark.parametrize("atomic", [0, 1])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("shape", [(6, 5, 8, 7, 16, 16), (8, 8, 4, 6, 8, 8), (3, 4, 5, 5, 3, 7), (16, 16, 8, 12, 16, 16)])
-def test_spread_parity(dtype, shape):
+@pytest.mark.parametrize("shape", [(6, 5, 8, 7, 16, 16), (8, 8, 4, 6, 8, 8), (3, 4, 5, 5, 3, 7), (16, 16, 8, 12, 16, 16),
+                                   (1, 2, 3, 5, 4, 4), (2, 3, 9, 11, 4, 4), (33, 7, 2, 3, 4, 4)])
+def test_spread_parity(dtype, shape, atomic):
     g = Grid(*shape)
     p = Params()
     U, V, Om, m0 = random_inputs(g, p, dtype)
     psi = RNG.random(g.nc)
-    F, _ = gpu_spread(g, p, dtype, m0, psi)
+    F, _ = gpu_spread(g, p, dtype, m0, psi, atomic=atomic, twice=not atomic)
     ref = orc.spread_force(g, p, m0, psi)
     e = np.max(np.abs(F - ref)) / np.max(np.abs(ref))
     assert e <= TOL[dtype], e
