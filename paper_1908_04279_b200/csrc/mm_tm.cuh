@@ -153,9 +153,9 @@ struct TmCoef {
 #ifndef MM_TM_XSTAT
 #define MM_TM_XSTAT 1
 #endif
-// d = a * b + c, kept in program order among its kind (volatile): see tm_level
-__device__ __forceinline__ void fma_ord(float &d, float a, float b, float c) { asm volatile("fma.rn.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c)); }
-__device__ __forceinline__ void fma_ord(double &d, double a, double b, double c) { d = fma(a, b, c); }
+// acc += a * b, kept in program order among its kind (volatile): see tm_level
+__device__ __forceinline__ void fma_ord(float &acc, float a, float b) { asm volatile("fma.rn.f32 %0, %1, %2, %0;" : "+f"(acc) : "f"(a), "f"(b)); }
+__device__ __forceinline__ void fma_ord(double &acc, double a, double b) { asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(acc) : "d"(a), "d"(b)); }
 
 // One level of one plane: xo = level lv+1 from xi = level lv and the carry P of level lv (tensor memory, at `ta`), and
 // the new carry for the plane downstream.  SK: bit 0 = no cxm terms (all exactly 0 on this plane), 1 = no cxp, 2 = no
@@ -178,10 +178,13 @@ __device__ __forceinline__ void tm_level(const TmCoef<real, QA, CB> &k, const re
     }
     tm_wait_ld();
 #if MM_TM_XSTAT
-    if constexpr (sizeof(real) == 4) {
+    {
         // x-stationary, in program order: the (up to) six FMAs that read one xi are adjacent, so that the operand is
-        // read once from the register file (.reuse) -- a three-register FFMA with no reused operand holds the dispatch
-        // port for two cycles (profiles/r02a_README.md).  xo starts as the carry; each product is added exactly once.
+        // read once from the register file (.reuse): an FMA pays for its fresh register operands, two per cycle --
+        // 1.5 cycles with three, 1 with two (profiles/r02a_README.md).  xo starts as the carry and each product is
+        // added exactly once; inside a run the order is chosen so that an accumulator written by three consecutive
+        // runs (from the left cell, by the cell itself, from the right cell) is touched at positions 1, 4 and 6: no
+        // two writes of one accumulator are closer than 8 instructions, and the scheduler has no reason to break a run.
 #pragma unroll
         for (int q = 0; q < QA; ++q)
 #pragma unroll
@@ -192,23 +195,25 @@ __device__ __forceinline__ void tm_level(const TmCoef<real, QA, CB> &k, const re
 #pragma unroll
             for (int cb = 0; cb < CB; ++cb) {
                 const real xv = xi[q][cb];
-                fma_ord(xo[q][cb], k.c0j[q][cb], xv, xo[q][cb]);
-                fma_ord(Pn[q * CB + cb], k.csm[q][cb], xv, k.src[q][cb]);
-                if (!(SK & 1) && q + 1 < QA) fma_ord(xo[q + 1 < QA ? q + 1 : 0][cb], k.cxm[q + 1 < QA ? q + 1 : 0][cb], xv, xo[q + 1 < QA ? q + 1 : 0][cb]);
-                if (!(SK & 2) && q > 0) fma_ord(xo[q > 0 ? q - 1 : 0][cb], k.cxp[q > 0 ? q - 1 : 0][cb], xv, xo[q > 0 ? q - 1 : 0][cb]);
-                if (!(SK & 4) && cb + 1 < CB) fma_ord(xo[q][cb + 1 < CB ? cb + 1 : 0], k.cem[q][cb + 1 < CB ? cb + 1 : 0], xv, xo[q][cb + 1 < CB ? cb + 1 : 0]);
-                if (!(SK & 8) && cb > 0) fma_ord(xo[q][cb > 0 ? cb - 1 : 0], k.cep[q][cb > 0 ? cb - 1 : 0], xv, xo[q][cb > 0 ? cb - 1 : 0]);
+                constexpr int Z = 0;
+                if (!(SK & 4) && cb + 1 < CB) fma_ord(xo[q][cb + 1 < CB ? cb + 1 : Z], k.cem[q][cb + 1 < CB ? cb + 1 : Z], xv);
+                Pn[q * CB + cb] = k.src[q][cb];
+                fma_ord(Pn[q * CB + cb], k.csm[q][cb], xv);
+                if (!(SK & 1) && q + 1 < QA) fma_ord(xo[q + 1 < QA ? q + 1 : Z][cb], k.cxm[q + 1 < QA ? q + 1 : Z][cb], xv);
+                fma_ord(xo[q][cb], k.c0j[q][cb], xv);
+                if (!(SK & 2) && q > 0) fma_ord(xo[q > 0 ? q - 1 : Z][cb], k.cxp[q > 0 ? q - 1 : Z][cb], xv);
+                if (!(SK & 8) && cb > 0) fma_ord(xo[q][cb > 0 ? cb - 1 : Z], k.cep[q][cb > 0 ? cb - 1 : Z], xv);
             }
         tm_st<QA * CB>(ta, Pn);
 #pragma unroll
         for (int cb = 0; cb < CB; ++cb) {
-            if (!(SK & 1)) fma_ord(xo[0][cb], k.cxm[0][cb], dn[cb], xo[0][cb]);
-            if (!(SK & 2)) fma_ord(xo[QA - 1][cb], k.cxp[QA - 1][cb], up[cb], xo[QA - 1][cb]);
+            if (!(SK & 1)) fma_ord(xo[0][cb], k.cxm[0][cb], dn[cb]);
+            if (!(SK & 2)) fma_ord(xo[QA - 1][cb], k.cxp[QA - 1][cb], up[cb]);
         }
 #pragma unroll
         for (int q = 0; q < QA; ++q) {
-            if (!(SK & 4)) fma_ord(xo[q][0], k.cem[q][0], lf[q], xo[q][0]);
-            if (!(SK & 8)) fma_ord(xo[q][CB - 1], k.cep[q][CB - 1], rt[q], xo[q][CB - 1]);
+            if (!(SK & 4)) fma_ord(xo[q][0], k.cem[q][0], lf[q]);
+            if (!(SK & 8)) fma_ord(xo[q][CB - 1], k.cep[q][CB - 1], rt[q]);
         }
         return;
     }
