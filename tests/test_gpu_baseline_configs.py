@@ -183,6 +183,80 @@ def _full_size(idx, scheme):
           f"their density {worst_all:.2e}  (tol {tol})")
 
 
+@pytest.mark.parametrize("idx", [3, 4])
+def test_full_size_macro_cadence_properties(idx):
+    """The macro-cadence operations (NEXT-2, NEXT-4) at BASELINE full size, in the launch configuration `bench.py --full`
+    times.  The oracle cannot produce a fluid-grid field of 8.6 G cells in test time, so what is checked holds at any size:
+    the spreading as a gather against the same spreading with atomic adds (two unrelated algorithms); the total spread
+    force against the S9 moments (oracle pin F2); the coarse bound density conserves the Psi-weighted number of bound
+    motors (pin N2) against a plain fp64 torch reduction; and the entry point without allocation returns the same bits."""
+    import dataclasses
+    import torch
+    from paper_1908_04279_b200 import MM, binding as b
+
+    w = mi.CONFIGS[idx]
+    g = w.grid
+    free_b, _ = torch.cuda.mem_get_info()
+    if 2 * g.cells * ES[w.dtype] + (4 << 30) > free_b:
+        pytest.skip(f"configs[{idx}] needs {2 * g.cells * ES[w.dtype] / 1e9:.0f} GB of device memory")
+    tdt = torch.float64 if w.dtype == "f64" else torch.float32
+    dev = torch.device("cuda:0")
+    gen = torch.Generator(device=dev).manual_seed(1234 + idx)
+    b0 = torch.empty(g.cells, dtype=tdt, device=dev)
+    b1 = torch.empty(g.cells, dtype=tdt, device=dev)
+    mask = torch.from_numpy(mi.inside_mask(g.nxi, g.neta)).to(dev)
+    psi = torch.rand(g.nc, dtype=torch.float64, device=dev, generator=gen) * 3.0
+    dV = (w.params.s_hi - w.params.s_lo) / g.ns * (2 * w.params.R / g.nxi) * (2 * w.params.R / g.neta)
+    wq = 2 * np.pi / g.ntheta * dV
+    # a first context only to take the density in (M_total is chosen from the data below)
+    mm = MM(g, w.params, w.dtype, b0, b1)
+    total = 0.0                                    # w sum_c Psi_c sum_cells m, fp64
+    step = max(1, (1 << 26) // g.inner)
+    for c0 in range(0, g.nc, step):
+        n = min(step, g.nc - c0)
+        blk = torch.rand((n, g.ns, g.nxi, g.neta), dtype=tdt, device=dev, generator=gen) * mask
+        mm.set_density_range(c0, n, blk)           # lands in buffer 0, the current one
+        total += float((blk.double().sum(dim=(1, 2, 3)) * psi[c0:c0 + n]).sum()) * wq
+    mm.destroy()
+    # M_total well above every node sum (no cap), of the order of the sums (the table is fixed point in units of it)
+    p = dataclasses.replace(w.params, m_free=16.0 * total / (g.nx * g.ny))
+    mm = MM(g, p, w.dtype, b0, b1)
+    for c0 in range(0, g.nc, step):                # buffer 0 holds the density already: tell the context, chunk by chunk,
+        n = min(step, g.nc - c0)                   # from a copy (source and destination of a copy must not alias)
+        blk = b0.view(g.nc, g.ns, g.nxi, g.neta)[c0:c0 + n].clone()
+        mm.set_density_range(c0, n, blk)
+    mm.set_psi(psi)
+    tol = TOL[w.dtype]
+
+    # ---- NEXT-4: gather == atomic adds; total force == dtheta sum_c Psi_c Force_c
+    Fg = torch.empty((g.nx, g.ny, 2), dtype=torch.float64, device=dev)
+    Fa = torch.empty_like(Fg)
+    mm.spread_force(Fg)
+    mm.set_option(b.MM_OPT_SPREAD_ATOMIC, 1)
+    mm.spread_force(Fa)
+    mm.set_option(b.MM_OPT_SPREAD_ATOMIC, 0)
+    scale = float(Fa.abs().max())
+    assert scale > 0 and float((Fg - Fa).abs().max()) / scale <= 1e-12
+    F = torch.empty((g.nc, 2), dtype=torch.float64, device=dev)
+    T = torch.empty(g.nc, dtype=torch.float64, device=dev)
+    mm.moments(F, T)
+    tot = (2 * np.pi / g.ntheta) * (psi[:, None] * F).sum(dim=0)
+    ref_scale = (2 * np.pi / g.ntheta) * float((psi[:, None] * F.abs()).sum())
+    assert float((Fg.sum(dim=(0, 1)) - tot).abs().max()) / ref_scale <= tol
+
+    # ---- NEXT-2: conservation, and the entry point without allocation on the same buffer
+    Mbc = torch.empty((g.nx, g.ny), dtype=torch.float64, device=dev)
+    Mf = torch.empty_like(Mbc)
+    mm.update_free_motors(Mbc, Mf)
+    assert float(Mbc.max()) < p.m_free                      # no node capped: the density was not rescaled
+    assert abs(float(Mbc.sum()) - total) / total <= 1e-12
+    assert float((Mf - (p.m_free - Mbc)).abs().max()) == 0.0
+    Mbc2, Mf2 = torch.empty_like(Mbc), torch.empty_like(Mbc)
+    b.free_motors_noalloc(g, p, w.dtype, b0, psi, Mbc2, Mf2)
+    assert torch.equal(Mbc2, Mbc) and torch.equal(Mf2, Mf)  # fixed-point sums: the order of the deposits does not matter
+    mm.destroy()
+
+
 def _is_current(mm, b0, g, npdt):
     """True when b0 holds the current density: compare configuration 0 read through the ABI with b0's."""
     out = np.empty((1, g.ns, g.nxi, g.neta), npdt)
