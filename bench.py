@@ -280,11 +280,13 @@ def measure(mm, w, idx, args, steps, warmup, dev, stream, world, log, full_proto
     ev = kernel_evidence(idx, kname)
     # (1) the roof the fused kernel sits under: FMA issue (no tensor cores: 7-point stencil + reduction)
     fma_peak = b.measure_fma_peak(w.dtype, stream.cuda_stream)             # TFLOP/s, register-only probe, this run
+    fma_fresh3 = b.measure_fma_rate(w.dtype, 3, stream.cuda_stream)        # ... with three fresh register operands per FMA
     nominal_fma = 148 * (64 if w.dtype == "f64" else 128) * 2 * 1.965e9 / 1e12
     alu_tflops = 2.0 * FMA_PER_CELL_UPDATE * cell_updates / sub_s / 1e12
     roofline = {"bound": "alu", "kernel": kname, "achieved": round(alu_tflops, 3), "peak": round(fma_peak, 3),
                 "unit": "TFLOP/s", "frac": round(alu_tflops / fma_peak, 4), "traffic": ev.get("dram_bytes_per_launch"),
                 "peak_source": f"measured in this run: mm_measure_fma_peak({w.dtype}), register-only FMA probe on all SMs",
+                "peak_three_fresh_operands": round(fma_fresh3, 3), "frac_three_fresh_operands": round(alu_tflops / fma_fresh3, 4),
                 "peak_nominal": round(nominal_fma, 2),
                 "peak_nominal_derivation": "148 SMs x %d FMA lanes x 2 flops x 1.965 GHz" % (64 if w.dtype == "f64" else 128),
                 "flops_per_cell_update": 2 * FMA_PER_CELL_UPDATE,
@@ -293,8 +295,10 @@ def measure(mm, w, idx, args, steps, warmup, dev, stream, world, log, full_proto
                 "avg_launch_ms": round(sub_ms / max(n_launch, 1), 4), "kernel_share_of_step": round(sub_ms / ms, 4),
                 "note": "achieved = the method's 6 FMAs per cell-update (12 flops) x cell-updates of the timed mm_substep calls / "
                         "their CUDA-event time; the fused kernel moves one read + one write of the density per fuse_T substeps "
-                        "and is bound by FMA issue, not HBM (roofline_hbm); a three-register FFMA issues every other cycle "
-                        "(DESIGN.md section 8), so 0.5 is the practical ceiling of frac for fp32"}
+                        "and is bound by FMA issue, not HBM (roofline_hbm); an FMA pays for its fresh register operands at two "
+                        "per cycle and scheduler (DESIGN.md section 8a): peak_three_fresh_operands = mm_measure_fma_rate(dtype, 3) "
+                        "in this run is the rate of FMAs whose coefficient, value and accumulator all change, as this "
+                        "stencil's do; about half of the executed instructions are the method's FMAs"}
     # (2) the HBM side: real DRAM rate of the fused pass, the algorithmic (T = 1 byte count) rate, the unfused kernel
     peak, peak_src = measured_peaks()
     alg_gbs = 2.0 * es * cell_updates / sub_s / 1e9                      # 2*sizeof(real) B per cell-update

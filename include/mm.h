@@ -235,6 +235,11 @@ mm_status mm_get_option(const mm_ctx *ctx, mm_option opt, int64_t *value); /* cu
  * device (about 10 ms, on the given cudaStream_t, synchronises it) and returns the rate in TFLOP/s (2 flops per FMA).
  * Needs no context.  MM_ERR_CUDA without a device. */
 mm_status mm_measure_fma_peak(mm_dtype dtype, void *cuda_stream, double *tflops);
+/* The same measurement by the number of FRESH register operands per FMA: fresh_operands = 1 is mm_measure_fma_peak (two
+ * operands loop-invariant: the FMA unit's rate); 3 = coefficient, value and accumulator all change from one FMA to the
+ * next, as in a stencil with per-lane coefficients: the rate the register file sustains (two 32-bit operands per cycle
+ * and scheduler: about 2/3 of the peak for fp32).  MM_ERR_INVALID_ARG for other counts. */
+mm_status mm_measure_fma_rate(mm_dtype dtype, int32_t fresh_operands, void *cuda_stream, double *tflops);
 
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t mm_launch_count(const mm_ctx *ctx);

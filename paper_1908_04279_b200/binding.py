@@ -21,7 +21,7 @@ MM_LOCAL_FUSE_T = 4
 EXPORTS = ["mm_create", "mm_set_density", "mm_get_density", "mm_set_density_range", "mm_get_density_range",
            "mm_set_filament_velocity", "mm_substep", "mm_moments", "mm_set_option", "mm_get_option", "mm_launch_count",
            "mm_kernel_name", "mm_destroy", "mm_status_string", "mm_last_error", "mm_advance_local", "mm_local_steps", "mm_set_psi",
-           "mm_spread_force", "mm_update_free_motors", "mm_measure_fma_peak", "mm_free_motors_noalloc"]
+           "mm_spread_force", "mm_update_free_motors", "mm_measure_fma_peak", "mm_measure_fma_rate", "mm_free_motors_noalloc"]
 MM_NOALLOC_MAX_NODES = 16384
 
 
@@ -80,6 +80,7 @@ def lib():
         L.mm_last_error.argtypes = [vp]
         L.mm_last_error.restype = ctypes.c_char_p
         L.mm_measure_fma_peak.argtypes = [ctypes.c_int, vp, ctypes.POINTER(dbl)]
+        L.mm_measure_fma_rate.argtypes = [ctypes.c_int, ctypes.c_int32, vp, ctypes.POINTER(dbl)]
         _lib = L
     return _lib
 
@@ -135,6 +136,19 @@ def measure_fma_peak(dtype: str, stream: int | None = None) -> float:
         stream = torch.cuda.current_stream().cuda_stream
     out = ctypes.c_double()
     st = L.mm_measure_fma_peak(MM_F64 if dtype == "f64" else MM_F32, ctypes.c_void_p(stream), ctypes.byref(out))
+    if st != MM_OK:
+        raise MMError(st, L.mm_status_string(st).decode(), L.mm_last_error(None).decode())
+    return float(out.value)
+
+
+def measure_fma_rate(dtype: str, fresh_operands: int, stream: int | None = None) -> float:
+    """TFLOP/s of the FMA probe with 1 or 3 fresh register operands per FMA (mm_measure_fma_rate)."""
+    L = lib()
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    out = ctypes.c_double()
+    st = L.mm_measure_fma_rate(MM_F64 if dtype == "f64" else MM_F32, int(fresh_operands), ctypes.c_void_p(stream), ctypes.byref(out))
     if st != MM_OK:
         raise MMError(st, L.mm_status_string(st).decode(), L.mm_last_error(None).decode())
     return float(out.value)

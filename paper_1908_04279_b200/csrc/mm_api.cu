@@ -776,6 +776,52 @@ static mm_status fma_peak_impl(cudaStream_t stream, double *tflops)
     return MM_OK;
 }
 
+template <typename real>
+static mm_status fma_fresh_impl(cudaStream_t stream, double *tflops)
+{
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return fail(nullptr, MM_ERR_CUDA, "no CUDA device");
+    real *out = nullptr, *in = nullptr;
+    if (cudaMalloc(&out, (size_t)sms * 512 * sizeof(real)) != cudaSuccess || cudaMalloc(&in, 24 * sizeof(real)) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(out);
+        return fail(nullptr, MM_ERR_NOMEM, "device allocation failed");
+    }
+    real h[24];
+    for (int i = 0; i < 24; ++i) h[i] = i < 8 ? (real)(0.5 + 0.01 * i) : (i < 16 ? (real)(0.25 + 0.01 * i) : (real)(1e-3 * i));
+    cudaMemcpyAsync(in, h, sizeof h, cudaMemcpyHostToDevice, stream);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = sizeof(real) == 8 ? 2048 : 4096;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {   // the first repetition is the warm-up
+        cudaEventRecord(e0, stream);
+        fma_fresh_kernel<real><<<sms, 512, 0, stream>>>(out, in, iters);
+        cudaEventRecord(e1, stream);
+        if (cudaEventSynchronize(e1) != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double flops = 2.0 * 64.0 * iters * 512.0 * sms;
+        if (rep > 0 && ms > 0.f && flops / (ms * 1e-3) / 1e12 > best) best = flops / (ms * 1e-3) / 1e12;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out); cudaFree(in);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess || best <= 0.0) return fail(nullptr, MM_ERR_CUDA, std::string("FMA operand probe failed: ") + cudaGetErrorString(e));
+    *tflops = best;
+    return MM_OK;
+}
+
+extern "C" mm_status mm_measure_fma_rate(mm_dtype dtype, int32_t fresh_operands, void *cuda_stream, double *tflops)
+{
+    if (!tflops) return fail(nullptr, MM_ERR_INVALID_ARG, "NULL argument");
+    if (dtype != MM_F32 && dtype != MM_F64) return fail(nullptr, MM_ERR_INVALID_ARG, "bad dtype");
+    if (fresh_operands == 1) return mm_measure_fma_peak(dtype, cuda_stream, tflops);
+    if (fresh_operands != 3) return fail(nullptr, MM_ERR_INVALID_ARG, "fresh_operands must be 1 (mm_measure_fma_peak) or 3");
+    return dtype == MM_F64 ? fma_fresh_impl<double>((cudaStream_t)cuda_stream, tflops) : fma_fresh_impl<float>((cudaStream_t)cuda_stream, tflops);
+}
+
 extern "C" mm_status mm_measure_fma_peak(mm_dtype dtype, void *cuda_stream, double *tflops)
 {
     if (!tflops) return fail(nullptr, MM_ERR_INVALID_ARG, "NULL argument");

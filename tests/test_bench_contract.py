@@ -41,6 +41,8 @@ def test_cuda_arm_line_and_option_legs():
     assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-3
     assert 0 < r["frac"] < 1 and 0.5 * r["peak_nominal"] < r["peak"] < 1.1 * r["peak_nominal"] and "traffic" in r
     assert r["kernel"].startswith("tm<") and r["flops_per_cell_update"] == 12
+    assert 0.5 * r["peak"] < r["peak_three_fresh_operands"] < 0.95 * r["peak"]
+    assert abs(r["frac_three_fresh_operands"] - r["achieved"] / r["peak_three_fresh_operands"]) < 1e-3
     assert h["bound"] == "hbm" and h["unit"] == "GB/s" and abs(h["frac"] - h["achieved"] / h["peak"]) < 1e-3
     for k in ("frac_nominal_8tbs", "effective_gbs", "effective_frac", "t1_gbs", "t1_frac", "t1_frac_nominal_8tbs"):
         assert k in h, k
