@@ -130,7 +130,7 @@ extern "C" mm_status mm_create(const mm_grid *grid, const mm_params *params, mm_
     c->loc_lambda = nullptr; c->loc_n = c->loc_nmax = c->loc_list = c->loc_count = nullptr; c->loc_dt = nullptr;
     c->loc_valid = false;
     c->psi = c->fline = c->F2 = c->spread_G = c->spread_part = nullptr; c->psi_set = false; c->opt_spread_atomic = 0;
-    c->Mf_f32 = nullptr;
+    c->Mf_f32 = nullptr; c->node_tab_x = c->node_tab_y = nullptr;
     c->Mf = c->Mbc = c->free_raw = c->free_factor = nullptr; c->free_fx = nullptr; c->free_any = nullptr; c->coupled = false;
     c->mom_valid = c->vel_set = false; c->tile_ok = false; c->fline_valid = false;
     c->dens_cov_count = 0;
@@ -198,7 +198,7 @@ extern "C" mm_status mm_destroy(mm_ctx *c)
     cudaFree(c->loc_lambda); cudaFree(c->loc_n); cudaFree(c->loc_nmax); cudaFree(c->loc_dt);
     cudaFree(c->loc_list); cudaFree(c->loc_count);
     cudaFree(c->psi); cudaFree(c->fline); cudaFree(c->F2); cudaFree(c->spread_G); cudaFree(c->spread_part);
-    cudaFree(c->Mf_f32); cudaFree(c->Mf); cudaFree(c->Mbc); cudaFree(c->free_raw); cudaFree(c->free_factor); cudaFree(c->free_fx); cudaFree(c->free_any);
+    cudaFree(c->node_tab_x); cudaFree(c->Mf_f32); cudaFree(c->Mf); cudaFree(c->Mbc); cudaFree(c->free_raw); cudaFree(c->free_factor); cudaFree(c->free_fx); cudaFree(c->free_any);
     delete c;
     return MM_OK;
 }
@@ -664,10 +664,15 @@ extern "C" mm_status mm_update_free_motors(mm_ctx *c, double *Mb_coarse, double 
     if (c->dens_cov_count != c->nc || !c->psi_set) return fail(c, MM_ERR_STATE, "set density and psi first");
     const size_t nn = (size_t)c->g.nx * c->g.ny;
     if (!c->free_any) {   // allocated as a group, committed together
-        void *g[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-        const size_t bytes[7] = {nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * 16,
-                                 nn * sizeof(float), sizeof(int)};
-        for (int i = 0; i < 7; ++i)
+        void *g[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+        // the anchor-node tables of the vector / tensor-memory kernels (16-bit entries; the BASELINE offset planes)
+        const mm_grid &gr = c->g;
+        const bool tabs = ((gr.nxi == 16 && gr.neta == 16) || (gr.nxi == 8 && gr.neta == 8)) && gr.nx <= 65535 && gr.ny <= 65535;
+        const size_t tabx_bytes = (((size_t)gr.nx * gr.ntheta * gr.ns * gr.nxi * 2 + 255) / 256) * 256;
+        const size_t taby_bytes = (size_t)gr.ny * gr.ntheta * gr.ns * gr.neta * 2;
+        const size_t bytes[8] = {nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * sizeof(double), nn * 16,
+                                 nn * sizeof(float), sizeof(int), tabs ? tabx_bytes + taby_bytes : 256};
+        for (int i = 0; i < 8; ++i)
             if (cudaMalloc(&g[i], bytes[i]) != cudaSuccess) {
                 cudaGetLastError();
                 for (int k = 0; k < i; ++k) cudaFree(g[k]);
@@ -675,6 +680,23 @@ extern "C" mm_status mm_update_free_motors(mm_ctx *c, double *Mb_coarse, double 
             }
         c->Mf = (double *)g[0]; c->Mbc = (double *)g[1]; c->free_raw = (double *)g[2]; c->free_factor = (double *)g[3];
         c->free_fx = (unsigned long long *)g[4]; c->Mf_f32 = (float *)g[5]; c->free_any = (int *)g[6];
+        if (tabs) {
+            unsigned short *tx = (unsigned short *)g[7], *ty = (unsigned short *)((char *)g[7] + tabx_bytes);
+            FreeGeom q;
+            const mm_params &p = c->p;
+            q.R = p.R; q.dxi = 2.0 * p.R / gr.nxi; q.deta = 2.0 * p.R / gr.neta; q.ds = (p.s_hi - p.s_lo) / gr.ns; q.s_lo = p.s_lo;
+            q.ns = gr.ns; q.nxi = gr.nxi; q.neta = gr.neta; q.ntheta = gr.ntheta; q.nx = gr.nx; q.ny = gr.ny;
+            node_table_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(q, tx, ty);
+            if (cudaGetLastError() != cudaSuccess) {
+                for (int k = 0; k < 8; ++k) cudaFree(g[k]);
+                c->Mf = c->Mbc = c->free_raw = c->free_factor = nullptr; c->free_fx = nullptr; c->Mf_f32 = nullptr; c->free_any = nullptr;
+                return fail(c, MM_ERR_CUDA, "anchor-node table kernel failed to launch");
+            }
+            c->launches++;
+            c->node_tab_x = tx; c->node_tab_y = ty;
+        } else {
+            cudaFree(g[7]);
+        }
     }
     mm_status s = c->dtype == MM_F64 ? free_impl<double>(c) : free_impl<float>(c);
     if (s != MM_OK) return s;

@@ -31,6 +31,7 @@ struct KParams {
     const double *Mf;                  // NULL, or the free-motor table [nx][ny] (NEXT-2); generic kernels only
     const real *Mf_r;                  // the same table rounded to `real` (fp64 contexts: the table itself): what the
                                        // coefficient-form kernels gather -- no conversion per cell, half the bytes in L1
+    const unsigned short *node_x, *node_y;   // NULL, or the context's anchor-node tables (mm_free.cuh, node_table_kernel)
     int32_t nx, ny;
     double geo_R, geo_dxi, geo_deta, geo_ds, geo_s_lo;   // fp64 geometry for the anchor map (never rounded to fp32)
 };

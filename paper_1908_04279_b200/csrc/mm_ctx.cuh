@@ -47,6 +47,7 @@ struct mm_ctx {
     double *spread_G, *spread_part; // ... scaled plane forces transposed to [theta][j][node][2], per-chunk partial sums
     int opt_spread_atomic;
     bool psi_set, fline_valid;      // fline_valid: fline holds the plane forces of the CURRENT density
+    unsigned short *node_tab_x, *node_tab_y;     // anchor-node tables (one allocation; NULL when nx or ny > 65535)
     float *Mf_f32;                               // fp32 contexts: M_f rounded to fp32 (written with the table)
     double *Mf, *Mbc, *free_raw, *free_factor;   // NEXT-2: free / coarse bound motor tables [nx][ny], scratch
     unsigned long long *free_fx;   // [nx][ny][2]: the coarse sums in 128-bit fixed point (mm_free.cuh)
@@ -94,6 +95,7 @@ inline KParams<real> make_kparams(const mm_ctx *c, double dt)
     k.dt_kon = (real)(dt * p.k_on);
     k.Mf = (c->coupled && c->Mf) ? c->Mf : nullptr;
     k.Mf_r = !k.Mf ? nullptr : (sizeof(real) == 8 ? (const real *)c->Mf : (const real *)c->Mf_f32);
+    k.node_x = k.Mf ? c->node_tab_x : nullptr; k.node_y = k.Mf ? c->node_tab_y : nullptr;
     k.nx = g.nx; k.ny = g.ny;
     k.geo_R = p.R; k.geo_dxi = dxi; k.geo_deta = deta; k.geo_ds = ds; k.geo_s_lo = p.s_lo;
     k.dt_endx = (real)(dt * (p.end_detach_mult - 1.0));

@@ -139,6 +139,33 @@ __device__ __noinline__ void fx_deposit_rare(uint32_t *L0, uint32_t *L1, uint32_
     fx_deposit(L0, L1, L2, n, q);
 }
 
+// The anchor-node tables of a context for the coupled substep kernel (mm_tm.cuh): the x node depends on (ix, itheta, j,
+// a) only, the y node on (iy, itheta, j, b), and the geometry never changes, so the fp64 evaluation (1600 instructions
+// per lane and configuration in that kernel) is done once: tabx[((ix ntheta + itheta) ns + j) nxi + a],
+// taby[((iy ntheta + itheta) ns + j) neta + b].  Same expression, operation by operation, as the inline evaluation
+// (ties break alike).  The deposit pass below keeps the inline evaluation: a table look-up per plane there is a
+// dependent global load in front of the atomics (measured: 10.9 -> 12.2 ms on configs[4]).
+__global__ void __launch_bounds__(256) node_table_kernel(const FreeGeom q, unsigned short *__restrict__ tabx, unsigned short *__restrict__ taby)
+{
+    const int64_t nxe = (int64_t)q.nx * q.ntheta * q.ns * q.nxi, nye = (int64_t)q.ny * q.ntheta * q.ns * q.neta;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < nxe + nye; e += (int64_t)gridDim.x * blockDim.x) {
+        const bool isx = e < nxe;
+        const int64_t i = isx ? e : e - nxe;
+        const int no = isx ? q.nxi : q.neta, n = isx ? q.nx : q.ny;
+        const int k = (int)(i % no);
+        const int j = (int)((i / no) % q.ns);
+        const int itheta = (int)((i / ((int64_t)no * q.ns)) % q.ntheta);
+        const int row = (int)(i / ((int64_t)no * q.ns * q.ntheta));
+        const double theta = 2.0 * 3.14159265358979323846264338327950288 * (double)itheta / (double)q.ntheta;
+        const double cs = isx ? cos(theta) : sin(theta);
+        const double base = __ddiv_rn((double)row, (double)n);
+        const double off = __dadd_rn(-q.R, __dmul_rn(k + 0.5, isx ? q.dxi : q.deta));
+        const double sj = __dadd_rn(q.s_lo, __dmul_rn(j + 0.5, q.ds));
+        const double r = __dmul_rn(__dsub_rn(__dadd_rn(base, __dmul_rn(sj, cs)), off), (double)n);
+        (isx ? tabx : taby)[i] = (unsigned short)wrap_floor(__dadd_rn(r, 0.5), n);
+    }
+}
+
 // old = L[addr]; L[addr] += x -- skipped (old = 0) when x == 0; a predicated ATOMS, no branch around it
 __device__ __forceinline__ uint32_t atoms_add_nz(uint32_t saddr, uint32_t x)
 {

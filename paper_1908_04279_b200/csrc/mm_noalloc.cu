@@ -7,13 +7,15 @@
 // overlap on the GPU (different streams, no ordering between them) race; the array keeps the last call's contents and
 // each call clears what must start at zero.
 #include "mm_ctx.cuh"
-// mm_free.cuh defines two non-template functions with host-side symbols (free_cap_kernel, fx_deposit_rare), which
-// mm_api.cu already emits: this unit's copies get names of their own (free_cap_kernel is not used here -- the node pass
-// below names the scratch array directly)
+// mm_free.cuh defines three non-template functions with host-side symbols (free_cap_kernel, node_table_kernel,
+// fx_deposit_rare), which mm_api.cu already emits: this unit's copies get names of their own (the first two are not
+// used here -- the node pass below names the scratch array directly, and without a context there are no node tables)
 #define free_cap_kernel free_cap_kernel_unused_in_noalloc_unit
+#define node_table_kernel node_table_kernel_unused_in_noalloc_unit
 #define fx_deposit_rare fx_deposit_rare_noalloc_unit
 #include "mm_free.cuh"
 #undef free_cap_kernel
+#undef node_table_kernel
 #undef fx_deposit_rare
 
 #include <mutex>

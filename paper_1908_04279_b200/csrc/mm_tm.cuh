@@ -404,6 +404,22 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                 const int iy = (int)((c / kp.ntheta) % kp.ny), ix = (int)(c / ((int64_t)kp.ntheta * kp.ny));
                 const double mf_tx = __ddiv_rn((double)ix, (double)kp.nx), mf_ty = __ddiv_rn((double)iy, (double)kp.ny);
                 __syncwarp();   // the previous configuration's planes are done with the tables
+                if (kp.node_x) {
+                    // the context's tables: rows (ix, itheta) and (iy, itheta), ns x NXI and ns x NETA entries, copied 8
+                    // entries at a time into the interleaved per-warp table
+                    constexpr int VX = NXI / 8, VY = NETA / 8;
+                    static_assert(NXI % 8 == 0 && NETA % 8 == 0, "vector copy of the node tables");
+                    const uint4 *sx = reinterpret_cast<const uint4 *>(kp.node_x + ((int64_t)ix * kp.ntheta + kth) * kp.ns * NXI);
+                    const uint4 *sy = reinterpret_cast<const uint4 *>(kp.node_y + ((int64_t)iy * kp.ntheta + kth) * kp.ns * NETA);
+                    for (int e = lane; e < kp.ns * VX; e += 32) {
+                        const int jj = e / VX, part = e - jj * VX;
+                        *reinterpret_cast<uint4 *>(nod + jj * (NXI + NETA) + part * 8) = __ldg(sx + e);
+                    }
+                    for (int e = lane; e < kp.ns * VY; e += 32) {
+                        const int jj = e / VY, part = e - jj * VY;
+                        *reinterpret_cast<uint4 *>(nod + jj * (NXI + NETA) + NXI + part * 8) = __ldg(sy + e);
+                    }
+                } else
                 for (int e = lane; e < kp.ns * (NXI + NETA); e += 32) {
                     const int jj = e / (NXI + NETA), r = e - jj * (NXI + NETA);
                     const double sjd = __dadd_rn(kp.geo_s_lo, __dmul_rn(jj + 0.5, kp.geo_ds));
