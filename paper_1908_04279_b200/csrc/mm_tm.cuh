@@ -367,6 +367,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
         for (int64_t i = 0; i < total && i < D; ++i) issue();
 
     TmCoef<real, QA, CB> co;
+    const double pf_scale = PF ? kp.mom_scale / kp.geo_ds : 0.0;   // -k dxi deta (one fp64 division per thread, not per plane)
     real hbx = 0, hbe = 0, ct = 0, st = 0, dtc = real(1);
     int nlev = nlev_pass;
     bool last_pass = true;
@@ -399,10 +400,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             st = kp.sin_t[kth];
             const real U = kp.U[c], Vv = kp.V[c], Om = kp.Om[c];
             if (MF) {
-                const double theta = 2.0 * 3.14159265358979323846264338327950288 * (double)kth / (double)kp.ntheta;
-                const double mf_ct = cos(theta), mf_st = sin(theta);
                 const int iy = (int)((c / kp.ntheta) % kp.ny), ix = (int)(c / ((int64_t)kp.ntheta * kp.ny));
-                const double mf_tx = __ddiv_rn((double)ix, (double)kp.nx), mf_ty = __ddiv_rn((double)iy, (double)kp.ny);
                 __syncwarp();   // the previous configuration's planes are done with the tables
                 if (kp.node_x) {
                     // the context's tables: rows (ix, itheta) and (iy, itheta), ns x NXI and ns x NETA entries, copied 8
@@ -419,7 +417,10 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                         const int jj = e / VY, part = e - jj * VY;
                         *reinterpret_cast<uint4 *>(nod + jj * (NXI + NETA) + NXI + part * 8) = __ldg(sy + e);
                     }
-                } else
+                } else {
+                const double theta = 2.0 * 3.14159265358979323846264338327950288 * (double)kth / (double)kp.ntheta;
+                const double mf_ct = cos(theta), mf_st = sin(theta);
+                const double mf_tx = __ddiv_rn((double)ix, (double)kp.nx), mf_ty = __ddiv_rn((double)iy, (double)kp.ny);
                 for (int e = lane; e < kp.ns * (NXI + NETA); e += 32) {
                     const int jj = e / (NXI + NETA), r = e - jj * (NXI + NETA);
                     const double sjd = __dadd_rn(kp.geo_s_lo, __dmul_rn(jj + 0.5, kp.geo_ds));
@@ -434,6 +435,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                         n = wrap_node(__dadd_rn(__dmul_rn(__dsub_rn(hy_, etd), (double)kp.ny), 0.5), kp.ny);
                     }
                     nod[e] = (unsigned short)n;
+                }
                 }
                 __syncwarp();
             }
@@ -619,7 +621,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     a += __shfl_xor_sync(0xffffffffu, b, 16);
 #pragma unroll
                     for (int o = 8; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-                    if ((lane & 15) == 0) fline[(c * ns + j) * 2 + (lane >> 4)] = (kp.mom_scale / kp.geo_ds) * (double)a;
+                    if ((lane & 15) == 0) fline[(c * ns + j) * 2 + (lane >> 4)] = pf_scale * (double)a;
                 }
             }
         }
