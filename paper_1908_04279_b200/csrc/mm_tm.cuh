@@ -160,7 +160,7 @@ __device__ __forceinline__ void fma_ord(double &acc, double a, double b) { asm v
 // One level of one plane: xo = level lv+1 from xi = level lv and the carry P of level lv (tensor memory, at `ta`), and
 // the new carry for the plane downstream.  SK: bit 0 = no cxm terms (all exactly 0 on this plane), 1 = no cxp, 2 = no
 // cem, 3 = no cep.
-template <int SK, typename real, int QA, int CB, int LB>
+template <int SK, bool XS, typename real, int QA, int CB, int LB>
 __device__ __forceinline__ void tm_level(const TmCoef<real, QA, CB> &k, const real (&xi)[QA][CB], real (&xo)[QA][CB], uint32_t ta)
 {
     real Pl[QA * CB];
@@ -178,7 +178,9 @@ __device__ __forceinline__ void tm_level(const TmCoef<real, QA, CB> &k, const re
     }
     tm_wait_ld();
 #if MM_TM_XSTAT
-    {
+    // taken by the fp64 kernels and the coupled-source fp32 kernels (XS): measured on one box, fp32 plain 2403 G/s
+    // without / 2396 with, coupled whole step 1593 / 1611, fp64 plain 1230 / 1265
+    if constexpr (sizeof(real) == 8 || XS) {
         // x-stationary, in program order: the (up to) six FMAs that read one xi are adjacent, so that the operand is
         // read once from the register file (.reuse): an FMA pays for its fresh register operands, two per cycle --
         // 1.5 cycles with three, 1 with two (profiles/r02a_README.md).  xo starts as the carry and each product is
@@ -262,19 +264,19 @@ __device__ __forceinline__ void tm_plane(const TmCoef<real, QA, CB> &k, real (&x
     if constexpr (COMPACT) {
 #pragma unroll 1
         for (int lv = 0; lv < nlev; lv += 2) {
-            tm_level<SK, real, QA, CB, LB>(k, x, y, tbase + lv * CPL);
+            tm_level<SK, COMPACT, real, QA, CB, LB>(k, x, y, tbase + lv * CPL);
             if (lv + 1 == nlev) { odd = true; break; }
-            tm_level<SK, real, QA, CB, LB>(k, y, x, tbase + lv * CPL + CPL);
+            tm_level<SK, COMPACT, real, QA, CB, LB>(k, y, x, tbase + lv * CPL + CPL);
         }
     } else {
         int lv = 0;
 #pragma unroll 1
         for (; lv + 2 <= nlev; lv += 2) {
-            tm_level<SK, real, QA, CB, LB>(k, x, y, tbase + lv * CPL);
-            tm_level<SK, real, QA, CB, LB>(k, y, x, tbase + lv * CPL + CPL);
+            tm_level<SK, COMPACT, real, QA, CB, LB>(k, x, y, tbase + lv * CPL);
+            tm_level<SK, COMPACT, real, QA, CB, LB>(k, y, x, tbase + lv * CPL + CPL);
         }
         if (lv < nlev) {
-            tm_level<SK, real, QA, CB, LB>(k, x, y, tbase + lv * CPL);
+            tm_level<SK, COMPACT, real, QA, CB, LB>(k, x, y, tbase + lv * CPL);
             odd = true;
         }
     }
