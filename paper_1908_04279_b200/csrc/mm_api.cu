@@ -606,6 +606,7 @@ static mm_status free_impl(mm_ctx *c)
     FreeGeom q;
     q.R = p.R; q.dxi = 2.0 * p.R / g.nxi; q.deta = 2.0 * p.R / g.neta; q.ds = (p.s_hi - p.s_lo) / g.ns; q.s_lo = p.s_lo;
     q.ns = g.ns; q.nxi = g.nxi; q.neta = g.neta; q.ntheta = g.ntheta; q.nx = g.nx; q.ny = g.ny;
+    q.tabx = c->node_tab_x; q.taby = c->node_tab_y;
     const int nn = g.nx * g.ny;
     const double w = 2.0 * 3.14159265358979323846264338327950288 / (double)g.ntheta * q.ds * q.dxi * q.deta;
     CUDA_TRY(c, cudaMemsetAsync(c->free_raw, 0, (size_t)nn * sizeof(double), c->stream));
@@ -686,6 +687,7 @@ extern "C" mm_status mm_update_free_motors(mm_ctx *c, double *Mb_coarse, double 
             const mm_params &p = c->p;
             q.R = p.R; q.dxi = 2.0 * p.R / gr.nxi; q.deta = 2.0 * p.R / gr.neta; q.ds = (p.s_hi - p.s_lo) / gr.ns; q.s_lo = p.s_lo;
             q.ns = gr.ns; q.nxi = gr.nxi; q.neta = gr.neta; q.ntheta = gr.ntheta; q.nx = gr.nx; q.ny = gr.ny;
+            q.tabx = q.taby = nullptr;
             node_table_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(q, tx, ty);
             if (cudaGetLastError() != cudaSuccess) {
                 for (int k = 0; k < 8; ++k) cudaFree(g[k]);

@@ -14,6 +14,7 @@ namespace mm {
 struct FreeGeom {   // fp64 geometry of the anchor map
     double R, dxi, deta, ds, s_lo;
     int32_t ns, nxi, neta, ntheta, nx, ny;
+    const unsigned short *tabx, *taby;   // NULL, or the context's anchor-node tables (node_table_kernel)
 };
 
 __device__ __forceinline__ int anchor_node(const FreeGeom &q, int ix, int iy, double ct, double st, double sj, double xi,
@@ -143,8 +144,9 @@ __device__ __noinline__ void fx_deposit_rare(uint32_t *L0, uint32_t *L1, uint32_
 // a) only, the y node on (iy, itheta, j, b), and the geometry never changes, so the fp64 evaluation (1600 instructions
 // per lane and configuration in that kernel) is done once: tabx[((ix ntheta + itheta) ns + j) nxi + a],
 // taby[((iy ntheta + itheta) ns + j) neta + b].  Same expression, operation by operation, as the inline evaluation
-// (ties break alike).  The deposit pass below keeps the inline evaluation: a table look-up per plane there is a
-// dependent global load in front of the atomics (measured: 10.9 -> 12.2 ms on configs[4]).
+// (ties break alike).  The fp32 deposit pass below reads them too, one 16-bit load per lane and plane issued with the
+// density loads (a look-up at the point of use, a dependent load in front of the atomics, measured 10.9 -> 12.2 ms on
+// configs[4]; prefetched 9.7 ms).
 __global__ void __launch_bounds__(256) node_table_kernel(const FreeGeom q, unsigned short *__restrict__ tabx, unsigned short *__restrict__ taby)
 {
     const int64_t nxe = (int64_t)q.nx * q.ntheta * q.ns * q.nxi, nye = (int64_t)q.ny * q.ntheta * q.ns * q.neta;
@@ -229,22 +231,42 @@ __global__ void __launch_bounds__(PRIV ? (sizeof(real) == 4 ? MM_FREE_PRIV_THREA
         if (MODE == 0 && wp == 0.0) continue;
         const double wps = wp * inv_unit * 4294967296.0;   // powers of two: wps * m rounds as wp * m
         real *mc = dens + c * inner + lane * VW;
+        // with the context's tables the node of this lane (x node of row a = lane, or y node of column b = lane - 16)
+        // is one 16-bit load per plane, issued with the density loads of the plane (a look-up at the point of use is a
+        // dependent load in front of the atomics: slower than the inline evaluation).  fp32 contexts only: 10.9 -> 9.7 ms
+        // on configs[4]; the fp64 pass, closer to its HBM roof and short of registers, got slower with it (3.6 -> 4.1 ms)
+        constexpr bool USE_TAB = sizeof(real) == 4;
+        const unsigned short *tab = nullptr;
+        if (USE_TAB && q.tabx) {
+            const int kk = k16 < (lane < 16 ? NXI : NETA) ? k16 : 0;
+            tab = lane < 16 ? q.tabx + ((int64_t)ix * q.ntheta + itheta) * q.ns * NXI + kk
+                            : q.taby + ((int64_t)iy * q.ntheta + itheta) * q.ns * NETA + kk;
+        }
+        const int tstride = lane < 16 ? NXI : NETA;
         for (int j0 = 0; j0 < q.ns; j0 += PL) {
             Vec v[PL][NV];
+            int tnode[PL];
 #pragma unroll
-            for (int pl = 0; pl < PL; ++pl)
+            for (int pl = 0; pl < PL; ++pl) {
 #pragma unroll
                 for (int k = 0; k < NV; ++k)
                     if (j0 + pl < q.ns) v[pl][k] = *reinterpret_cast<const Vec *>(mc + (int64_t)(j0 + pl) * PLANE + k * 32 * VW);
+                if (USE_TAB) tnode[pl] = (tab && j0 + pl < q.ns) ? (int)tab[(j0 + pl) * tstride] : 0;
+            }
 #pragma unroll
             for (int pl = 0; pl < PL; ++pl) {
                 const int j = j0 + pl;
                 if (j >= q.ns) break;
                 // lanes 0..15: x node of row a = lane (times ny); lanes 16..31: y node of column b = lane - 16; every
                 // operation rounded separately, exactly the oracle's expression (ties)
-                const double sj = __dadd_rn(q.s_lo, __dmul_rn(j + 0.5, q.ds));
-                const double r = __dmul_rn(__dsub_rn(__dadd_rn(base, __dmul_rn(sj, cs)), off), nd);
-                const int my_node = lane < 16 ? wrap_floor(__dadd_rn(r, 0.5), q.nx) * ldt : wrap_floor(__dadd_rn(r, 0.5), q.ny);
+                int my_node;
+                if (USE_TAB && tab) {
+                    my_node = lane < 16 ? tnode[pl] * ldt : tnode[pl];
+                } else {
+                    const double sj = __dadd_rn(q.s_lo, __dmul_rn(j + 0.5, q.ds));
+                    const double r = __dmul_rn(__dsub_rn(__dadd_rn(base, __dmul_rn(sj, cs)), off), nd);
+                    my_node = lane < 16 ? wrap_floor(__dadd_rn(r, 0.5), q.nx) * ldt : wrap_floor(__dadd_rn(r, 0.5), q.ny);
+                }
                 int nb[VW];
 #pragma unroll
                 for (int e = 0; e < VW; ++e) nb[e] = __shfl_sync(0xffffffffu, my_node, 16 + b0 + e);

@@ -82,6 +82,7 @@ static mm_status noalloc_impl(const mm_grid &g, const mm_params &p, real *dens, 
     FreeGeom q;
     q.R = p.R; q.dxi = 2.0 * p.R / g.nxi; q.deta = 2.0 * p.R / g.neta; q.ds = (p.s_hi - p.s_lo) / g.ns; q.s_lo = p.s_lo;
     q.ns = g.ns; q.nxi = g.nxi; q.neta = g.neta; q.ntheta = g.ntheta; q.nx = g.nx; q.ny = g.ny;
+    q.tabx = q.taby = nullptr;   // no context, no tables: the nodes are evaluated inline
     const int nn = g.nx * g.ny;
     const int64_t nc = (int64_t)nn * g.ntheta;
     const double w = 2.0 * 3.14159265358979323846264338327950288 / (double)g.ntheta * q.ds * q.dxi * q.deta;
