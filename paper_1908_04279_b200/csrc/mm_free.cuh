@@ -223,9 +223,13 @@ __global__ void __launch_bounds__(PRIV ? (sizeof(real) == 4 ? MM_FREE_PRIV_THREA
     for (int64_t c = warp0; c < nc; c += nwarps) {
         const int itheta = (int)(c % q.ntheta);
         const int iy = (int)((c / q.ntheta) % q.ny), ix = (int)(c / ((int64_t)q.ntheta * q.ny));
-        const double theta = 2.0 * 3.14159265358979323846264338327950288 * (double)itheta / (double)q.ntheta;
-        const double cs = lane < 16 ? cos(theta) : sin(theta);
-        const double base = lane < 16 ? __ddiv_rn((double)ix, (double)q.nx) : __ddiv_rn((double)iy, (double)q.ny);
+        constexpr bool USE_TAB = sizeof(real) == 4;
+        double cs = 0.0, base = 0.0;   // the inline node evaluation only
+        if (!(USE_TAB && q.tabx)) {
+            const double theta = 2.0 * 3.14159265358979323846264338327950288 * (double)itheta / (double)q.ntheta;
+            cs = lane < 16 ? cos(theta) : sin(theta);
+            base = lane < 16 ? __ddiv_rn((double)ix, (double)q.nx) : __ddiv_rn((double)iy, (double)q.ny);
+        }
         const double nd = lane < 16 ? (double)q.nx : (double)q.ny;
         const double wp = MODE == 0 ? w * psi[c] : 0.0;
         if (MODE == 0 && wp == 0.0) continue;
@@ -235,7 +239,6 @@ __global__ void __launch_bounds__(PRIV ? (sizeof(real) == 4 ? MM_FREE_PRIV_THREA
         // is one 16-bit load per plane, issued with the density loads of the plane (a look-up at the point of use is a
         // dependent load in front of the atomics: slower than the inline evaluation).  fp32 contexts only: 10.9 -> 9.7 ms
         // on configs[4]; the fp64 pass, closer to its HBM roof and short of registers, got slower with it (3.6 -> 4.1 ms)
-        constexpr bool USE_TAB = sizeof(real) == 4;
         const unsigned short *tab = nullptr;
         if (USE_TAB && q.tabx) {
             const int kk = k16 < (lane < 16 ? NXI : NETA) ? k16 : 0;
