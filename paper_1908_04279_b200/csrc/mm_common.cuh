@@ -23,6 +23,7 @@ struct KParams {
     real dt_kon;                       // dt * k_on  (coupled source: dt k_on M_f(r0))
     real dt_endx;                      // dt * (end_detach_mult - 1)         (S6)
     double mom_scale;                  // -k_spring * ds*dxi*deta            (S9)
+    double pf_scale;                   // -k_spring * dxi*deta: scale of a plane force (NEXT-4), = mom_scale / ds
     // per-configuration inputs and tables (device pointers)
     const real *U, *V, *Om;            // [nc]
     const real *cos_t, *sin_t;         // [ntheta], cos/sin(2 pi k / ntheta) evaluated in fp64

@@ -100,6 +100,7 @@ inline KParams<real> make_kparams(const mm_ctx *c, double dt)
     k.geo_R = p.R; k.geo_dxi = dxi; k.geo_deta = deta; k.geo_ds = ds; k.geo_s_lo = p.s_lo;
     k.dt_endx = (real)(dt * (p.end_detach_mult - 1.0));
     k.mom_scale = -p.k_spring * ds * dxi * deta;
+    k.pf_scale = k.mom_scale / ds;   // the quotient the kernels formed (same rounding as before)
     k.U = (const real *)c->U; k.V = (const real *)c->V; k.Om = (const real *)c->Om;
     k.cos_t = (const real *)c->cos_t; k.sin_t = (const real *)c->sin_t;
     k.kappa = (const real *)c->kappa; k.inside = c->inside;

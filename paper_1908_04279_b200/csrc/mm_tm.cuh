@@ -369,7 +369,6 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
         for (int64_t i = 0; i < total && i < D; ++i) issue();
 
     TmCoef<real, QA, CB> co;
-    const double pf_scale = PF ? kp.mom_scale / kp.geo_ds : 0.0;   // -k dxi deta (one fp64 division per thread, not per plane)
     real hbx = 0, hbe = 0, ct = 0, st = 0, dtc = real(1);
     int nlev = nlev_pass;
     bool last_pass = true;
@@ -623,7 +622,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     a += __shfl_xor_sync(0xffffffffu, b, 16);
 #pragma unroll
                     for (int o = 8; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-                    if ((lane & 15) == 0) fline[(c * ns + j) * 2 + (lane >> 4)] = pf_scale * (double)a;
+                    if ((lane & 15) == 0) fline[(c * ns + j) * 2 + (lane >> 4)] = kp.pf_scale * (double)a;   // a kernel parameter: no register held
                 }
             }
         }
