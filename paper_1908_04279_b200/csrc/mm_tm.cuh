@@ -595,21 +595,28 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     *reinterpret_cast<V128 *>(oc + (int64_t)j * PLANE + (a0 + q) * NETA + b0 + v4 * VW) = v;
                 }
             if (mom) {
-                real fxp = 0, fyp = 0;
+                // sum_ab xi_a m and sum_ab eta_b m over the lane's patch, with xi_a = xi_a0 + q dxi, eta_b = eta_b0 + cb
+                // deta: S = sum m, fxp = xi_a0 S + dxi sum_q q rs_q, fyp = eta_b0 S + deta sum_cb cb cs_cb -- two
+                // per-lane coordinates instead of QA + CB (which the compiler rematerialised on every plane)
+                real rs[QA], cs[CB];
 #pragma unroll
                 for (int q = 0; q < QA; ++q) {
-                    real rs = x[q][0];
+                    rs[q] = x[q][0];
 #pragma unroll
-                    for (int cb = 1; cb < CB; ++cb) rs += x[q][cb];
-                    fxp = fma(xiq[q], rs, fxp);
+                    for (int cb = 1; cb < CB; ++cb) rs[q] += x[q][cb];
                 }
 #pragma unroll
                 for (int cb = 0; cb < CB; ++cb) {
-                    real csum = x[0][cb];
+                    cs[cb] = x[0][cb];
 #pragma unroll
-                    for (int q = 1; q < QA; ++q) csum += x[q][cb];
-                    fyp = fma(etab[cb], csum, fyp);
+                    for (int q = 1; q < QA; ++q) cs[cb] += x[q][cb];
                 }
+                real S = rs[0], wq = real(0), wc = real(0);
+#pragma unroll
+                for (int q = 1; q < QA; ++q) { S += rs[q]; wq = fma(real(q), rs[q], wq); }
+#pragma unroll
+                for (int cb = 1; cb < CB; ++cb) wc = fma(real(cb), cs[cb], wc);
+                const real fxp = fma(kp.dxi, wq, xiq[0] * S), fyp = fma(kp.deta, wc, etab[0] * S);
                 FX += fxp;
                 FY += fyp;
                 TQ = fma(sj, ct * fyp - st * fxp, TQ);
