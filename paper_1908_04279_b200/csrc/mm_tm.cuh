@@ -392,10 +392,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     int64_t k = 0, c = 0;
     int ch = 0, slot = 0;
     uint32_t phase = 0;
+    real *optr = out;   // this lane's first cell of the plane being stored
     for (int64_t i = 0; i < total; ++i) {
         if (ch == 0) {
             // ---- per configuration (S2-S4, S6 folded; everything that does not depend on s)
             c = (loc && list) ? (int64_t)list[gw + k * nw] : gw + k * nw;
+            optr = out + c * inner + a0 * NETA + b0;
             const int kth = (int)(c % kp.ntheta);
             ct = kp.cos_t[kth];
             st = kp.sin_t[kth];
@@ -498,7 +500,6 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
 
         mbar_wait(&full[slot], phase);
         const real *sp = ring + (size_t)slot * P * PLANE;
-        real *oc = out + c * inner;
 #pragma unroll 1
         for (int pl = 0; pl < P; ++pl) {
             const int j = ch * P + pl;
@@ -592,8 +593,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     V128 v;
 #pragma unroll
                     for (int e = 0; e < VW; ++e) v.v[e] = x[q][v4 * VW + e];
-                    *reinterpret_cast<V128 *>(oc + (int64_t)j * PLANE + (a0 + q) * NETA + b0 + v4 * VW) = v;
+                    *reinterpret_cast<V128 *>(optr + q * NETA + v4 * VW) = v;
                 }
+            optr += PLANE;   // carried from plane to plane: the 64-bit address is not rebuilt (15 instructions) every plane
             if (mom) {
                 // sum_ab xi_a m and sum_ab eta_b m over the lane's patch, with xi_a = xi_a0 + q dxi, eta_b = eta_b0 + cb
                 // deta: S = sum m, fxp = xi_a0 S + dxi sum_q q rs_q, fyp = eta_b0 S + deta sum_cb cb cs_cb -- two
