@@ -499,7 +499,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
         }
 
         mbar_wait(&full[slot], phase);
-        const real *sp = ring + (size_t)slot * P * PLANE;
+        const real *sp = ring + (size_t)slot * P * PLANE + a0 * NETA + b0;   // this lane's first cell; advanced plane by plane
 #pragma unroll 1
         for (int pl = 0; pl < P; ++pl) {
             const int j = ch * P + pl;
@@ -563,7 +563,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             for (int q = 0; q < QA; ++q)
 #pragma unroll
                 for (int v4 = 0; v4 < CB / VW; ++v4) {
-                    const V128 v = *reinterpret_cast<const V128 *>(sp + pl * PLANE + (a0 + q) * NETA + b0 + v4 * VW);
+                    const V128 v = *reinterpret_cast<const V128 *>(sp + q * NETA + v4 * VW);
 #pragma unroll
                     for (int e = 0; e < VW; ++e) x[q][v4 * VW + e] = v.v[e];
                 }
@@ -595,6 +595,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     for (int e = 0; e < VW; ++e) v.v[e] = x[q][v4 * VW + e];
                     *reinterpret_cast<V128 *>(optr + q * NETA + v4 * VW) = v;
                 }
+            sp += PLANE;
             optr += PLANE;   // carried from plane to plane: the 64-bit address is not rebuilt (15 instructions) every plane
             if (mom) {
                 // sum_ab xi_a m and sum_ab eta_b m over the lane's patch, with xi_a = xi_a0 + q dxi, eta_b = eta_b0 + cb
