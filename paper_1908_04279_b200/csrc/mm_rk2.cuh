@@ -403,8 +403,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
                     V128 v;
 #pragma unroll
                     for (int e = 0; e < VW; ++e) v.v[e] = o[q][v4 * VW + e];
-                    *reinterpret_cast<V128 *>(oc + (int64_t)j2 * PLANE + (a0 + q) * NETA + b0 + v4 * VW) = v;
+                    *reinterpret_cast<V128 *>(oc + q * NETA + v4 * VW) = v;
                 }
+            oc += PLANE;   // this lane's first cell of the next plane stored (carried: the 64-bit address is not rebuilt)
             if (mom) {   // S9 partial sums of the new density
                 const real sj2 = kp.s_lo + (real(j2) + real(0.5)) * kp.ds;
                 real fxp = 0, fyp = 0;
@@ -468,7 +469,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
     for (int64_t it = 0; it < total; ++it) {
         if (ch == 0) {
             c = gw + k * nw;
-            oc = out + c * inner;
+            oc = out + c * inner + a0 * NETA + b0;
             const int kth = (int)(c % kp.ntheta);
             const real ct = kp.cos_t[kth], st = kp.sin_t[kth];
             ctc = ct; stc = st;
